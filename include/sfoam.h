@@ -1,0 +1,131 @@
+/* sfoam.h -- C ABI of libsfoam: the EPRL vertex-amplitude tensor of arXiv 2107.13952 on one B200 (sm_100a).
+ *
+ * What is computed (eq. (3)):
+ *
+ *   A[i1..i5] = prod_{e=1..5} sqrt(2 i_e+1) *
+ *               sum_{shells l_f} sum_{k2..k5} prod_{a=2..5} (2 k_a+1) B_a[t_a(l)][i_a,k_a] * {15j}(l_f; i1,k2..k5)
+ *
+ * with the {15j} symbol of eq. (5) assembled from five {6j} symbols, the shells
+ * j_f <= l_f <= j_f + Delta_l of the six virtual spins (l23 l24 l25 l34 l35 l45), l_1a = j_1a gauge-fixed, and the
+ * four booster tensors B_a supplied by the caller (they are inputs: PAPER.md:169-171).  The steps are those of the
+ * vertex-tensor algorithm.
+ *
+ * Conventions
+ *   - Every spin is passed as the integer two_j = 2j.  two_dl = 2*Delta_l must be even (virtual spins step by 1).
+ *   - Spin order  two_j[10] = (j12 j13 j14 j15 j23 j24 j25 j34 j35 j45)   (Listing 8).
+ *   - Node spin orders (first pair | second pair); the node's intertwiner recouples the two pairs:
+ *       node 1 (j12 j13 | j14 j15) -> i1        node 2 (j23 j24 | j25 j12) -> i2,k2     node 3 (j34 j35 | j13 j23) -> i3,k3
+ *       node 4 (j45 j14 | j24 j34) -> i4,k4     node 5 (j15 j25 | j35 j45) -> i5,k5
+ *   - Canonical shell order: lexicographic in the offsets (o23 o24 o25 o34 o35 o45), o = l - j in 0..Delta_l,
+ *     o45 fastest (index order of eq. (9)).  shell = ((((o23*n+o24)*n+o25)*n+o34)*n+o35)*n+o45, n = Delta_l+1.
+ *   - Booster layout (dense, C row-major, FP64, DEVICE memory):  B_a[t][ii][kk],  a = 2..5,
+ *       t  = (u*n+v)*n+w with (u,v,w) the offsets of the edge's virtual spins in the paper's superscript order
+ *            (PAPER.md:171): edge 2 (l23 l24 l25), edge 3 (l34 l35 l23), edge 4 (l45 l24 l34), edge 5 (l25 l35 l45);
+ *       ii = (two_i - two_i_min_a)/2 in [0,n_i);  kk = (two_k - two_k_base_a)/2 in [0,n_k_pad), sizes from
+ *            sf_booster_dims().  Entries outside the triple's valid k-range are ignored (treated as 0).
+ *   - Output layout: out[(((a1*n2+a2)*n3+a3)*n4+a4)*n5+a5], a_e = (two_i_e - two_i_min_e)/2: the same bytes as the
+ *     paper's column-major A^{i5 i4 i3 i2 i1}.
+ *   - The result is bitwise reproducible run to run for identical inputs (fixed-order accumulation, no float atomics).
+ *
+ * Ownership: the caller owns booster and output buffers; the library owns the {6j} table and its scratch memory
+ * (released by sf_finalize).  All functions return SF_OK (0) or a negative sf_status; none throws or aborts; `out` is
+ * not written when an error is returned before launch.  There is NO CPU fallback: without a CUDA device every compute
+ * entry point returns SF_ECUDA.
+ */
+#ifndef SFOAM_H
+#define SFOAM_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    SF_OK       = 0,
+    SF_ENOTINIT = -1,   /* sf_init has not been called                                                   */
+    SF_EARG     = -2,   /* null pointer, negative spin, two_dl negative or odd, bad edge / range           */
+    SF_ESPIN    = -3,   /* a boundary node's four spins have an odd sum or an empty intertwiner range      */
+    SF_ETABLE   = -4,   /* {6j} table requested but absent / too small                                     */
+    SF_ENOMEM   = -5,   /* host or device allocation failed                                                */
+    SF_ECUDA    = -6    /* CUDA runtime error (no device, launch failure)                                  */
+} sf_status;
+
+/* CUDA stream handle (a cudaStream_t), passed as an opaque pointer so that this header needs no CUDA include. */
+typedef void *sf_stream_t;
+
+/* The four booster tensors of step 3: DEVICE pointers, edges 2,3,4,5 in B[0..3]. */
+typedef struct {
+    const double *B[4];
+} sf_boosters;
+
+/* Create the global context on the current CUDA device.  gamma is the Immirzi parameter the paper's cinit() takes
+ * (PAPER.md:207-219); with caller-supplied boosters the path does not depend on it (it enters only through B4,
+ * PAPER.md:61-65), so it is stored and reported back, nothing else.  Idempotent. */
+int sf_init(double gamma);
+int sf_finalize(void);
+const char *sf_strerror(int status);
+double sf_gamma(void);
+
+/* Build (or replace) the device-resident table of all {6j} symbols with every 2j <= two_jmax, one slot per class
+ * of the 24 tetrahedral symmetries (the paper precomputes 6j tables: PAPER.md:103, 207).  two_jmax < 0 frees it.
+ * While a table is resident, the S arrays of step 4 are gathered from it when every argument fits, and evaluated
+ * directly otherwise.  Returns SF_EARG for two_jmax > 100 (table would exceed 24 GB). */
+int sf_sixj_table(int two_jmax);
+/* Number of slots of the resident table (0 if none), and its two_jmax (-1 if none). */
+long sf_sixj_table_slots(void);
+int sf_sixj_table_two_jmax(void);
+
+/* Test hooks for {6j} parity.  two_j6 = (a b c d e f) for {a b c; d e f}; HOST pointers.
+ * sf_sixj_get evaluates one symbol on the device (direct Racah sum).  sf_sixj_batch evaluates n symbols;
+ * mode 0 = direct evaluation, mode 1 = gather from the resident table (SF_ETABLE if absent or an argument exceeds it). */
+int sf_sixj_get(const int two_j6[6], double *host_out);
+int sf_sixj_batch(const int *two_j6, long n, int mode, double *host_out);
+
+/* Pure host integer helpers (step 2): boundary intertwiner ranges of nodes 1..5. */
+int sf_vertex_dims(const int two_j[10], int two_i_min[5], int n_i[5]);
+/* Booster tensor dims of edge a in 2..5: number of triples (Delta_l+1)^3, n_i, and the padded k layout. */
+int sf_booster_dims(const int two_j[10], int two_dl, int edge, int *n_triples, int *n_i, int *two_k_base, int *n_k_pad);
+/* Valid k-range of triple t of edge a (n_k = 0 if empty). */
+int sf_booster_krange(const int two_j[10], int two_dl, int edge, int t, int *two_k_min, int *n_k);
+/* The same for all (Delta_l+1)^3 triples of the edge at once: two_k_min[t], n_k[t]. */
+int sf_booster_kranges(const int two_j[10], int two_dl, int edge, int *two_k_min, int *n_k);
+
+/* Algorithmic work of shells [shell_lo, shell_hi) counted on valid ranges only:
+ *   *f_con = sum over shells of 2*(n1 K2 K3 K4 K5 n5 + n1 K2 K3 K4 n4 n5 + n1 K2 K3 n3 n4 n5 + n1 K2 n2 n3 n4 n5)
+ *   *n_nonempty = shells with all four k-ranges non-empty;  *n_w = sum over shells of n1 K2 K3 K4 K5.
+ * Host integer function. */
+int sf_vertex_work(const int two_j[10], int two_dl, long shell_lo, long shell_hi,
+                   double *f_con, long *n_nonempty, double *n_w);
+
+/* The vertex tensor (steps 4-7).  boosters / out: DEVICE pointers; out holds prod(n_i) doubles and
+ * is overwritten.  Asynchronous w.r.t. the host, ordered on `stream`.  Requires sf_init. */
+int sf_vertex_amplitude(const int two_j[10], int two_dl, const sf_boosters *boosters, double *out, sf_stream_t stream);
+/* Same, restricted to shells [shell_lo, shell_hi) of the canonical order (the full call is [0,(Delta_l+1)^6)).
+ * Ranges are additive: the sum of the outputs over a partition of the shells equals the full tensor up to rounding. */
+int sf_vertex_amplitude_range(const int two_j[10], int two_dl, const sf_boosters *boosters,
+                              long shell_lo, long shell_hi, double *out, sf_stream_t stream);
+/* End-to-end variant with HOST buffers (pinned or pageable): copies the four boosters to the device, computes, copies
+ * the tensor back and synchronises `stream`.  host_boosters[e] holds n_triples*n_i*n_k_pad doubles. */
+int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const double *const host_boosters[4],
+                             double *host_out, sf_stream_t stream);
+
+/* Number of kernels the library launched since sf_init / the last reset (bench.py's gpu_launches). */
+long sf_launch_count(int reset);
+/* Milliseconds of device time (CUDA events on the call's stream) spent in each stage of the LAST vertex call,
+ * recorded when sf_set_timing(1) is on: [0] S arrays (step 4), [1] assembly + contraction (steps 5-6(iii)),
+ * [2] accumulation (step 6(iv) + normalisation).  Enabling timing makes the vertex calls synchronous. */
+int sf_set_timing(int on);
+int sf_last_stage_ms(double ms[3]);
+
+/* Path selection for steps 5-7.  0 = automatic: the fused on-chip path when one i1-slice of the tensor fits the SM
+ * (accumulators in registers, intermediates in shared memory), the staged path (intermediates through global memory,
+ * split along i1 when needed: PAPER.md:184-186) otherwise.  1 = staged, 2 = fused (the vertex calls then return
+ * SF_EARG for tensors the fused path cannot hold).  sf_last_path() = path the last vertex call took (1 or 2). */
+int sf_set_path(int path);
+int sf_last_path(void);
+/* Bytes of global scratch the staged path may use for its two ping-pong buffers (default 6 GiB). */
+void sf_set_staged_budget(unsigned long bytes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFOAM_H */

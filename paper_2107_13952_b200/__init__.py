@@ -1,0 +1,244 @@
+"""sfoam-b200: thin Python binding of libsfoam.so, the C-ABI CUDA library declared in include/sfoam.h.
+
+Argument marshalling only: every step of the path (the {6j} table, the S arrays, the {15j} assembly, the mode
+products and the shell accumulation) runs in the library's CUDA kernels.  PyTorch tensors are used for device memory
+and streams; any object with `data_ptr()` (device) works.  There is no CPU fallback: if the library has not been
+built, or no CUDA device is present, the calls raise.
+
+Function names are those of the header; spins are 2j integers; `two_j` has the order
+(j12 j13 j14 j15 j23 j24 j25 j34 j35 j45) of Listing 8 of the paper.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsfoam.so")
+
+SF_OK, SF_ENOTINIT, SF_EARG, SF_ESPIN, SF_ETABLE, SF_ENOMEM, SF_ECUDA = 0, -1, -2, -3, -4, -5, -6
+
+
+class SfError(RuntimeError):
+    def __init__(self, status, what):
+        self.status = status
+        super().__init__(f"{what}: {_lib().sf_strerror(status).decode()} ({status})")
+
+
+class _Boosters(ctypes.Structure):
+    _fields_ = [("B", ctypes.c_void_p * 4)]
+
+
+_LIB = None
+_I10 = ctypes.c_int * 10
+_I5 = ctypes.c_int * 5
+_I6 = ctypes.c_int * 6
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2107_13952_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        lib.sf_strerror.restype = ctypes.c_char_p
+        lib.sf_gamma.restype = ctypes.c_double
+        lib.sf_init.argtypes = [ctypes.c_double]
+        lib.sf_sixj_table_slots.restype = ctypes.c_long
+        lib.sf_launch_count.restype = ctypes.c_long
+        lib.sf_sixj_batch.argtypes = [ctypes.c_void_p, ctypes.c_long, ctypes.c_int, ctypes.c_void_p]
+        lib.sf_vertex_work.argtypes = [_I10, ctypes.c_int, ctypes.c_long, ctypes.c_long,
+                                       ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_long),
+                                       ctypes.POINTER(ctypes.c_double)]
+        lib.sf_vertex_amplitude.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_void_p,
+                                            ctypes.c_void_p]
+        lib.sf_vertex_amplitude_range.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_long,
+                                                  ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
+        lib.sf_vertex_amplitude_host.argtypes = [_I10, ctypes.c_int, ctypes.c_void_p * 4, ctypes.c_void_p,
+                                                 ctypes.c_void_p]
+        lib.sf_set_staged_budget.argtypes = [ctypes.c_size_t]
+        _LIB = lib
+    return _LIB
+
+
+def _check(status, what):
+    if status != SF_OK:
+        raise SfError(status, what)
+
+
+def _spins(two_j):
+    if len(two_j) != 10:
+        raise ValueError("two_j must hold the ten boundary spins (12 13 14 15 23 24 25 34 35 45)")
+    return _I10(*[int(s) for s in two_j])
+
+
+def _ptr(t):
+    return ctypes.c_void_p(t.data_ptr() if hasattr(t, "data_ptr") else int(t))
+
+
+def _stream(stream):
+    if stream is None:
+        return ctypes.c_void_p(0)
+    return ctypes.c_void_p(getattr(stream, "cuda_stream", stream))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# context
+# ---------------------------------------------------------------------------------------------------------------
+def sf_init(gamma):
+    _check(_lib().sf_init(float(gamma)), "sf_init")
+
+
+def sf_finalize():
+    _check(_lib().sf_finalize(), "sf_finalize")
+
+
+def sf_gamma():
+    return _lib().sf_gamma()
+
+
+def sf_strerror(status):
+    return _lib().sf_strerror(int(status)).decode()
+
+
+def sf_launch_count(reset=False):
+    return int(_lib().sf_launch_count(int(bool(reset))))
+
+
+def sf_set_timing(on):
+    _check(_lib().sf_set_timing(int(bool(on))), "sf_set_timing")
+
+
+def sf_last_stage_ms():
+    ms = (ctypes.c_double * 3)()
+    _check(_lib().sf_last_stage_ms(ms), "sf_last_stage_ms")
+    return list(ms)
+
+
+def sf_set_path(path):
+    """0 = automatic, 1 = staged (general sizes), 2 = fused on-chip path (raises SF_EARG at call time if too large)."""
+    _check(_lib().sf_set_path(int(path)), "sf_set_path")
+
+
+def sf_last_path():
+    return int(_lib().sf_last_path())
+
+
+def sf_set_staged_budget(nbytes):
+    _lib().sf_set_staged_budget(int(nbytes))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# {6j}
+# ---------------------------------------------------------------------------------------------------------------
+def sf_sixj_table(two_jmax):
+    _check(_lib().sf_sixj_table(int(two_jmax)), "sf_sixj_table")
+
+
+def sf_sixj_table_slots():
+    return int(_lib().sf_sixj_table_slots())
+
+
+def sf_sixj_table_two_jmax():
+    return int(_lib().sf_sixj_table_two_jmax())
+
+
+def sf_sixj_get(two_j6):
+    out = ctypes.c_double()
+    _check(_lib().sf_sixj_get(_I6(*[int(s) for s in two_j6]), ctypes.byref(out)), "sf_sixj_get")
+    return out.value
+
+
+def sf_sixj_batch(two_j6, mode=0):
+    """two_j6: int array [n, 6] of (a b c d e f) for {a b c; d e f}.  mode 0 = direct evaluation, 1 = table gather."""
+    args = np.ascontiguousarray(two_j6, dtype=np.int32).reshape(-1, 6)
+    out = np.empty(len(args), dtype=np.float64)
+    _check(_lib().sf_sixj_batch(args.ctypes.data, len(args), int(mode), out.ctypes.data), "sf_sixj_batch")
+    return out
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# host integer helpers
+# ---------------------------------------------------------------------------------------------------------------
+def sf_vertex_dims(two_j):
+    lo, n = _I5(), _I5()
+    _check(_lib().sf_vertex_dims(_spins(two_j), lo, n), "sf_vertex_dims")
+    return list(lo), list(n)
+
+
+def sf_booster_dims(two_j, two_dl, edge):
+    """(n_triples, n_i, two_k_base, n_k_pad) of the dense booster tensor B_edge[t][ii][kk]."""
+    v = [ctypes.c_int() for _ in range(4)]
+    _check(_lib().sf_booster_dims(_spins(two_j), int(two_dl), int(edge), *[ctypes.byref(x) for x in v]),
+           "sf_booster_dims")
+    return tuple(x.value for x in v)
+
+
+def sf_booster_krange(two_j, two_dl, edge, t):
+    lo, n = ctypes.c_int(), ctypes.c_int()
+    _check(_lib().sf_booster_krange(_spins(two_j), int(two_dl), int(edge), int(t), ctypes.byref(lo), ctypes.byref(n)),
+           "sf_booster_krange")
+    return lo.value, n.value
+
+
+def sf_booster_kranges(two_j, two_dl, edge):
+    """[(two_k_min, n_k)] for every triple t of the edge."""
+    nt = (int(two_dl) // 2 + 1) ** 3
+    lo, n = (ctypes.c_int * nt)(), (ctypes.c_int * nt)()
+    _check(_lib().sf_booster_kranges(_spins(two_j), int(two_dl), int(edge), lo, n), "sf_booster_kranges")
+    return list(zip(lo, n))
+
+
+def sf_vertex_work(two_j, two_dl, shell_lo=0, shell_hi=None):
+    """dict(f_con, n_nonempty, n_w): algorithmic contraction flops, non-empty shells, W entries of the shell range."""
+    if shell_hi is None:
+        shell_hi = (int(two_dl) // 2 + 1) ** 6
+    f, ne, nw = ctypes.c_double(), ctypes.c_long(), ctypes.c_double()
+    _check(_lib().sf_vertex_work(_spins(two_j), int(two_dl), int(shell_lo), int(shell_hi), ctypes.byref(f),
+                                 ctypes.byref(ne), ctypes.byref(nw)), "sf_vertex_work")
+    return {"f_con": f.value, "n_nonempty": ne.value, "n_w": nw.value}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the vertex tensor
+# ---------------------------------------------------------------------------------------------------------------
+def _boosters(boosters):
+    if isinstance(boosters, dict):
+        boosters = [boosters[e] for e in (2, 3, 4, 5)]
+    if len(boosters) != 4:
+        raise ValueError("need the four booster tensors of edges 2..5")
+    b = _Boosters()
+    for e, t in enumerate(boosters):
+        b.B[e] = t.data_ptr() if hasattr(t, "data_ptr") else int(t)
+    return b
+
+
+def sf_vertex_amplitude(two_j, two_dl, boosters, out, stream=None):
+    """boosters: four DEVICE float64 tensors B_a[t][ii][kk] (edges 2..5; list or {2:..,5:..}); out: DEVICE float64
+    tensor of prod(n_i) elements, overwritten with A[i1][i2][i3][i4][i5].  Asynchronous on `stream`."""
+    b = _boosters(boosters)
+    _check(_lib().sf_vertex_amplitude(_spins(two_j), int(two_dl), ctypes.byref(b), _ptr(out), _stream(stream)),
+           "sf_vertex_amplitude")
+    return out
+
+
+def sf_vertex_amplitude_range(two_j, two_dl, boosters, shell_lo, shell_hi, out, stream=None):
+    b = _boosters(boosters)
+    _check(_lib().sf_vertex_amplitude_range(_spins(two_j), int(two_dl), ctypes.byref(b), int(shell_lo), int(shell_hi),
+                                            _ptr(out), _stream(stream)), "sf_vertex_amplitude_range")
+    return out
+
+
+def sf_vertex_amplitude_host(two_j, two_dl, host_boosters, host_out, stream=None):
+    """End-to-end variant: host_boosters are four HOST float64 arrays (numpy, or pinned torch CPU tensors), host_out
+    a HOST float64 array; copies in, computes, copies back and synchronises."""
+    if isinstance(host_boosters, dict):
+        host_boosters = [host_boosters[e] for e in (2, 3, 4, 5)]
+    arr = (ctypes.c_void_p * 4)()
+    for e, t in enumerate(host_boosters):
+        arr[e] = t.data_ptr() if hasattr(t, "data_ptr") else t.ctypes.data
+    optr = host_out.data_ptr() if hasattr(host_out, "data_ptr") else host_out.ctypes.data
+    _check(_lib().sf_vertex_amplitude_host(_spins(two_j), int(two_dl), arr, ctypes.c_void_p(optr), _stream(stream)),
+           "sf_vertex_amplitude_host")
+    return host_out

@@ -1,0 +1,283 @@
+// sf_api.cu -- the C ABI of libsfoam (include/sfoam.h): context, scratch memory, and the vertex entry points that
+// string the steps of the vertex-tensor algorithm together.
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "sf_internal.h"
+
+#define SF_NSCRATCH 24
+enum { SLOT_ACC = 0, SLOT_BUF0 = 1, SLOT_BUF1 = 2, SLOT_S = 3 /*..7*/, SLOT_KR = 8 /*..11*/, SLOT_HB = 12 /*..15*/,
+       SLOT_HOUT = 16, SLOT_PART = 17, SLOT_MISC = 18 };
+
+struct SfContext {
+    bool init = false;
+    double gamma = 0.0;
+    void* scratch[SF_NSCRATCH] = {};
+    size_t scratch_bytes[SF_NSCRATCH] = {};
+    long launches = 0;
+    int path = 0;          // 0 auto, 1 staged, 2 fused
+    int last_path = 0;
+    bool timing = false;
+    cudaEvent_t ev[4] = {};
+    double stage_ms[3] = {};
+};
+static SfContext g_ctx;
+
+void sf_count_launch(int n) { g_ctx.launches += n; }
+
+void* sf_scratch(int slot, size_t bytes)
+{
+    if (slot < 0 || slot >= SF_NSCRATCH) return nullptr;
+    if (bytes == 0) bytes = 8;
+    if (g_ctx.scratch_bytes[slot] >= bytes) return g_ctx.scratch[slot];
+    if (g_ctx.scratch[slot]) {
+        cudaDeviceSynchronize();   // the old block may still be in use on a stream
+        cudaFree(g_ctx.scratch[slot]);
+        g_ctx.scratch[slot] = nullptr;
+        g_ctx.scratch_bytes[slot] = 0;
+    }
+    void* p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    g_ctx.scratch[slot] = p;
+    g_ctx.scratch_bytes[slot] = bytes;
+    return p;
+}
+
+void sf_timing_mark(int idx, cudaStream_t st)
+{
+    if (g_ctx.timing && idx >= 0 && idx < 4) cudaEventRecord(g_ctx.ev[idx], st);
+}
+
+extern "C" int sf_init(double gamma)
+{
+    if (g_ctx.init) {
+        g_ctx.gamma = gamma;
+        return SF_OK;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return SF_ECUDA;   // no CPU fallback
+    }
+    int rc = sf_sixj_module_init();
+    if (rc != SF_OK) return rc;
+    for (int q = 0; q < 4; ++q)
+        if (cudaEventCreate(&g_ctx.ev[q]) != cudaSuccess) return SF_ECUDA;
+    g_ctx.gamma = gamma;
+    g_ctx.init = true;
+    g_ctx.launches = 0;
+    return SF_OK;
+}
+
+extern "C" int sf_finalize(void)
+{
+    if (!g_ctx.init) return SF_OK;
+    cudaDeviceSynchronize();
+    for (int s = 0; s < SF_NSCRATCH; ++s) {
+        if (g_ctx.scratch[s]) cudaFree(g_ctx.scratch[s]);
+        g_ctx.scratch[s] = nullptr;
+        g_ctx.scratch_bytes[s] = 0;
+    }
+    sf_sixj_module_free();
+    for (int q = 0; q < 4; ++q) cudaEventDestroy(g_ctx.ev[q]);
+    g_ctx.init = false;
+    return SF_OK;
+}
+
+extern "C" double sf_gamma(void) { return g_ctx.gamma; }
+
+extern "C" const char* sf_strerror(int status)
+{
+    switch (status) {
+        case SF_OK: return "ok";
+        case SF_ENOTINIT: return "sf_init has not been called";
+        case SF_EARG: return "invalid argument";
+        case SF_ESPIN: return "a boundary node has an odd spin sum or an empty intertwiner range";
+        case SF_ETABLE: return "6j table absent or too small";
+        case SF_ENOMEM: return "out of memory";
+        case SF_ECUDA: return "CUDA error (no device or launch failure)";
+        default: return "unknown status";
+    }
+}
+
+extern "C" int sf_sixj_table(int two_jmax)
+{
+    if (!g_ctx.init) return SF_ENOTINIT;
+    return sf_sixj_table_build(two_jmax, 0);
+}
+
+extern "C" long sf_launch_count(int reset)
+{
+    long n = g_ctx.launches;
+    if (reset) g_ctx.launches = 0;
+    return n;
+}
+
+extern "C" int sf_set_timing(int on)
+{
+    g_ctx.timing = on != 0;
+    return SF_OK;
+}
+extern "C" int sf_last_stage_ms(double ms[3])
+{
+    if (!ms) return SF_EARG;
+    memcpy(ms, g_ctx.stage_ms, sizeof g_ctx.stage_ms);
+    return SF_OK;
+}
+// 0 = automatic (fused on-chip path when the tensor fits, staged path otherwise), 1 = staged, 2 = fused
+extern "C" int sf_set_path(int path)
+{
+    if (path < 0 || path > 2) return SF_EARG;
+    g_ctx.path = path;
+    return SF_OK;
+}
+extern "C" int sf_last_path(void) { return g_ctx.last_path; }
+
+// ranges of the virtual intertwiners k_a for every booster triple (step 2): the node's recoupling
+// pairs with the edge's three virtual spins at l = j + offset (superscript order of PAPER.md:171)
+__global__ void k_kranges(SfProblem P, int nt, SfKRange* __restrict__ out)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= 4 * nt) return;
+    const int e = q / nt, t = q % nt, nl = P.nl;
+    const int u = 2 * (t / (nl * nl)), v = 2 * ((t / nl) % nl), w = 2 * (t % nl);
+    const int* j = P.two_j;
+    int a, b, c, d;
+    if (e == 0) {          // node 2 (l23 l24 | l25 j12), triple (l23 l24 l25)
+        a = j[J23] + u; b = j[J24] + v; c = j[J25] + w; d = j[J12];
+    } else if (e == 1) {   // node 3 (l34 l35 | j13 l23), triple (l34 l35 l23)
+        a = j[J34] + u; b = j[J35] + v; c = j[J13]; d = j[J23] + w;
+    } else if (e == 2) {   // node 4 (l45 j14 | l24 l34), triple (l45 l24 l34)
+        a = j[J45] + u; b = j[J14]; c = j[J24] + v; d = j[J34] + w;
+    } else {               // node 5 (j15 l25 | l35 l45), triple (l25 l35 l45)
+        a = j[J15]; b = j[J25] + u; c = j[J35] + v; d = j[J45] + w;
+    }
+    const int lo = max(abs(a - b), abs(c - d)), hi = min(a + b, c + d);
+    SfKRange r;
+    r.two_k_min = lo;
+    r.n_k = (((a + b) ^ (c + d)) & 1) || hi < lo ? 0 : (hi - lo) / 2 + 1;
+    out[q] = r;
+}
+
+static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo, long shell_hi,
+                        double* out, cudaStream_t st, bool full)
+{
+    if (!g_ctx.init) return SF_ENOTINIT;
+    if (!two_j || !boosters || !out) return SF_EARG;
+    for (int e = 0; e < 4; ++e)
+        if (!boosters->B[e]) return SF_EARG;
+    SfDims D;
+    int rc = sf_host_dims(two_j, two_dl, &D);
+    if (rc != SF_OK) return rc;
+    if (full) {
+        shell_lo = 0;
+        shell_hi = D.n_shells;
+    }
+    if (shell_lo < 0 || shell_hi > D.n_shells || shell_lo > shell_hi) return SF_EARG;
+    // largest factorial argument of any 6j on the path stays inside the table of sf_sixj.cuh
+    {
+        int m = 0;
+        for (int s = 0; s < 10; ++s) m = two_j[s] > m ? two_j[s] : m;
+        if (2 * (m + two_dl) + 2 >= 1000) return SF_EARG;
+    }
+
+    SfProblem P;
+    memcpy(P.two_j, D.two_j, sizeof P.two_j);
+    P.nl = D.nl;
+    memcpy(P.two_i_min, D.two_i_min, sizeof P.two_i_min);
+    memcpy(P.n_i, D.n_i, sizeof P.n_i);
+    memcpy(P.two_k_base, D.two_k_base, sizeof P.two_k_base);
+    memcpy(P.n_k_pad, D.n_k_pad, sizeof P.n_k_pad);
+    memcpy(P.k_max, D.k_max, sizeof P.k_max);
+    P.two_x_base = D.two_x_base;
+    P.n_x_pad = D.n_x_pad;
+    for (int e = 0; e < 4; ++e) P.B[e] = boosters->B[e];
+
+    // step 2: per-triple k-range tables, computed on the device (no host->device copy on the call path)
+    const int nt = D.nl * D.nl * D.nl;
+    {
+        SfKRange* d = (SfKRange*)sf_scratch(SLOT_KR, sizeof(SfKRange) * nt * 4);
+        if (!d) return SF_ENOMEM;
+        for (int e = 0; e < 4; ++e) P.kr[e] = d + (long)e * nt;
+        k_kranges<<<(4 * nt + 127) / 128, 128, 0, st>>>(P, nt, d);
+        sf_count_launch(1);
+    }
+
+    // step 4: the five S arrays
+    SfSliceSizes sz;
+    sf_slice_sizes(D, &sz);
+    double* S[5];
+    for (int w = 0; w < 5; ++w) {
+        S[w] = (double*)sf_scratch(SLOT_S + w, sizeof(double) * sz.n[w]);
+        if (!S[w]) return SF_ENOMEM;
+        P.S[w] = S[w];
+    }
+    sf_timing_mark(0, st);
+    rc = sf_build_slices(D, S, sf_sixj_table_get(), st);
+    if (rc != SF_OK) return rc;
+    sf_timing_mark(1, st);
+
+    // steps 5-7
+    const bool fused_ok = sf_vertex_fused_supported(D);
+    if (g_ctx.path == 2 && !fused_ok) return SF_EARG;
+    const bool use_fused = g_ctx.path == 2 || (g_ctx.path == 0 && fused_ok);
+    g_ctx.last_path = use_fused ? 2 : 1;
+    rc = use_fused ? sf_vertex_fused(D, P, shell_lo, shell_hi, out, st) : sf_vertex_staged(D, P, shell_lo, shell_hi, out, st);
+    if (rc != SF_OK) return rc;
+    sf_timing_mark(3, st);
+    if (g_ctx.timing) {
+        SF_CUDA_OK(cudaEventSynchronize(g_ctx.ev[3]));
+        float a = 0, b = 0, c = 0;
+        cudaEventElapsedTime(&a, g_ctx.ev[0], g_ctx.ev[1]);
+        cudaEventElapsedTime(&b, g_ctx.ev[1], g_ctx.ev[2]);
+        cudaEventElapsedTime(&c, g_ctx.ev[2], g_ctx.ev[3]);
+        g_ctx.stage_ms[0] = a;
+        g_ctx.stage_ms[1] = b;
+        g_ctx.stage_ms[2] = c;
+    }
+    return SF_OK;
+}
+
+extern "C" int sf_vertex_amplitude(const int two_j[10], int two_dl, const sf_boosters* boosters, double* out,
+                                   sf_stream_t stream)
+{
+    return vertex_range(two_j, two_dl, boosters, 0, 0, out, (cudaStream_t)stream, true);
+}
+
+extern "C" int sf_vertex_amplitude_range(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo,
+                                         long shell_hi, double* out, sf_stream_t stream)
+{
+    return vertex_range(two_j, two_dl, boosters, shell_lo, shell_hi, out, (cudaStream_t)stream, false);
+}
+
+extern "C" int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const double* const host_boosters[4],
+                                        double* host_out, sf_stream_t stream)
+{
+    if (!g_ctx.init) return SF_ENOTINIT;
+    if (!two_j || !host_boosters || !host_out) return SF_EARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    SfDims D;
+    int rc = sf_host_dims(two_j, two_dl, &D);
+    if (rc != SF_OK) return rc;
+    const long nt = (long)D.nl * D.nl * D.nl;
+    sf_boosters b;
+    for (int e = 0; e < 4; ++e) {
+        if (!host_boosters[e]) return SF_EARG;
+        const size_t bytes = sizeof(double) * nt * D.n_i[e + 1] * D.n_k_pad[e];
+        double* d = (double*)sf_scratch(SLOT_HB + e, bytes);
+        if (!d) return SF_ENOMEM;
+        SF_CUDA_OK(cudaMemcpyAsync(d, host_boosters[e], bytes, cudaMemcpyHostToDevice, st));
+        b.B[e] = d;
+    }
+    double* dout = (double*)sf_scratch(SLOT_HOUT, sizeof(double) * D.n_out);
+    if (!dout) return SF_ENOMEM;
+    rc = vertex_range(two_j, two_dl, &b, 0, 0, dout, st, true);
+    if (rc != SF_OK) return rc;
+    SF_CUDA_OK(cudaMemcpyAsync(host_out, dout, sizeof(double) * D.n_out, cudaMemcpyDeviceToHost, st));
+    SF_CUDA_OK(cudaStreamSynchronize(st));
+    return SF_OK;
+}

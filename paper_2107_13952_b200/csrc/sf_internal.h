@@ -1,0 +1,108 @@
+// sf_internal.h -- internal declarations of libsfoam (CUDA path).  Not part of the C ABI (include/sfoam.h is).
+//
+// Notation follows the paper (arXiv 2107.13952): boundary spins j_ab, virtual spins l_ab, boundary intertwiners i_e,
+// virtual intertwiners k_e, recoupling spin x of eq. (5).  All spins are integers two_* = 2*spin.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sfoam.h"
+
+// spin order of two_j[10] (Listing 8)
+enum { J12 = 0, J13, J14, J15, J23, J24, J25, J34, J35, J45 };
+
+// -------------------------------------------------------------------------------------------------------------
+// Host-side description of one vertex problem (steps 1-2 of the algorithm)
+// -------------------------------------------------------------------------------------------------------------
+struct SfDims {
+    int two_j[10];
+    int two_dl, nl;                 // nl = Delta_l + 1
+    long n_shells;                  // nl^6
+    int two_i_min[5], n_i[5];       // boundary intertwiner ranges, nodes 1..5
+    int two_k_base[4], n_k_pad[4];  // booster k layout of edges 2..5 (union over triples)
+    int k_max[4];                   // largest n_k over the triples of each edge
+    int two_x_base, n_x_pad;        // union range of the recoupling spin x (triad (i1 l25 x))
+    long n_out;                     // prod n_i
+};
+
+// per-triple k-range tables, kr[e][t] = (two_k_min, n_k), e = 0..3 for edges 2..5
+struct SfKRange {
+    int two_k_min, n_k;
+};
+
+int sf_host_pair_range(int a, int b, int c, int d, int* lo);           // count, *lo = minimum
+int sf_host_dims(const int two_j[10], int two_dl, SfDims* D);          // SF_OK / SF_EARG / SF_ESPIN
+void sf_host_kranges(const SfDims& D, int e, SfKRange* out);           // out[nl^3]
+void sf_host_shell_offsets(const SfDims& D, long shell, int o[6]);
+
+// -------------------------------------------------------------------------------------------------------------
+// Device-side problem descriptor, passed by value to every vertex kernel
+// -------------------------------------------------------------------------------------------------------------
+struct SfProblem {
+    int two_j[10];
+    int nl;
+    int two_i_min[5], n_i[5];
+    int two_k_base[4], n_k_pad[4], k_max[4];
+    int two_x_base, n_x_pad;
+    const SfKRange* kr[4];        // device: per edge, nl^3 entries
+    const double* S[5];           // device: S1..S5, layouts in sf_slices.cu
+    const double* B[4];           // device: caller's boosters, edges 2..5
+};
+
+// shell -> offsets (o23 o24 o25 o34 o35 o45), o45 fastest (eq. (9))
+__host__ __device__ inline void sf_shell_offsets(long shell, int nl, int o[6])
+{
+    for (int q = 5; q >= 0; --q) {
+        o[q] = (int)(shell % nl);
+        shell /= nl;
+    }
+}
+// booster triple indices in the paper's superscript order
+__host__ __device__ inline void sf_triples(const int o[6], int nl, int t[4])
+{
+    t[0] = (o[0] * nl + o[1]) * nl + o[2];   // edge 2: (l23 l24 l25)
+    t[1] = (o[3] * nl + o[4]) * nl + o[0];   // edge 3: (l34 l35 l23)
+    t[2] = (o[5] * nl + o[1]) * nl + o[3];   // edge 4: (l45 l24 l34)
+    t[3] = (o[2] * nl + o[4]) * nl + o[5];   // edge 5: (l25 l35 l45)
+}
+
+// -------------------------------------------------------------------------------------------------------------
+// {6j} machinery (sf_sixj.cu)
+// -------------------------------------------------------------------------------------------------------------
+struct SfSixjTable {
+    int two_jmax;            // -1 if absent
+    long n_slots;
+    const double* values;    // device
+    const long* base4;       // device: prefix sums over (a,b,c,e) groups
+};
+
+int sf_sixj_module_init(void);                       // uploads the factorial table
+void sf_sixj_module_free(void);
+int sf_sixj_table_build(int two_jmax, cudaStream_t st);
+SfSixjTable sf_sixj_table_get(void);
+
+// -------------------------------------------------------------------------------------------------------------
+// S arrays of step 4 (sf_slices.cu) and the two vertex paths
+// -------------------------------------------------------------------------------------------------------------
+struct SfSliceSizes {
+    long n[5];    // elements of S1..S5
+};
+void sf_slice_sizes(const SfDims& D, SfSliceSizes* sz);
+int sf_build_slices(const SfDims& D, double* const S[5], const SfSixjTable& tab, cudaStream_t st);
+
+struct SfScratch;   // owned by the context (sf_api.cu)
+int sf_vertex_staged(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
+int sf_vertex_fused(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
+bool sf_vertex_fused_supported(const SfDims& D);
+
+// scratch allocator owned by the context: grows on demand, freed by sf_finalize.  slot = small integer id.
+void* sf_scratch(int slot, size_t bytes);
+void sf_count_launch(int n);
+void sf_timing_mark(int idx, cudaStream_t st);   // records event idx of the stage timing when it is enabled
+void sf_launch_finalize(const SfProblem& P, long n_out, const double* acc, double* out, cudaStream_t st);
+
+#define SF_CUDA_OK(call)                                   \
+    do {                                                   \
+        cudaError_t err__ = (call);                        \
+        if (err__ != cudaSuccess) return SF_ECUDA;         \
+    } while (0)

@@ -1,0 +1,115 @@
+"""GPU parity of kernel (a), the {6j} evaluation and the canonical table, against the oracle's exact values.
+
+Bar (north_star, reading G16): |gpu - exact| <= 1e-12 |exact| for every symbol with 2j <= 60; |gpu| <= 1e-18 where
+the exact value is 0 (triad failure or a non-trivial zero).
+"""
+import itertools
+import random
+
+import numpy as np
+import pytest
+
+import paper_2107_13952_b200 as sf
+from oracle import wigner
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def ctx():
+    sf.sf_init(1.2)
+    yield
+    sf.sf_sixj_table(-1)
+
+
+def _check(args, got, rel=1e-12):
+    for a, g in zip(args, got):
+        ex = wigner.sixj(*a)
+        if ex == 0.0:
+            assert abs(g) <= 1e-18, (a, g)
+        else:
+            assert abs(g - ex) <= rel * abs(ex), (a, g, ex)
+
+
+def _random_valid(rng, jmax):
+    """A random symbol whose four triads hold (rejection on the last argument ranges)."""
+    while True:
+        a, b, d, e = (rng.randint(0, jmax) for _ in range(4))
+        cs = [c for c in range(abs(a - b), min(a + b, jmax) + 1, 2) if abs(d - e) <= c <= d + e and (d + e + c) % 2 == 0]
+        if not cs:
+            continue
+        c = rng.choice(cs)
+        fs = [f for f in range(abs(a - e), min(a + e, jmax) + 1, 2) if abs(d - b) <= f <= d + b and (d + b + f) % 2 == 0]
+        if not fs:
+            continue
+        return (a, b, c, d, e, rng.choice(fs))
+
+
+def test_all_symbols_up_to_spin_2_direct_and_exact_values():
+    args = list(itertools.product(range(5), repeat=6))          # every tuple with 2j <= 4, valid or not
+    got = sf.sf_sixj_batch(args, mode=0)
+    _check(args, got)
+    # printed exact values (tests/golden/sixj_exact_values.txt)
+    assert sf.sf_sixj_get([1, 1, 2, 1, 1, 2]) == pytest.approx(1 / 6, rel=1e-14)
+    assert sf.sf_sixj_get([4, 4, 4, 4, 4, 4]) == pytest.approx(-3 / 70, rel=1e-14)
+    assert sf.sf_sixj_get([10, 10, 10, 10, 10, 10]) == pytest.approx(1 / 52, rel=1e-14)
+    assert abs(sf.sf_sixj_get([4, 4, 4, 3, 3, 3])) <= 1e-18      # non-trivial zero
+
+
+def test_random_symbols_two_j_le_60_direct():
+    rng = random.Random(60)
+    args = [_random_valid(rng, 60) for _ in range(1500)] + [(60,) * 6, (60, 60, 60, 59, 59, 59), (60, 59, 1, 30, 31, 60)]
+    _check(args, sf.sf_sixj_batch(args, mode=0))
+
+
+def test_large_spins_direct():
+    # config 4 reaches 2x = 142; cancellation ~6e10 there: double-double must hold 1e-12
+    rng = random.Random(150)
+    args = [_random_valid(rng, 150) for _ in range(150)] + [(150,) * 6, (142, 84, 72, 60, 100, 96)]
+    _check(args, sf.sf_sixj_batch(args, mode=0))
+    # beyond that the alternating sum cancels faster than double-double resolves: the accuracy degrades gracefully
+    args = [(200,) * 6, (200, 180, 100, 160, 150, 150)]
+    _check(args, sf.sf_sixj_batch(args, mode=0), rel=1e-9)
+
+
+def test_table_gather_equals_exact_and_uses_symmetry():
+    sf.sf_sixj_table(24)
+    assert sf.sf_sixj_table_two_jmax() == 24
+    slots = sf.sf_sixj_table_slots()
+    # number of VALID tuples with 2j <= 24, by brute force over triads, / 24 is the ideal class count
+    rng = random.Random(24)
+    args = [_random_valid(rng, 24) for _ in range(1200)]
+    args += [tuple(rng.randint(0, 24) for _ in range(6)) for _ in range(300)]      # mostly invalid -> 0
+    got = sf.sf_sixj_batch(args, mode=1)
+    _check(args, got)
+    # all 24 tetrahedral images of one symbol hit the table and agree bitwise
+    a, b, c, d, e, f = 7, 12, 9, 10, 5, 8
+    cols = [(a, d), (b, e), (c, f)]
+    images = []
+    for perm in itertools.permutations(range(3)):
+        p = [cols[q] for q in perm]
+        for flip in ((0, 0, 0), (1, 1, 0), (1, 0, 1), (0, 1, 1)):
+            up = [p[q][flip[q]] for q in range(3)]
+            dn = [p[q][1 - flip[q]] for q in range(3)]
+            images.append(tuple(up + dn))
+    vals = sf.sf_sixj_batch(images, mode=1)
+    assert len(set(images)) == 24 and len(set(vals.tolist())) == 1
+    # every symbol with 2j <= 6 through the table
+    small = list(itertools.product(range(7), repeat=6))
+    _check(small, sf.sf_sixj_batch(small, mode=1))
+    # the table is far smaller than the full (J+1)^6 box
+    assert 0 < slots < 25 ** 6 // 20
+    with pytest.raises(sf.SfError) as err:
+        sf.sf_sixj_batch([(25, 25, 24, 2, 2, 2)], mode=1)
+    assert err.value.status == sf.SF_ETABLE
+
+
+def test_table_two_jmax_60_sampled():
+    sf.sf_sixj_table(60)
+    assert sf.sf_sixj_table_slots() > 10 ** 7
+    rng = random.Random(6060)
+    args = [_random_valid(rng, 60) for _ in range(1500)]
+    got_t = sf.sf_sixj_batch(args, mode=1)
+    got_d = sf.sf_sixj_batch(args, mode=0)
+    _check(args, got_t)
+    assert np.allclose(got_t, got_d, rtol=1e-14, atol=1e-18)   # table slot = direct value of the canonical image

@@ -1,0 +1,211 @@
+"""GPU parity of the vertex tensor (steps 4-7 of the algorithm) against the oracle, through the
+C ABI, on the five workloads of BASELINE.json (small ones in full, large ones on shell sub-ranges the oracle finishes
+in seconds), for both the staged and the fused path, plus edge cases, additivity, determinism and error behaviour.
+"""
+import itertools
+import random
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2107_13952_b200 as sf
+import workloads as wl
+from oracle import ranges
+from oracle import vertex as ov
+from gpu_common import TOL, abi_dims, assert_parity, boosters_for, run_gpu, run_oracle, to_device
+
+pytestmark = pytest.mark.gpu
+
+PATHS = [pytest.param(1, id="staged"), pytest.param(0, id="auto")]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def ctx():
+    sf.sf_init(wl.GAMMA)
+    yield
+    sf.sf_set_path(0)
+    sf.sf_sixj_table(-1)
+
+
+@pytest.fixture(params=PATHS)
+def path(request):
+    sf.sf_set_path(request.param)
+    yield request.param
+    sf.sf_set_path(0)
+
+
+def _full(cfg, what):
+    B = boosters_for(cfg)
+    Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B)
+    Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B)
+    return assert_parity(Ag, Ao, Aabs, what=what), Ag, Ao
+
+
+def test_config0_full(path):
+    worst, Ag, Ao = _full(wl.CONFIGS[0], "config 0")
+    assert Ag.shape == (3,) * 5 and np.abs(Ao).max() > 0
+    assert sf.sf_last_path() == (1 if path == 1 else 2)      # automatic selection takes the fused on-chip path here
+
+
+@pytest.mark.parametrize("two_j", [1, 2, 3, 4, 6, 9, 12])
+def test_config1_bf_sweep(path, two_j):
+    """Identity boosters, Delta_l = 0  =>  A = N(i) {15j}  (reading G8)."""
+    cfg = wl.config1(two_j)
+    worst, Ag, Ao = _full(cfg, cfg["name"])
+    if two_j == 1:      # printed exact values, SURVEY.md 8(c) P5
+        assert Ag[0, 0, 0, 0, 0] == pytest.approx(1 / 16, rel=1e-13)
+        assert Ag[1, 1, 1, 1, 1] == pytest.approx(3 ** 2.5 * 3 ** 4 * (-7 / 432), rel=1e-13)
+
+
+def test_config1_bf_j10_full_tensor():
+    """The largest BF tensor, 21^5 entries (staged path: it does not fit on chip)."""
+    cfg = wl.config1(20)
+    worst, Ag, Ao = _full(cfg, cfg["name"])
+    assert Ag.shape == (21,) * 5
+
+
+@pytest.mark.parametrize("dl", [0, 1, 2])
+def test_config2_small_shell_counts_full(path, dl):
+    cfg = wl.config2(dl)
+    _full(cfg, cfg["name"])
+
+
+@pytest.mark.parametrize("dl,lo,n", [(4, 7000, 40), (8, 531441 - 25, 25), (8, 0, 12), (7, 100000, 30)])
+def test_config2_sub_ranges(path, dl, lo, n):
+    """Larger Delta_l on contiguous shell sub-ranges (Delta_l = 7, 8 contain empty shells: reading G10)."""
+    cfg = wl.config2(dl)
+    B = boosters_for(cfg)
+    Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, lo + n)
+    Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, lo + n)
+    assert_parity(Ag, Ao, Aabs, what=f"{cfg['name']} shells [{lo},{lo + n})")
+
+
+def test_config3_scattered_shells(path):
+    """The headline workload (j = 5, Delta_l = 10) on single shells spread over the grid, and one short range."""
+    cfg = wl.CONFIGS[3]
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    rng = random.Random(3)
+    picks = [0, 11 ** 6 - 1] + [rng.randrange(11 ** 6) for _ in range(3)]
+    for s in picks:
+        Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, s, s + 1, Bdev=Bdev)
+        Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, s, s + 1)
+        assert_parity(Ag, Ao, Aabs, what=f"config 3 shell {s}")
+    lo = 11 ** 5 * 3 + 11 ** 2 * 5 + 7
+    Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, lo + 9, Bdev=Bdev)
+    Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, lo + 9)
+    assert_parity(Ag, Ao, Aabs, what="config 3 short range")
+    assert sf.sf_last_path() == (1 if path == 1 else 2)
+
+
+def _config4(lam):
+    base, _ = wl.config4_base_spins(lambda tj: all(n > 0 for _, n in ranges.boundary_ranges(tj)))
+    assert base == [8, 7, 12, 3, 8, 5, 9, 12, 3, 7]
+    return wl.config4(base, lam)
+
+
+@pytest.mark.parametrize("lam,n", [(1, 60), (2, 6), (3, 1)])
+def test_config4_sub_ranges(path, lam, n):
+    cfg = _config4(lam)
+    B = boosters_for(cfg)
+    lo = 7 ** 6 // 2 + 11
+    Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, lo + n)
+    Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, lo + n)
+    assert_parity(Ag, Ao, Aabs, what=f"{cfg['name']} shells [{lo},{lo + n})")
+
+
+def test_table_and_direct_slices_agree(path):
+    """With a resident table the S arrays are gathered from it; the tensor must not change beyond rounding."""
+    cfg = wl.config2(2)
+    B = boosters_for(cfg)
+    sf.sf_sixj_table(-1)
+    A0 = run_gpu(cfg["two_j"], cfg["two_dl"], B)
+    sf.sf_sixj_table(30)
+    A1 = run_gpu(cfg["two_j"], cfg["two_dl"], B)
+    sf.sf_sixj_table(-1)
+    Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B)
+    assert_parity(A1, Ao, Aabs, what="table-gathered slices")
+    assert np.abs(A1 - A0).max() <= 1e-13 * Aabs.max()
+
+
+def test_additivity_and_determinism(path):
+    cfg = wl.config2(3)
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    two_j, two_dl = cfg["two_j"], cfg["two_dl"]
+    full = run_gpu(two_j, two_dl, B, Bdev=Bdev)
+    again = run_gpu(two_j, two_dl, B, Bdev=Bdev)
+    assert np.array_equal(full, again), "not bitwise reproducible run to run"
+    cuts = [0, 1, 777, 2048, 4095, 4096]
+    parts = sum(run_gpu(two_j, two_dl, B, a, b, Bdev=Bdev) for a, b in zip(cuts[:-1], cuts[1:]))
+    scale = np.abs(full).max()
+    assert np.abs(parts - full).max() <= 1e-12 * scale
+    empty = run_gpu(two_j, two_dl, B, 100, 100, Bdev=Bdev)
+    assert (empty == 0).all()
+
+
+def test_one_hot_boosters_pick_one_w_entry(path):
+    """B_a = e_i e_k^T at one triple each  =>  A[i1, i2..i5] = prod sqrt(2i+1) prod (2k_a+1) {15j}  (pin P6(ii))."""
+    from oracle import fifteenj
+    two_j, two_dl = [2] * 10, 4
+    edge_dims, k_ranges = abi_dims(two_j, two_dl)
+    lo_i, n_i = sf.sf_vertex_dims(two_j)
+    rng = random.Random(11)
+    for _ in range(4):
+        offs = tuple(rng.randrange(3) for _ in range(6))
+        two_l = ranges.shell_spins(two_j, offs)
+        hot, ks, iis = {}, [], []
+        for edge in (2, 3, 4, 5):
+            t = ranges.triple_index(edge, offs, two_dl)
+            klo, nk = k_ranges[edge][t]
+            k = klo + 2 * rng.randrange(nk)
+            ii = rng.randrange(n_i[edge - 1])
+            hot[edge] = (t, ii, (k - edge_dims[edge][1]) // 2)
+            ks.append(k)
+            iis.append(ii)
+        A = run_gpu(two_j, two_dl, wl.one_hot_boosters(3, edge_dims, hot))
+        for a1 in range(n_i[0]):
+            i1 = lo_i[0] + 2 * a1
+            norm = np.sqrt(np.prod([i1 + 1] + [lo_i[e + 1] + 2 * iis[e] + 1 for e in range(4)]))
+            ref = norm * np.prod([k + 1 for k in ks]) * fifteenj.fifteenj(two_l, i1, ks)
+            assert A[(a1, *iis)] == pytest.approx(ref, rel=1e-12, abs=1e-16)
+        mask = np.ones_like(A, dtype=bool)
+        mask[(slice(None), *iis)] = False
+        assert (A[mask] == 0).all()
+
+
+def test_half_integer_nonhomogeneous_full(path):
+    two_j, two_dl = [4, 3, 1, 4, 2, 5, 5, 5, 4, 3], 4
+    cfg = dict(two_j=two_j, two_dl=two_dl, boosters="random", seed=77)
+    B = boosters_for(cfg)
+    Ag = run_gpu(two_j, two_dl, B)
+    Ao, Aabs = run_oracle(two_j, two_dl, B)
+    assert_parity(Ag, Ao, Aabs, what="half-integer non-homogeneous")
+
+
+def test_errors(path):
+    two_j = [2] * 10
+    B = to_device(boosters_for(wl.CONFIGS[0]))
+    out = torch.zeros(3 ** 5, dtype=torch.float64, device="cuda")
+    for bad_j, bad_dl, status in [([2] * 9 + [3], 4, sf.SF_ESPIN), (two_j, 3, sf.SF_EARG), (two_j, -2, sf.SF_EARG)]:
+        with pytest.raises(sf.SfError) as e:
+            sf.sf_vertex_amplitude(bad_j, bad_dl, B, out)
+        assert e.value.status == status
+    with pytest.raises(sf.SfError) as e:
+        sf.sf_vertex_amplitude_range(two_j, 4, B, 10, 5, out)
+    assert e.value.status == sf.SF_EARG
+    with pytest.raises(sf.SfError) as e:
+        sf.sf_vertex_amplitude_range(two_j, 4, B, 0, 730, out)
+    assert e.value.status == sf.SF_EARG
+    assert (out == 0).all()          # untouched on error
+
+
+def test_host_entry_point_matches_device_entry_point():
+    cfg = wl.CONFIGS[0]
+    B = boosters_for(cfg)
+    Ad = run_gpu(cfg["two_j"], cfg["two_dl"], B)
+    hb = [torch.from_numpy(B[e]).pin_memory() for e in (2, 3, 4, 5)]
+    ho = torch.empty(3 ** 5, dtype=torch.float64).pin_memory()
+    sf.sf_vertex_amplitude_host(cfg["two_j"], cfg["two_dl"], hb, ho, torch.cuda.current_stream())
+    assert np.array_equal(ho.numpy().reshape(Ad.shape), Ad)
