@@ -1,0 +1,323 @@
+"""bench.py -- throughput of the EPRL vertex-tensor hot path (all rows of SURVEY.md 8(a)) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one workload: one sf_vertex_amplitude call (k-range tables, the five S
+arrays of {6j}, {15j} assembly + four mode products over every shell, fixed-order accumulation, normalisation).  The
+default workload is config 3 of BASELINE.json (all spins j = 5, Delta_l = 10: 1 771 561 shells, A[11^5]), the
+configuration the headline metric is quoted on.  The {6j} table (sf_sixj_table, a one-off like the paper's precomputed
+tables) is built before the timed region and reported separately.
+
+N > 1: the path does not shard (north_star: one GPU, no collectives) => N independent replicas, one per rank,
+"scaling": "weak"; value = shells of all replicas / max-over-ranks time.
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the oracle (oracle/, plain CPU loops) on the host cores on a
+bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "eprl_shells_contracted_per_s"
+UNIT = "shells/s"
+
+
+def workload(config, sub):
+    if config == 0:
+        return wl.CONFIGS[0]
+    if config == 2:
+        return wl.config2(sub if sub is not None else 8)
+    if config == 3:
+        return wl.CONFIGS[3]
+    raise SystemExit("bench workloads: --config 0, 2 (with --sub DELTA_L) or 3")
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), [c.strip() for c in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for t, r in self.rows if t0 <= t <= t1] or [r for _, r in self.rows[-3:]]
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); smax.append(float(r[1])); power.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# CPU baseline = the oracle as it stands, on a bounded sample of the workload
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, B, n_sample, seed=12345):
+    """(lo, hi, S arrays): a seeded contiguous range of `n_sample` shells and the exact-{6j} S arrays it needs (the
+    paper also precomputes its {6j} tables; not timed)."""
+    from oracle import vertex as ov
+    L = ov.Layout(cfg["two_j"], cfg["two_dl"])
+    n_sample = min(n_sample, L.n_shells)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    lo = int(rng.integers(0, L.n_shells - n_sample + 1))
+    S = ov.build_s_arrays(L, lo, lo + n_sample, processes=os.cpu_count() or 1)
+    return lo, lo + n_sample, S
+
+
+def oracle_time(cfg, B, lo, hi, S, threads):
+    from oracle import vertex as ov
+    t0 = time.perf_counter()
+    r = ov.vertex_l1(cfg["two_j"], cfg["two_dl"], B, shell_lo=lo, shell_hi=hi, long_double=False, want_abs=False,
+                     threads=threads, s_arrays=S)
+    return time.perf_counter() - t0, r
+
+
+def dims_from_oracle(cfg):
+    from oracle import ranges
+    edge_dims, k_ranges = {}, {}
+    for edge in (2, 3, 4, 5):
+        _, n_i, _, base, pad = ranges.booster_dims(cfg["two_j"], cfg["two_dl"], edge)
+        edge_dims[edge] = (n_i, base, pad)
+        k_ranges[edge] = ranges.booster_k_ranges(cfg["two_j"], cfg["two_dl"], edge)
+    return edge_dims, k_ranges
+
+
+def run_reference(args, cfg, rank):
+    """The oracle as it stands on the host cores: each step = one bounded sample of the workload's shells."""
+    if rank != 0:
+        return
+    edge_dims, k_ranges = dims_from_oracle(cfg)
+    nl = cfg["two_dl"] // 2 + 1
+    B = wl.random_boosters(cfg["seed"], nl, edge_dims, k_ranges)
+    cores = os.cpu_count() or 1
+    n_sample = min(args.ref_shells, nl ** 6)
+    lo, hi, S = oracle_sample(cfg, B, n_sample)
+    for _ in range(args.warmup):
+        oracle_time(cfg, B, lo, min(hi, lo + max(1, n_sample // 8)), S, cores)
+    total = 0.0
+    for _ in range(args.steps):
+        dt, _ = oracle_time(cfg, B, lo, hi, S, cores)
+        total += dt
+    value = (hi - lo) * args.steps / total
+    sample = f"shells [{lo},{hi}) of {nl ** 6} per step (seeded contiguous range), exact-6j S arrays precomputed untimed"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "two_j": cfg["two_j"], "two_dl": cfg["two_dl"], "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args, cfg, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2107_13952_b200 as sf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    two_j, two_dl = cfg["two_j"], cfg["two_dl"]
+    nl = two_dl // 2 + 1
+    n_shells = nl ** 6
+
+    sf.sf_init(wl.GAMMA)
+    # one-off {6j} table (kernel (a)), outside the timed region, timed on its own
+    t0 = time.perf_counter()
+    sf.sf_sixj_table(args.table)
+    torch.cuda.synchronize()
+    table_ms = 1e3 * (time.perf_counter() - t0)
+
+    edge_dims, k_ranges = {}, {}
+    for edge in (2, 3, 4, 5):
+        _, n_i_e, base, pad = sf.sf_booster_dims(two_j, two_dl, edge)
+        edge_dims[edge] = (n_i_e, base, pad)
+        k_ranges[edge] = sf.sf_booster_kranges(two_j, two_dl, edge)
+    B = wl.random_boosters(cfg["seed"], nl, edge_dims, k_ranges)
+    Bhost = [torch.from_numpy(B[e]).pin_memory() for e in (2, 3, 4, 5)]
+    Bdev = [b.cuda() for b in Bhost]
+    _, n_i = sf.sf_vertex_dims(two_j)
+    out = torch.zeros(tuple(n_i), dtype=torch.float64, device="cuda")
+    out_host = torch.zeros(tuple(n_i), dtype=torch.float64).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    # algorithmic work (valid ranges only): host integer count of the contraction, device integer count of eq. (5) terms
+    work = sf.sf_vertex_work(two_j, two_dl)
+    n_terms = sf.sf_vertex_terms(two_j, two_dl)
+    f_con, f_asm = work["f_con"], 6.0 * n_terms
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        flush.zero_()
+        sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)
+    torch.cuda.synchronize()
+
+    # ---- timed region: K steps, inputs resident in HBM ----
+    sf.sf_set_timing(True)            # the library brackets its stages with CUDA events on `stream`
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.3)
+    sf.sf_launch_count(reset=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage = np.zeros(3)
+    barrier()
+    w0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(args.steps):
+        flush.zero_()
+        sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)
+        stage += np.array(sf.sf_last_stage_ms())
+    e1.record(stream)
+    barrier()
+    w1 = time.perf_counter()
+    launches = sf.sf_launch_count()
+    clocks = sampler.stop(w0, w1)
+    sf.sf_set_timing(False)
+    ms = e0.elapsed_time(e1)
+    last_path = sf.sf_last_path()
+    A_dev = out.cpu().numpy().copy()
+
+    # ---- end to end: host buffers in, host tensor out, through sf_vertex_amplitude_host ----
+    for _ in range(min(args.warmup, 2)):
+        sf.sf_vertex_amplitude_host(two_j, two_dl, Bhost, out_host, stream)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        flush.zero_()
+        sf.sf_vertex_amplitude_host(two_j, two_dl, Bhost, out_host, stream)      # synchronises `stream` itself
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    h2d = int(sum(b.numel() * 8 for b in Bhost))
+    d2h = int(out_host.numel() * 8)
+    assert np.array_equal(out_host.numpy(), A_dev), "host and device entry points disagree"
+
+    if world > 1:
+        t = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_step = ms / args.steps
+    value = world * n_shells * args.steps / (ms * 1e-3)
+    kern_ms = stage[1] / args.steps                                     # the fused (or staged) steps 5-6(iii) kernel(s)
+    achieved = (f_con + f_asm) / (kern_ms * 1e-3) / 1e12
+    peak_dfma, peak_dmma = sf.sf_fp64_peak(0), sf.sf_fp64_peak(1)
+    peak = max(peak_dfma, peak_dmma)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": cfg["name"], "two_j": two_j, "two_dl": two_dl, "shells": n_shells,
+                   "nonempty_shells": work["n_nonempty"], "out_shape": n_i, "boosters": "seeded N(0,1)*(1+u+v+w)^-1.5",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "256 MiB device memset between steps (inside the timed region)",
+                   "sixj_table_two_jmax": args.table, "path": {1: "staged", 2: "fused"}.get(last_path, "?")},
+        "vertex_tensors_per_s": world * args.steps / (ms * 1e-3),
+        "clocks": clocks,
+        "e2e": {"value": world * n_shells * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s / args.steps},
+        "gpu_launches": launches,
+        "roofline": {"bound": "alu", "kernel": "k_vertex_fused" if last_path == 2 else "k_stage_*",
+                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": "measured in this process: FP64 DFMA %.2f, DMMA(mma.sync m8n8k4) %.2f TFLOP/s"
+                                    % (peak_dfma, peak_dmma),
+                     "flop_per_step": {"contraction": f_con, "assembly": f_asm}, "kernel_ms": kern_ms},
+        "stages_ms_per_step": {"s_arrays": stage[0] / args.steps, "assembly_contraction": kern_ms,
+                               "accumulate_normalise": stage[2] / args.steps},
+        "sixj_table_build_ms": table_ms,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        n_sample = min(args.ref_shells, n_shells)
+        lo, hi, S = oracle_sample(cfg, B, n_sample)
+        dt, r = oracle_time(cfg, B, lo, hi, S, cores)
+        line["cpu_baseline"] = {"value": (hi - lo) / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"shells [{lo},{hi}) of {n_shells} (seeded contiguous range, {dt:.1f} s), "
+                                          "exact-6j S arrays precomputed untimed"}
+        # the same sample through the CUDA path: a parity spot check at the bench's launch configuration
+        sub = torch.zeros(tuple(n_i), dtype=torch.float64, device="cuda")
+        sf.sf_vertex_amplitude_range(two_j, two_dl, Bdev, lo, hi, sub, stream)
+        torch.cuda.synchronize()
+        scale = float(np.abs(r["A"]).max())
+        line["cpu_baseline"]["max_abs_diff_over_max"] = float(np.abs(sub.cpu().numpy() - r["A"]).max() / scale)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--sub", type=int, default=None, help="Delta_l of config 2")
+    ap.add_argument("--table", type=int, default=60, help="two_jmax of the resident {6j} table (-1: none)")
+    ap.add_argument("--ref-shells", type=int, default=8000, help="shells in the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = workload(args.config, args.sub)
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+    else:
+        run_ours(args, cfg, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

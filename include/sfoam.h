@@ -96,6 +96,17 @@ int sf_booster_kranges(const int two_j[10], int two_dl, int edge, int *two_k_min
 int sf_vertex_work(const int two_j[10], int two_dl, long shell_lo, long shell_hi,
                    double *f_con, long *n_nonempty, double *n_w);
 
+/* Number of (entry, x) summands of eq. (5) over shells [shell_lo, shell_hi): the sum over the entries
+ * (i1 k2 k3 k4 k5) of every non-empty shell of the size of the intersection of the five triads that contain x.  The
+ * algorithmic assembly work is F_asm = 6 * n_terms (five multiplications by a {6j} or by (2x+1), one addition).
+ * Counted by a device kernel (integer work, exact); synchronises the default stream.  Requires sf_init. */
+int sf_vertex_terms(const int two_j[10], int two_dl, long shell_lo, long shell_hi, double *n_terms);
+
+/* FP64 roofline denominators measured in this process: TFLOP/s of dependent-chain microbenchmarks,
+ * kind 0 = DFMA (vector FP64 fused multiply-add), kind 1 = DMMA (mma.sync m8n8k4 f64 on the tensor cores).
+ * Best of 5 launches of a few ms each; synchronises the default stream.  Requires sf_init. */
+int sf_fp64_peak(int kind, double *tflops);
+
 /* The vertex tensor (steps 4-7).  boosters / out: DEVICE pointers; out holds prod(n_i) doubles and
  * is overwritten.  Asynchronous w.r.t. the host, ordered on `stream`.  Requires sf_init. */
 int sf_vertex_amplitude(const int two_j[10], int two_dl, const sf_boosters *boosters, double *out, sf_stream_t stream);

@@ -51,6 +51,9 @@ def _lib():
         lib.sf_vertex_work.argtypes = [_I10, ctypes.c_int, ctypes.c_long, ctypes.c_long,
                                        ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_long),
                                        ctypes.POINTER(ctypes.c_double)]
+        lib.sf_vertex_terms.argtypes = [_I10, ctypes.c_int, ctypes.c_long, ctypes.c_long,
+                                        ctypes.POINTER(ctypes.c_double)]
+        lib.sf_fp64_peak.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
         lib.sf_vertex_amplitude.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_void_p,
                                             ctypes.c_void_p]
         lib.sf_vertex_amplitude_range.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_long,
@@ -198,6 +201,23 @@ def sf_vertex_work(two_j, two_dl, shell_lo=0, shell_hi=None):
     _check(_lib().sf_vertex_work(_spins(two_j), int(two_dl), int(shell_lo), int(shell_hi), ctypes.byref(f),
                                  ctypes.byref(ne), ctypes.byref(nw)), "sf_vertex_work")
     return {"f_con": f.value, "n_nonempty": ne.value, "n_w": nw.value}
+
+
+def sf_vertex_terms(two_j, two_dl, shell_lo=0, shell_hi=None):
+    """Number of (entry, x) summands of eq. (5) over the shell range (device integer kernel); F_asm = 6 * n_terms."""
+    if shell_hi is None:
+        shell_hi = (int(two_dl) // 2 + 1) ** 6
+    n = ctypes.c_double()
+    _check(_lib().sf_vertex_terms(_spins(two_j), int(two_dl), int(shell_lo), int(shell_hi), ctypes.byref(n)),
+           "sf_vertex_terms")
+    return n.value
+
+
+def sf_fp64_peak(kind):
+    """Measured FP64 peak in TFLOP/s: kind 0 = DFMA chains, kind 1 = DMMA (mma.sync m8n8k4 f64) chains."""
+    v = ctypes.c_double()
+    _check(_lib().sf_fp64_peak(int(kind), ctypes.byref(v)), "sf_fp64_peak")
+    return v.value
 
 
 # ---------------------------------------------------------------------------------------------------------------

@@ -163,6 +163,29 @@ __global__ void k_kranges(SfProblem P, int nt, SfKRange* __restrict__ out)
     out[q] = r;
 }
 
+// steps 1-2 on the device side: the problem descriptor and the per-triple k-range tables (no host->device copy)
+static int setup_problem(const SfDims& D, const sf_boosters* boosters, SfProblem& P, cudaStream_t st)
+{
+    memset(&P, 0, sizeof P);
+    memcpy(P.two_j, D.two_j, sizeof P.two_j);
+    P.nl = D.nl;
+    memcpy(P.two_i_min, D.two_i_min, sizeof P.two_i_min);
+    memcpy(P.n_i, D.n_i, sizeof P.n_i);
+    memcpy(P.two_k_base, D.two_k_base, sizeof P.two_k_base);
+    memcpy(P.n_k_pad, D.n_k_pad, sizeof P.n_k_pad);
+    memcpy(P.k_max, D.k_max, sizeof P.k_max);
+    P.two_x_base = D.two_x_base;
+    P.n_x_pad = D.n_x_pad;
+    for (int e = 0; e < 4; ++e) P.B[e] = boosters ? boosters->B[e] : nullptr;
+    const int nt = D.nl * D.nl * D.nl;
+    SfKRange* d = (SfKRange*)sf_scratch(SLOT_KR, sizeof(SfKRange) * nt * 4);
+    if (!d) return SF_ENOMEM;
+    for (int e = 0; e < 4; ++e) P.kr[e] = d + (long)e * nt;
+    k_kranges<<<(4 * nt + 127) / 128, 128, 0, st>>>(P, nt, d);
+    sf_count_launch(1);
+    return SF_OK;
+}
+
 static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo, long shell_hi,
                         double* out, cudaStream_t st, bool full)
 {
@@ -186,26 +209,8 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
     }
 
     SfProblem P;
-    memcpy(P.two_j, D.two_j, sizeof P.two_j);
-    P.nl = D.nl;
-    memcpy(P.two_i_min, D.two_i_min, sizeof P.two_i_min);
-    memcpy(P.n_i, D.n_i, sizeof P.n_i);
-    memcpy(P.two_k_base, D.two_k_base, sizeof P.two_k_base);
-    memcpy(P.n_k_pad, D.n_k_pad, sizeof P.n_k_pad);
-    memcpy(P.k_max, D.k_max, sizeof P.k_max);
-    P.two_x_base = D.two_x_base;
-    P.n_x_pad = D.n_x_pad;
-    for (int e = 0; e < 4; ++e) P.B[e] = boosters->B[e];
-
-    // step 2: per-triple k-range tables, computed on the device (no host->device copy on the call path)
-    const int nt = D.nl * D.nl * D.nl;
-    {
-        SfKRange* d = (SfKRange*)sf_scratch(SLOT_KR, sizeof(SfKRange) * nt * 4);
-        if (!d) return SF_ENOMEM;
-        for (int e = 0; e < 4; ++e) P.kr[e] = d + (long)e * nt;
-        k_kranges<<<(4 * nt + 127) / 128, 128, 0, st>>>(P, nt, d);
-        sf_count_launch(1);
-    }
+    rc = setup_problem(D, boosters, P, st);
+    if (rc != SF_OK) return rc;
 
     // step 4: the five S arrays
     SfSliceSizes sz;
@@ -279,5 +284,31 @@ extern "C" int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const d
     if (rc != SF_OK) return rc;
     SF_CUDA_OK(cudaMemcpyAsync(host_out, dout, sizeof(double) * D.n_out, cudaMemcpyDeviceToHost, st));
     SF_CUDA_OK(cudaStreamSynchronize(st));
+    return SF_OK;
+}
+
+void sf_launch_count_terms(const SfProblem& P, long shell_lo, long shell_hi, unsigned long long* total, cudaStream_t st);
+
+extern "C" int sf_vertex_terms(const int two_j[10], int two_dl, long shell_lo, long shell_hi, double* n_terms)
+{
+    if (!g_ctx.init) return SF_ENOTINIT;
+    if (!two_j || !n_terms) return SF_EARG;
+    SfDims D;
+    int rc = sf_host_dims(two_j, two_dl, &D);
+    if (rc != SF_OK) return rc;
+    if (shell_lo < 0 || shell_hi > D.n_shells || shell_lo > shell_hi) return SF_EARG;
+    SfProblem P;
+    rc = setup_problem(D, nullptr, P, 0);
+    if (rc != SF_OK) return rc;
+    unsigned long long* d = (unsigned long long*)sf_scratch(SLOT_MISC, 256);
+    if (!d) return SF_ENOMEM;
+    SF_CUDA_OK(cudaMemsetAsync(d, 0, sizeof(unsigned long long), 0));
+    if (shell_hi > shell_lo) {
+        sf_launch_count_terms(P, shell_lo, shell_hi, d, 0);
+        sf_count_launch(1);
+    }
+    unsigned long long h = 0;
+    SF_CUDA_OK(cudaMemcpy(&h, d, sizeof h, cudaMemcpyDeviceToHost));
+    *n_terms = (double)h;
     return SF_OK;
 }
