@@ -263,13 +263,13 @@ def run_ours(args, cfg, rank, world, local_rank):
                    "nonempty_shells": work["n_nonempty"], "out_shape": n_i, "boosters": "seeded N(0,1)*(1+u+v+w)^-1.5",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "256 MiB device memset between steps (inside the timed region)",
-                   "sixj_table_two_jmax": args.table, "path": {1: "staged", 2: "fused"}.get(last_path, "?")},
+                   "sixj_table_two_jmax": args.table, "path": {1: "staged", 2: "fused", 3: "line"}.get(last_path, "?")},
         "vertex_tensors_per_s": world * args.steps / (ms * 1e-3),
         "clocks": clocks,
         "e2e": {"value": world * n_shells * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s / args.steps},
         "gpu_launches": launches,
-        "roofline": {"bound": "alu", "kernel": "k_vertex_fused" if last_path == 2 else "k_stage_*",
+        "roofline": {"bound": "alu", "kernel": {2: "k_vertex_fused", 3: "k_vertex_line"}.get(last_path, "k_stage_*"),
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
                      "peak_source": "measured in this process: FP64 DFMA %.2f, DMMA(mma.sync m8n8k4) %.2f TFLOP/s"
                                     % (peak_dfma, peak_dmma),

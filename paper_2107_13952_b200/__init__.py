@@ -120,7 +120,8 @@ def sf_last_stage_ms():
 
 
 def sf_set_path(path):
-    """0 = automatic, 1 = staged (general sizes), 2 = fused on-chip path (raises SF_EARG at call time if too large)."""
+    """0 = automatic, 1 = staged (general sizes), 2 = first fused on-chip path, 3 = line path (on-chip, register
+    accumulation over lines of shells); 2 and 3 raise SF_EARG at call time for shapes they do not hold."""
     _check(_lib().sf_set_path(int(path)), "sf_set_path")
 
 

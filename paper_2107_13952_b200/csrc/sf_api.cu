@@ -131,7 +131,7 @@ extern "C" int sf_last_stage_ms(double ms[3])
 // 0 = automatic (fused on-chip path when the tensor fits, staged path otherwise), 1 = staged, 2 = fused
 extern "C" int sf_set_path(int path)
 {
-    if (path < 0 || path > 2) return SF_EARG;
+    if (path < 0 || path > 3) return SF_EARG;
     g_ctx.path = path;
     return SF_OK;
 }
@@ -227,11 +227,14 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
     sf_timing_mark(1, st);
 
     // steps 5-7
-    const bool fused_ok = sf_vertex_fused_supported(D);
-    if (g_ctx.path == 2 && !fused_ok) return SF_EARG;
-    const bool use_fused = g_ctx.path == 2 || (g_ctx.path == 0 && fused_ok);
-    g_ctx.last_path = use_fused ? 2 : 1;
-    rc = use_fused ? sf_vertex_fused(D, P, shell_lo, shell_hi, out, st) : sf_vertex_staged(D, P, shell_lo, shell_hi, out, st);
+    const bool line_ok = sf_vertex_line_supported(D), fused_ok = sf_vertex_fused_supported(D);
+    if ((g_ctx.path == 2 && !fused_ok) || (g_ctx.path == 3 && !line_ok)) return SF_EARG;
+    int path = g_ctx.path;
+    if (path == 0) path = line_ok ? 3 : fused_ok ? 2 : 1;
+    g_ctx.last_path = path;
+    rc = path == 3   ? sf_vertex_line(D, P, shell_lo, shell_hi, out, st)
+         : path == 2 ? sf_vertex_fused(D, P, shell_lo, shell_hi, out, st)
+                     : sf_vertex_staged(D, P, shell_lo, shell_hi, out, st);
     if (rc != SF_OK) return rc;
     sf_timing_mark(3, st);
     if (g_ctx.timing) {

@@ -45,7 +45,7 @@ def _full(cfg, what):
 def test_config0_full(path):
     worst, Ag, Ao = _full(wl.CONFIGS[0], "config 0")
     assert Ag.shape == (3,) * 5 and np.abs(Ao).max() > 0
-    assert sf.sf_last_path() == (1 if path == 1 else 2)      # automatic selection takes the fused on-chip path here
+    assert sf.sf_last_path() == (1 if path == 1 else 3)      # automatic selection takes the on-chip line path here
 
 
 @pytest.mark.parametrize("two_j", [1, 2, 3, 4, 6, 9, 12])
@@ -96,7 +96,7 @@ def test_config3_scattered_shells(path):
     Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, lo + 9, Bdev=Bdev)
     Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, lo + 9)
     assert_parity(Ag, Ao, Aabs, what="config 3 short range")
-    assert sf.sf_last_path() == (1 if path == 1 else 2)
+    assert sf.sf_last_path() == (1 if path == 1 else 3)
 
 
 def _config4(lam):
