@@ -150,6 +150,22 @@ def run_reference(args, cfg, rank):
     print(json.dumps(line))
 
 
+def max_over_ranks(values, world, device):
+    """Element-wise maximum of per-rank timings over all ranks (replicas: the job takes as long as its slowest rank)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_value(units_per_rank, steps, world, seconds):
+    """Whole-job throughput of `world` replicas that each processed `units_per_rank` units per step."""
+    return world * units_per_rank * steps / seconds
+
+
 def run_ours(args, cfg, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -240,17 +256,14 @@ def run_ours(args, cfg, rank, world, local_rank):
     d2h = int(out_host.numel() * 8)
     assert np.array_equal(out_host.numpy(), A_dev), "host and device entry points disagree"
 
-    if world > 1:
-        t = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(t[0]), float(t[1])
+    ms, e2e_s = max_over_ranks([ms, e2e_s], world, "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     ms_step = ms / args.steps
-    value = world * n_shells * args.steps / (ms * 1e-3)
+    value = whole_job_value(n_shells, args.steps, world, ms * 1e-3)
     kern_ms = stage[1] / args.steps                                     # the fused (or staged) steps 5-6(iii) kernel(s)
     achieved = (f_con + f_asm) / (kern_ms * 1e-3) / 1e12
     peak_dfma, peak_dmma = sf.sf_fp64_peak(0), sf.sf_fp64_peak(1)
@@ -266,7 +279,7 @@ def run_ours(args, cfg, rank, world, local_rank):
                    "sixj_table_two_jmax": args.table, "path": {1: "staged", 2: "fused", 3: "line"}.get(last_path, "?")},
         "vertex_tensors_per_s": world * args.steps / (ms * 1e-3),
         "clocks": clocks,
-        "e2e": {"value": world * n_shells * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        "e2e": {"value": whole_job_value(n_shells, args.steps, world, e2e_s), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s / args.steps},
         "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": {2: "k_vertex_fused", 3: "k_vertex_line"}.get(last_path, "k_stage_*"),
