@@ -3,30 +3,35 @@
 //
 // Work unit = (block of shells with the same (l23 l24 l25), boundary intertwiner i1, batch of SLOTS values of k2
 // [, sub-range of the block's lines]).  The canonical shell order (eq. (9)) has l45 fastest, so a "line" =
-// the nl consecutive shells that differ only in l45, and a block = nl^2 consecutive lines.  For every shell of the unit
-// the CTA (16 warps) computes, with FP64 tensor-core MMAs (mma.sync m8n8k4 f64 = SASS DMMA.8x8x4; tcgen05 has no FP64
-// kind) whose operands are staged in shared memory:
+// the nl consecutive shells that differ only in l45, and a block = nl^2 consecutive lines.  Rows r = (s, c3): k2 slot s
+// of the batch and the compact index c3 of k3; c4 = compact index of k4 inside the shell's own range.
 //
-//   asm  W[(s,c3),c4][c5] = (-1)^R sum_x U[(s,c3)][x] S3[c3,c4][x] Y[c4][x][c5]                  eq. (5)
-//        per c4 one GEMM over the recoupling spin x (K = x), U = (2x+1) S5 S4 (unit constant), S3 (line constant),
-//        Y = S2 S1 (per shell): the five {6j} of eq. (5); the per-shell {15j} tensor W lives in MMA C fragments
-//   G1   T4[(s,c3),c4][i5] = sum_c5 W . (2k5+1) B5[i5,c5]      step 6(iii): the C fragments of W ARE the A
-//        fragments of this product under a permuted order of the contracted index (no data movement)
-//   G2   T3[(s,c3,i5)][i4] += sum_c4 T4 . (2k4+1) B4[i4,c4]    accumulated in registers over the shells of the line
-//   G3   T2[(s,i4,i5)][i3] += sum_c3 T3 . (2k3+1) B3[i3,c3]    once per line: B3 depends on (l34 l35 l23) only, so by
-//        linearity the product is applied to the line's sum (the contracted index is extended by the shell offset)
-//   G4   A[i2][(i3,i4,i5)]  = sum_s  T2 . (2k2+1) B2[i2,k2(s)] once per unit: B2 depends on (l23 l24 l25) only
+//   prep Z[l25 i1 l35 l45][k4][i5][x] = (-1)^(..) sum_k5 S2 S1 (2k5+1) B5[i5,k5]      two {6j} of eq. (5)
+//        contracted with the edge-5 booster (step 6(iii)).  S1, S2 and B5 depend on (l25 l35 l45, i1) only,
+//        so this product is formed once per (triple, i1) by k_line_prep_z -- a precomputation like the paper's steps 3-4.
+//   P1   T4[r,c4][i5] = sum_x (U[r][x] S3[c3,c4][x]) Z[c4][x][i5]     the sum over the recoupling spin x of eq. (5) with the
+//        other three {6j} (U = (2x+1) S5 S4 is unit constant, S3 line constant): the {15j} of the shell, already
+//        contracted over k5.  One GEMM over x per c4.
+//   P2   T3[(r,i5)][i4] += sum_c4 T4 . (2k4+1) B4[i4,c4]              accumulated in registers over the shells of a line
+//   G3   T2[(s,i4,i5)][i3] += sum_c3 T3 . (2k3+1) B3[i3,c3]           once per line (B3 does not depend on l45: linearity)
+//   G4   A[i2][(i3,i4,i5)]  = sum_s  T2 . (2k2+1) B2[i2,k2(s)]        once per unit (B2 depends on (l23 l24 l25) only)
 //
-// Every shell's W is assembled and contracted with its own four booster sub-matrices (step 6(i)-(iii)); step 6(iv),
-// the accumulation over shells, happens on T3 / T2 / A in a fixed order (shells ascending inside a unit, units
-// ascending in k_reduce_units), so the result is bitwise reproducible.  No float atomics.
+// Every product is an FP64 tensor-core MMA (mma.sync m8n8k4 f64 = SASS DMMA.8x8x4; tcgen05 has no FP64 kind).  The CTA
+// is warp specialised: 15 consumer warps run P1/P2/G3/G4, one producer warp streams each shell's Z block and weighted
+// B4 block from global memory into a two-stage shared-memory ring with bulk asynchronous copies (cp.async.bulk, SASS
+// UBLKCP) signalled through mbarriers.  T4 lives in shared memory in MMA-fragment order (one 32-lane fragment per
+// (tile, k-step), tile bases skewed) so that both the C-fragment stores of P1 and the A-fragment loads of P2 are
+// bank-conflict free and need no index arithmetic.
+//
+// Step 6(iv), the accumulation over shells, happens on T3 / T2 / A in a fixed order (shells ascending inside a unit,
+// units ascending in k_reduce_units), so the result is bitwise reproducible.  No float atomics.
 #include <stdio.h>
 
 #include "sf_internal.h"
 
-#define LINE_THREADS 512
-#define LINE_WARPS 16
-#define LINE_PFY 8              // prefetch registers (doubles) per thread for the next shell's Y operand
+#define LINE_CONSUMERS 480
+#define LINE_WARPS 15
+#define LINE_THREADS (LINE_CONSUMERS + 32)
 
 struct LineParams {
     SfProblem P;
@@ -34,12 +39,16 @@ struct LineParams {
     long blk0;                  // first block (shell_lo / nl^3)
     int n_blocks, n_batches, n_sub, n_units;
     int slots;                  // k2 values per batch
-    int LDK, NXF;               // row strides (doubles) of [rows][contracted k] and [rows][x] operands; both = 4 mod 8
-    int g1_shfl;                // 1: k ranges <= 12, the third k-step of G1 is built with one quad shuffle
+    int NXF;                    // x stride (doubles) of U, S3s, Z rows: 4 * k-steps of x, = 4 mod 8
+    int KS3, KS4, LDK3, LDK4;   // k-steps of the c3 / c4 contractions (call maxima) and the booster row strides 4*KS
+    int TS4, TS3;               // tile strides (doubles) of T4 (32 KS4 + 4) and of the G3 operand A3 (32 KS3)
+    int mt_max;                 // row tiles of 8 a unit can have
     int jsum;                   // sum of the ten boundary spins (2j units)
-    int offX2, offU, offS3, offY, offS1, offBw, offB2, n_smem;   // shared-memory offsets / total (doubles)
+    int zslab;                  // doubles of one (slab, k4) block of Z: NT8 * NXF
+    int offX2, offU, offS3, offZ, offBw4, offBw3, offBw2, offRow, offSh, offBar, n_smem;   // shared-memory offsets (doubles)
+    const double* Zg;           // [l25][i1][l35][l45][q4][NT8][NXF]
+    const double* Bw4g;         // [t4][NT8][LDK4] weighted, compact in c4, zero padded
     double* partial;            // [n_units][n2][n3*n4*n5]
-    unsigned int* counter;
 };
 
 __device__ __forceinline__ void line_dmma(double& c0, double& c1, double a, double b)
@@ -49,194 +58,270 @@ __device__ __forceinline__ void line_dmma(double& c0, double& c1, double a, doub
         : "d"(a), "d"(b));
 }
 
-struct LineShell {              // per-shell quantities (steps 2 and 6(ii): ranges of k3 k4 k5 and the selected sub-matrices)
-    int o34, o35, o45;
-    int t3, t4, t5;
-    int K3, K4, K5, q3b, q4b, q5b, kmin3, kmin4, kmin5;
-    int osum;
-};
-
-__device__ __forceinline__ bool line_shell(const SfProblem& P, long shell, int o23, int o24, int o25, LineShell& S)
+// ---- mbarrier / bulk-copy primitives (PTX ISA: mbarrier, cp.async.bulk) ----
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
 {
-    const int nl = P.nl;
-    const int r = (int)(shell % ((long)nl * nl * nl));
-    S.o45 = r % nl;
-    S.o35 = (r / nl) % nl;
-    S.o34 = r / (nl * nl);
-    S.t3 = (S.o34 * nl + S.o35) * nl + o23;
-    S.t4 = (S.o45 * nl + o24) * nl + S.o34;
-    S.t5 = (o25 * nl + S.o35) * nl + S.o45;
-    const SfKRange r3 = P.kr[1][S.t3], r4 = P.kr[2][S.t4], r5 = P.kr[3][S.t5];
-    S.K3 = r3.n_k; S.K4 = r4.n_k; S.K5 = r5.n_k;
-    S.kmin3 = r3.two_k_min; S.kmin4 = r4.two_k_min; S.kmin5 = r5.two_k_min;
-    S.q3b = (r3.two_k_min - P.two_k_base[1]) >> 1;
-    S.q4b = (r4.two_k_min - P.two_k_base[2]) >> 1;
-    S.q5b = (r5.two_k_min - P.two_k_base[3]) >> 1;
-    S.osum = o23 + o24 + o25 + S.o34 + S.o35 + S.o45;
-    return S.K3 > 0 && S.K4 > 0 && S.K5 > 0;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    unsigned done = 0;
+    for (unsigned spin = 0; !done; ++spin) {
+        asm volatile(
+            "{\n.reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+        if (spin > (1u << 28)) __trap();   // a lost signal must fail the launch, never hang the device
+    }
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(LINE_CONSUMERS) : "memory"); }
+
+// ---------------------------------------------------------------------------------------------------------
+// precomputation: Z and the weighted edge-4 booster blocks
+// ---------------------------------------------------------------------------------------------------------
+// Z[slab][q4][n][v], slab = ((o25 n1 + a1) nl + o35) nl + o45, x = |i1 - l25| + 2v:
+//   (-1)^(o25+o35+o45+q4) sum_{k5 valid} (-1)^q5 {j14 k5 x; l35 k4 l45} {i1 l25 x; k5 j14 j15} (2k5+1) B5[t5][n][q5]
+// one CTA per (slab, q4), one thread per (n, v).
+__global__ void k_line_prep_z(SfProblem P, int NT8, int NXF, double* __restrict__ Z)
+{
+    const int nl = P.nl, n1 = P.n_i[0], n5 = P.n_i[4], P4 = P.n_k_pad[2], P5 = P.n_k_pad[3], NX = P.n_x_pad;
+    long b = blockIdx.x;
+    const int q4 = (int)(b % P4);
+    b /= P4;
+    const long slab = b;
+    const int o45 = (int)(b % nl);
+    b /= nl;
+    const int o35 = (int)(b % nl);
+    b /= nl;
+    const int a1 = (int)(b % n1);
+    const int o25 = (int)(b / n1);
+    const int v = threadIdx.x % NXF, n = threadIdx.x / NXF;
+    const int i1 = P.two_i_min[0] + 2 * a1, l25 = P.two_j[J25] + 2 * o25;
+    const int x0 = abs(i1 - l25), nxs = ((i1 + l25 - x0) >> 1) + 1;
+    const int xg = ((x0 - P.two_x_base) >> 1) + v;
+    const int t5 = (o25 * nl + o35) * nl + o45;
+    const SfKRange r5 = P.kr[3][t5];
+    double val = 0.0;
+    if (n < n5 && v < nxs && r5.n_k > 0) {
+        const int q5b = (r5.two_k_min - P.two_k_base[3]) >> 1;
+        const double* s2 = P.S[1] + ((((long)(o35 * nl + o45) * P4 + q4) * P5 + q5b) * NX) + xg;
+        const double* s1 = P.S[0] + (((long)(o25 * n1 + a1) * P5 + q5b) * NX) + xg;
+        const double* b5 = P.B[3] + ((long)t5 * n5 + n) * P5 + q5b;
+        for (int c = 0; c < r5.n_k; ++c) {
+            double term = s2[(long)c * NX] * s1[(long)c * NX] * ((double)(r5.two_k_min + 2 * c + 1) * b5[c]);
+            if ((q5b + c) & 1) term = -term;
+            val += term;
+        }
+        if ((o25 + o35 + o45 + q4) & 1) val = -val;
+    }
+    Z[(slab * P4 + q4) * (long)(NT8 * NXF) + threadIdx.x] = val;
 }
 
-struct LinePF {                 // operands of the next shell, in flight while the current shell's G2 runs
-    double y[LINE_PFY];
-    double b[2];
+// Bw4[t4][n][c] = (2k4+1) B4[t4][n][q4b + c] for c < K4(t4), n < n4; zero elsewhere.  One CTA per triple.
+__global__ void k_line_prep_b4(SfProblem P, int NT8, int LDK4, double* __restrict__ Bw4)
+{
+    const int t4 = blockIdx.x, n4 = P.n_i[3], P4 = P.n_k_pad[2];
+    const SfKRange r4 = P.kr[2][t4];
+    const int q4b = (r4.two_k_min - P.two_k_base[2]) >> 1;
+    for (int e = threadIdx.x; e < NT8 * LDK4; e += blockDim.x) {
+        const int n = e / LDK4, c = e - n * LDK4;
+        double val = 0.0;
+        if (n < n4 && c < r4.n_k) val = (double)(r4.two_k_min + 2 * c + 1) * P.B[2][((long)t4 * n4 + n) * P4 + q4b + c];
+        Bw4[(long)t4 * NT8 * LDK4 + e] = val;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// the persistent kernel
+// ---------------------------------------------------------------------------------------------------------
+struct LineUnit {
+    long blk, s_begin, s_end;
+    int a1, o23, o24, o25, cb, nslots, q2b, k2min, i1, l25, x0, nxs, ksx, xg0;
+    bool empty;
 };
 
-// loads of the per-shell operands: Y[c4][k5][x] = (-1)^(..) S2 S1 (eq. (5)) and the weighted booster sub-matrices of
-// edges 5 and 4 (step 6(ii)).  Element e of thread tid is e = tid + 512 i.
-template <int NT>
-__device__ __forceinline__ void line_pf_load(const LineParams& lp, const LineShell& S, int tid, int h0, int nxs, int xg0,
-                                             const double* __restrict__ S1s, LinePF& pf)
+__device__ __forceinline__ void line_unit(const LineParams& lp, int unit, LineUnit& u)
 {
     const SfProblem& P = lp.P;
-    const int NT8 = NT * 8, NXF = lp.NXF, LDK = lp.LDK, nl = P.nl, NX = P.n_x_pad;
-    const int P4 = P.n_k_pad[2], P5 = P.n_k_pad[3];
-    const int n_y = S.K4 * NT8 * NXF;
-    const double* s2 = P.S[1] + (((long)(S.o35 * nl + S.o45) * P4 + S.q4b) * P5 + S.q5b) * NX + xg0;
-    const int par0 = h0 + S.osum + S.q4b + S.q5b;
-#pragma unroll
-    for (int i = 0; i < LINE_PFY; ++i) {
-        const int e = tid + LINE_THREADS * i;
-        double val = 0.0;
-        if (e < n_y) {
-            const int v = e % NXF, r = e / NXF, k5c = r % NT8, c4 = r / NT8;
-            if (k5c < S.K5 && v < nxs) {
-                val = s2[((long)c4 * P5 + k5c) * NX + v] * S1s[(S.q5b + k5c) * NXF + v];
-                if ((par0 + c4 + k5c) & 1) val = -val;
-            }
-        }
-        pf.y[i] = val;
-    }
-    const int nb = NT8 * LDK;
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        const int e = tid + LINE_THREADS * i;
-        double val = 0.0;
-        if (e < 2 * nb) {
-            const int which = e / nb, rem = e - which * nb, ii = rem / LDK, c = rem - ii * LDK;
-            if (which == 0) {
-                if (ii < P.n_i[4] && c < S.K5)
-                    val = (double)(S.kmin5 + 2 * c + 1) * P.B[3][((long)S.t5 * P.n_i[4] + ii) * P5 + S.q5b + c];
-            } else {
-                if (ii < P.n_i[3] && c < S.K4)
-                    val = (double)(S.kmin4 + 2 * c + 1) * P.B[2][((long)S.t4 * P.n_i[3] + ii) * P4 + S.q4b + c];
-            }
-        }
-        pf.b[i] = val;
-    }
-}
-
-template <int NT>
-__device__ __forceinline__ void line_pf_store(const LineParams& lp, const LineShell& S, int tid, double* __restrict__ Ys,
-                                              double* __restrict__ Bw5, double* __restrict__ Bw4, const LinePF& pf)
-{
-    const int NT8 = NT * 8, nb = NT8 * lp.LDK;
-    const int n_y = S.K4 * NT8 * lp.NXF;
-#pragma unroll
-    for (int i = 0; i < LINE_PFY; ++i) {
-        const int e = tid + LINE_THREADS * i;
-        if (e < n_y) Ys[e] = pf.y[i];
-    }
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-        const int e = tid + LINE_THREADS * i;
-        if (e < nb)
-            Bw5[e] = pf.b[i];
-        else if (e < 2 * nb)
-            Bw4[e - nb] = pf.b[i];
-    }
+    const int nl = P.nl, n1 = P.n_i[0];
+    int r_ = unit;
+    const int sub = r_ % lp.n_sub; r_ /= lp.n_sub;
+    const int batch = r_ % lp.n_batches; r_ /= lp.n_batches;
+    u.a1 = r_ % n1;
+    u.blk = lp.blk0 + r_ / n1;
+    u.o25 = (int)(u.blk % nl);
+    u.o24 = (int)((u.blk / nl) % nl);
+    u.o23 = (int)(u.blk / ((long)nl * nl));
+    const SfKRange r2 = P.kr[0][u.blk];
+    u.cb = batch * lp.slots;
+    u.nslots = min(lp.slots, r2.n_k - u.cb);
+    u.k2min = r2.two_k_min;
+    u.q2b = (r2.two_k_min - P.two_k_base[0]) >> 1;
+    const int nl2 = nl * nl;
+    const long nl3 = (long)nl2 * nl;
+    u.s_begin = max(u.blk * nl3 + (long)(sub * nl2 / lp.n_sub) * nl, lp.shell_lo);
+    u.s_end = min(u.blk * nl3 + (long)((sub + 1) * nl2 / lp.n_sub) * nl, lp.shell_hi);
+    u.i1 = P.two_i_min[0] + 2 * u.a1;
+    u.l25 = P.two_j[J25] + 2 * u.o25;
+    u.x0 = abs(u.i1 - u.l25);                        // the triad (i1 l25 x) of eq. (5)
+    u.nxs = ((u.i1 + u.l25 - u.x0) >> 1) + 1;
+    u.ksx = (u.nxs + 3) >> 2;
+    u.xg0 = (u.x0 - P.two_x_base) >> 1;
+    u.empty = u.nslots <= 0 || u.s_begin >= u.s_end;
 }
 
 template <int NT, int TPW>
 __global__ void __launch_bounds__(LINE_THREADS, 1) k_vertex_line(const LineParams lp)
 {
     extern __shared__ __align__(16) double smem[];
-    __shared__ unsigned int s_unit;
     const SfProblem& P = lp.P;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
     constexpr int NT8 = NT * 8;
-    constexpr int NKS1 = NT == 1 ? 2 : 4;           // k-steps of G1 (NT == 2: 3 of them when lp.g1_shfl)
-    const int LDK = lp.LDK, NXF = lp.NXF, SLOTS = lp.slots;
-    double* T4 = smem;                               // [rows (s,c3,i5)][LDK]; at a line's end A3 [rows (s,i4,i5)][LDK]
+    const int NXF = lp.NXF, SLOTS = lp.slots, TS4 = lp.TS4, TS3 = lp.TS3, LDK3 = lp.LDK3, LDK4 = lp.LDK4;
+    double* T4 = smem;                               // fragment-major [tile (mt,i5)][k-step][lane]; at a line's end A3
     double* X2 = smem + lp.offX2;                    // T2 sums [SLOTS][n3][n4*n5]
-    double* U = smem + lp.offU;                      // [SLOTS][P3][NXF]
+    double* U = smem + lp.offU;                      // [SLOTS*P3 + 1][NXF], last row zero
     double* S3s = smem + lp.offS3;                   // [K3][P4][NXF]
-    double* Ys = smem + lp.offY;                     // [K4][NT8][NXF]
-    double* S1s = smem + lp.offS1;                   // [P5][NXF]
-    double* Bw5 = smem + lp.offBw;                   // [NT8][LDK] weighted boosters (2k+1) B[i][c], zero padded
-    double* Bw4 = Bw5 + NT8 * LDK;                   // [2][NT8][LDK]
-    double* Bw3 = Bw4 + 2 * NT8 * LDK;               // [NT8][LDK]
-    double* Bw2 = smem + lp.offB2;                   // [n2][SLOTS]
+    double* Zs = smem + lp.offZ;                     // [2][K4max][NT8][NXF]
+    double* Bw4s = smem + lp.offBw4;                 // [2][NT8][LDK4]
+    double* Bw3 = smem + lp.offBw3;                  // [NT8][LDK3]
+    double* Bw2 = smem + lp.offBw2;                  // [n2][SLOTS]
+    int2* rowtab = (int2*)(smem + lp.offRow);        // per row: offsets of its U row and S3s row
+    int2* rowsc = rowtab + lp.mt_max * 8;            // per row: (s, c3), s = -1 beyond the line's rows
+    int2* shtab = (int2*)(smem + lp.offSh);          // [2][nl + 1]: per shell of the line (K4 or 0, q4b); [nl].x = count
+    const unsigned bar0 = smem_u32(smem + lp.offBar);   // full[0], full[1], empty[0], empty[1]
     const int nl = P.nl, n1 = P.n_i[0], n2 = P.n_i[1], n3 = P.n_i[2], n4 = P.n_i[3], n5 = P.n_i[4];
     const int n45 = n4 * n5, R = n3 * n45, NX = P.n_x_pad;
-    const int P2 = P.n_k_pad[0], P3 = P.n_k_pad[1], P4 = P.n_k_pad[2], P5 = P.n_k_pad[3];
+    const int P2 = P.n_k_pad[0], P3 = P.n_k_pad[1], P4 = P.n_k_pad[2];
     const long nl3 = (long)nl * nl * nl;
+    const int zstage = P.k_max[2] * lp.zslab, bstage = NT8 * LDK4;
 
     for (int z = tid; z < lp.n_smem; z += LINE_THREADS) smem[z] = 0.0;   // padding must hold finite values
+    __syncthreads();
+    if (tid == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar0 + 8, 1);
+        mbar_init(bar0 + 16, LINE_WARPS);
+        mbar_init(bar0 + 24, LINE_WARPS);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
 
-    for (;;) {
-        __syncthreads();
-        if (tid == 0) s_unit = atomicAdd(lp.counter, 1u);
-        __syncthreads();
-        const int unit = (int)s_unit;
-        if (unit >= lp.n_units) break;
-        int r_ = unit;
-        const int sub = r_ % lp.n_sub; r_ /= lp.n_sub;
-        const int batch = r_ % lp.n_batches; r_ /= lp.n_batches;
-        const int a1 = r_ % n1;
-        const long blk = lp.blk0 + r_ / n1;
-        const int o25 = (int)(blk % nl), o24 = (int)((blk / nl) % nl), o23 = (int)(blk / ((long)nl * nl));
-        const SfKRange r2 = P.kr[0][blk];
-        const int cb = batch * SLOTS, nslots = min(SLOTS, r2.n_k - cb);
-        const int q2b = (r2.two_k_min - P.two_k_base[0]) >> 1;
-        const int nl2 = nl * nl;
-        long s_begin = blk * nl3 + (long)(sub * nl2 / lp.n_sub) * nl, s_end = blk * nl3 + (long)((sub + 1) * nl2 / lp.n_sub) * nl;
-        s_begin = max(s_begin, lp.shell_lo);
-        s_end = min(s_end, lp.shell_hi);
-        double* dst = lp.partial + (long)unit * n2 * R;
-        const int i1 = P.two_i_min[0] + 2 * a1, l25 = P.two_j[J25] + 2 * o25, j13 = P.two_j[J13];
-        // x-range of the unit: the triad (i1 l25 x) of eq. (5) cut by the triads (k2 j13 x) of the batch's k2 values
-        const int k2f = r2.two_k_min + 2 * cb, k2l = k2f + 2 * (nslots - 1);
-        int x0 = abs(i1 - l25), x1 = i1 + l25;
-        {
-            const int lo2 = (k2f <= j13 && j13 <= k2l) ? ((j13 - k2f) & 1) : min(abs(k2f - j13), abs(k2l - j13));
-            const int hi2 = k2l + j13;
-            if (lo2 > x0) x0 += ((lo2 - x0 + 1) >> 1) << 1;
-            if (hi2 < x1) x1 -= ((x1 - hi2 + 1) >> 1) << 1;
+    // =====================================================================================================
+    // producer warp: for every non-empty shell of this CTA's units, in order, one Z block and one B4 block
+    // =====================================================================================================
+    if (warp == LINE_WARPS) {
+        int st = 0;
+        unsigned pe0 = 1, pe1 = 1;                   // a fresh barrier passes a wait on parity 1
+        for (int unit = blockIdx.x; unit < lp.n_units; unit += gridDim.x) {
+            LineUnit u;
+            line_unit(lp, unit, u);
+            if (u.empty) continue;
+            const long slab0 = (long)(u.o25 * n1 + u.a1) * nl;
+            for (long base = u.s_begin; base < u.s_end; base += 32) {
+                const long shell = base + lane;
+                bool ne = false;
+                long zoff = 0;
+                int zbytes = 0, boff = 0;
+                if (shell < u.s_end) {
+                    const int r = (int)(shell % nl3);
+                    const int o45 = r % nl, o35 = (r / nl) % nl, o34 = r / (nl * nl);
+                    const int t3 = (o34 * nl + o35) * nl + u.o23, t4 = (o45 * nl + u.o24) * nl + o34;
+                    const int t5 = (u.o25 * nl + o35) * nl + o45;
+                    const SfKRange r3 = P.kr[1][t3], r4 = P.kr[2][t4], r5 = P.kr[3][t5];
+                    ne = r3.n_k > 0 && r4.n_k > 0 && r5.n_k > 0;
+                    const int q4b = (r4.two_k_min - P.two_k_base[2]) >> 1;
+                    zoff = (((slab0 + o35) * nl + o45) * P4 + q4b) * (long)lp.zslab;
+                    zbytes = r4.n_k * lp.zslab * 8;
+                    boff = t4 * bstage;
+                }
+                unsigned mask = __ballot_sync(0xffffffffu, ne);
+                while (mask) {
+                    const int l = __ffs(mask) - 1;
+                    mask &= mask - 1;
+                    const long zo = __shfl_sync(0xffffffffu, zoff, l);
+                    const int zb = __shfl_sync(0xffffffffu, zbytes, l), bo = __shfl_sync(0xffffffffu, boff, l);
+                    if (lane == 0) {
+                        const unsigned full = bar0 + 8 * st, empty = bar0 + 16 + 8 * st;
+                        mbar_wait(empty, st ? pe1 : pe0);
+                        mbar_expect_tx(full, (unsigned)zb + (unsigned)bstage * 8u);
+                        bulk_g2s(smem_u32(Zs + st * zstage), lp.Zg + zo, (unsigned)zb, full);
+                        bulk_g2s(smem_u32(Bw4s + st * bstage), lp.Bw4g + bo, (unsigned)bstage * 8u, full);
+                    }
+                    if (st) pe1 ^= 1; else pe0 ^= 1;
+                    st ^= 1;
+                }
+            }
         }
-        const int nxs = x1 >= x0 ? ((x1 - x0) >> 1) + 1 : 0;
-        if (nslots <= 0 || s_begin >= s_end || nxs <= 0) {       // uniform over the CTA
-            for (int z = tid; z < n2 * R; z += LINE_THREADS) dst[z] = 0.0;
+        return;
+    }
+
+    // =====================================================================================================
+    // consumer warps
+    // =====================================================================================================
+    int st = 0;
+    unsigned pf0 = 0, pf1 = 0;
+    int lbuf = 0;                                    // shell-table buffer of the current line
+    int tbase[TPW];                                  // fragment address of this warp's T4 tiles (tile = warp + 16 j)
+#pragma unroll
+    for (int j = 0; j < TPW; ++j) {
+        const int tl = warp + LINE_WARPS * j;
+        tbase[j] = tl * TS4 + (((tl % n5) >> 1) & 3) + lane;
+    }
+    const int st_thread = 2 * q * TS4 + q + 4 * g;   // C-fragment store offset of this lane inside a row tile group
+
+    for (int unit = blockIdx.x; unit < lp.n_units; unit += gridDim.x) {
+        LineUnit u;
+        line_unit(lp, unit, u);
+        double* dst = lp.partial + (long)unit * n2 * R;
+        if (u.empty) {                               // uniform over the CTA
+            for (int z = tid; z < n2 * R; z += LINE_CONSUMERS) dst[z] = 0.0;
             continue;
         }
-        const int xg0 = (x0 - P.two_x_base) >> 1;
+        const int nslots = u.nslots, nxs = u.nxs, KSX = u.ksx, xg0 = u.xg0;
         // (-1)^R, 2R = sum of all fifteen labels (reading G1) = jsum + i1 + sum_a base_a + 2 (sum o + sum q_a)
-        const int h0 = (lp.jsum + i1 + P.two_k_base[0] + P.two_k_base[1] + P.two_k_base[2] + P.two_k_base[3]) >> 1;
+        const int h0 = (lp.jsum + u.i1 + P.two_k_base[0] + P.two_k_base[1] + P.two_k_base[2] + P.two_k_base[3]) >> 1;
+        consumer_bar();                              // the previous unit's G4 has read X2 and Bw2
 
-        // ---- unit constants: U = (-1)^(q2+q3) (2x+1) S5 S4, S1, weighted B2, zeroed T2 sums ----
+        // ---- unit constants: U = (-1)^(h0+o23+o24+q2+q3) (2x+1) S5 S4, weighted B2, zeroed T2 sums ----
         {
-            const double* s5 = P.S[4] + (((long)o25 * n1 + a1) * P2 + q2b + cb) * NX + xg0;
-            const double* s4 = P.S[3] + ((((long)o23 * nl + o24) * P2 + q2b + cb) * P3) * NX + xg0;
-            for (int e = tid; e < SLOTS * P3 * NXF; e += LINE_THREADS) {
+            const int cq2 = u.q2b + u.cb;
+            const double* s5 = P.S[4] + (((long)u.o25 * n1 + u.a1) * P2 + cq2) * NX + xg0;
+            const double* s4 = P.S[3] + ((((long)u.o23 * nl + u.o24) * P2 + cq2) * P3) * NX + xg0;
+            const int par = h0 + u.o23 + u.o24 + cq2;
+            for (int e = tid; e < SLOTS * P3 * NXF; e += LINE_CONSUMERS) {
                 const int v = e % NXF, r = e / NXF, q3 = r % P3, s = r / P3;
                 double val = 0.0;
                 if (s < nslots && v < nxs) {
-                    val = (double)(x0 + 2 * v + 1) * s5[(long)s * NX + v] * s4[((long)s * P3 + q3) * NX + v];
-                    if ((q2b + cb + s + q3) & 1) val = -val;
+                    val = (double)(u.x0 + 2 * v + 1) * s5[(long)s * NX + v] * s4[((long)s * P3 + q3) * NX + v];
+                    if ((par + s + q3) & 1) val = -val;
                 }
                 U[e] = val;
             }
-            const double* s1 = P.S[0] + (((long)o25 * n1 + a1) * P5) * NX + xg0;
-            for (int e = tid; e < P5 * NXF; e += LINE_THREADS) {
-                const int v = e % NXF, q5 = e / NXF;
-                S1s[e] = v < nxs ? s1[(long)q5 * NX + v] : 0.0;
-            }
-            for (int e = tid; e < n2 * SLOTS; e += LINE_THREADS) {
+            for (int e = tid; e < n2 * SLOTS; e += LINE_CONSUMERS) {
                 const int s = e % SLOTS, i2 = e / SLOTS;
-                Bw2[e] = s < nslots ? (double)(r2.two_k_min + 2 * (cb + s) + 1) * P.B[0][((long)blk * n2 + i2) * P2 + q2b + cb + s] : 0.0;
+                Bw2[e] = s < nslots ? (double)(u.k2min + 2 * (u.cb + s) + 1) * P.B[0][((long)u.blk * n2 + i2) * P2 + u.q2b + u.cb + s] : 0.0;
             }
-            for (int e = tid; e < SLOTS * R; e += LINE_THREADS) X2[e] = 0.0;
+            for (int e = tid; e < SLOTS * R; e += LINE_CONSUMERS) X2[e] = 0.0;
         }
-        __syncthreads();                             // S1s is read by the operand loads below
 
         double acc3[TPW][NT][2];
 #pragma unroll
@@ -244,222 +329,185 @@ __global__ void __launch_bounds__(LINE_THREADS, 1) k_vertex_line(const LineParam
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) acc3[j][nt][0] = acc3[j][nt][1] = 0.0;
 
-        // ---- G3 (once per line): T2 sums += sum_c3 T3 . (2k3+1) B3 ----
-        auto flush_line = [&](int K3) {
-            const int rows2 = nslots * K3 * n5, rows3 = nslots * n45;
-#pragma unroll
-            for (int j = 0; j < TPW; ++j) {
-                const int r = (warp + LINE_WARPS * j) * 8 + g;
-                if (r < rows2) {
-                    const int s = r / (K3 * n5), rem = r - s * K3 * n5, c3 = rem / n5, i5 = rem - c3 * n5;
-                    double* a3 = T4 + ((long)(s * n4) * n5 + i5) * LDK + c3;
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) {
-                        const int i4 = nt * 8 + 2 * q;
-                        if (i4 < n4) a3[(long)i4 * n5 * LDK] = acc3[j][nt][0];
-                        if (i4 + 1 < n4) a3[(long)(i4 + 1) * n5 * LDK] = acc3[j][nt][1];
+        for (long line = u.s_begin / nl; line * nl < u.s_end; ++line) {
+            // ---- line constants (step 2 ranges of the line, S3, weighted B3, row tables) ----
+            const int rl = (int)((line * nl) % nl3);
+            const int o35 = (rl / nl) % nl, o34 = rl / (nl * nl);
+            const int t3 = (o34 * nl + o35) * nl + u.o23;
+            const SfKRange r3 = P.kr[1][t3];
+            const int K3 = r3.n_k;
+            if (K3 == 0) continue;                   // uniform
+            const int q3b = (r3.two_k_min - P.two_k_base[1]) >> 1;
+            const int rows1 = nslots * K3, MT1 = (rows1 + 7) >> 3;
+            lbuf ^= 1;
+            int2* sh = shtab + lbuf * (nl + 1);
+            if (warp == 0) {
+                const long shell = line * nl + lane;
+                int K4 = 0, q4b = 0;
+                if (lane < nl && shell >= u.s_begin && shell < u.s_end) {
+                    const int t4 = (lane * nl + u.o24) * nl + o34, t5 = (u.o25 * nl + o35) * nl + lane;
+                    const SfKRange r4 = P.kr[2][t4], r5 = P.kr[3][t5];
+                    if (r4.n_k > 0 && r5.n_k > 0) {
+                        K4 = r4.n_k;
+                        q4b = (r4.two_k_min - P.two_k_base[2]) >> 1;
                     }
                 }
-#pragma unroll
-                for (int nt = 0; nt < NT; ++nt) acc3[j][nt][0] = acc3[j][nt][1] = 0.0;
+                const unsigned any = __ballot_sync(0xffffffffu, K4 > 0);
+                if (lane < nl) sh[lane] = make_int2(K4, q4b);
+                if (lane == 0) sh[nl] = make_int2(__popc(any), 0);
             }
-            __syncthreads();
-            double bq3[NT][4];
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-                for (int ks = 0; ks < 4; ++ks) bq3[nt][ks] = (4 * ks < LDK) ? Bw3[(nt * 8 + g) * LDK + 4 * ks + q] : 0.0;
-            const int ks3 = (K3 + 3) >> 2, ntiles3 = (rows3 + 7) >> 3;
-#pragma unroll
-            for (int j = 0; j < TPW; ++j) {
-                const int tile = warp + LINE_WARPS * j;
-                if (tile < ntiles3) {
-                    const double* a = T4 + (long)(tile * 8 + g) * LDK + q;
-                    double c[NT][2];
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) c[nt][0] = c[nt][1] = 0.0;
-#pragma unroll
-                    for (int ks = 0; ks < 4; ++ks)
-                        if (ks < ks3) {
-                            const double av = a[4 * ks];
-#pragma unroll
-                            for (int nt = 0; nt < NT; ++nt) line_dmma(c[nt][0], c[nt][1], av, bq3[nt][ks]);
-                        }
-                    const int r = tile * 8 + g;
-                    if (r < rows3) {
-                        const int s = r / n45, m = r - s * n45;
-                        double* x2 = X2 + (long)s * R + m;
-#pragma unroll
-                        for (int nt = 0; nt < NT; ++nt) {
-                            const int i3 = nt * 8 + 2 * q;
-                            if (i3 < n3) x2[(long)i3 * n45] += c[nt][0];
-                            if (i3 + 1 < n3) x2[(long)(i3 + 1) * n45] += c[nt][1];
-                        }
-                    }
-                }
-            }
-            __syncthreads();
-        };
-
-        // ---- first non-empty shell of the unit: stage its operands directly ----
-        LineShell S;
-        long shell = s_begin;
-        while (shell < s_end && !line_shell(P, shell, o23, o24, o25, S)) ++shell;
-        int pb = 0;                                  // Bw4 buffer of the current shell
-        if (shell < s_end) {
-            LinePF pf;
-            line_pf_load<NT>(lp, S, tid, h0, nxs, xg0, S1s, pf);
-            line_pf_store<NT>(lp, S, tid, Ys, Bw5, Bw4, pf);
-        }
-        long cur_line = -1;
-        int K3 = 0, q3b = 0;
-
-        while (shell < s_end) {
-            const long line = shell / nl;
-            if (line != cur_line) {
-                if (cur_line >= 0) flush_line(K3);
-                // ---- line constants: S3[c3][q4][x] and the weighted B3 ----
-                K3 = S.K3;
-                q3b = S.q3b;
-                const double* s3 = P.S[2] + (((((long)o24 * nl + S.o34) * nl + S.o35) * P3 + q3b) * P4) * NX + xg0;
-                for (int e = tid; e < K3 * P4 * NXF; e += LINE_THREADS) {
+            {
+                const double* s3 = P.S[2] + (((((long)u.o24 * nl + o34) * nl + o35) * P3 + q3b) * P4) * NX + xg0;
+                const bool neg = o34 & 1;
+                for (int e = tid; e < K3 * P4 * NXF; e += LINE_CONSUMERS) {
                     const int v = e % NXF, r = e / NXF;
-                    S3s[e] = v < nxs ? s3[(long)r * NX + v] : 0.0;
+                    double val = v < nxs ? s3[(long)r * NX + v] : 0.0;
+                    S3s[e] = neg ? -val : val;
                 }
-                for (int e = tid; e < NT8 * LDK; e += LINE_THREADS) {
-                    const int ii = e / LDK, c = e - ii * LDK;
+                for (int e = tid; e < NT8 * LDK3; e += LINE_CONSUMERS) {
+                    const int ii = e / LDK3, c = e - ii * LDK3;
                     Bw3[e] = (ii < n3 && c < K3)
-                                 ? (double)(S.kmin3 + 2 * c + 1) * P.B[1][((long)S.t3 * n3 + ii) * P3 + q3b + c]
+                                 ? (double)(r3.two_k_min + 2 * c + 1) * P.B[1][((long)t3 * n3 + ii) * P3 + q3b + c]
                                  : 0.0;
                 }
-                cur_line = line;
-                __syncthreads();
-            }
-            const int K4 = S.K4, K5 = S.K5, q4b = S.q4b, l35 = P.two_j[J35] + 2 * S.o35;
-
-            // ---- P1: assembly of W (eq. (5)) chained into G1 (contract k5); T4 -> shared memory ----
-            {
-                double bq5[NT][NKS1];
-#pragma unroll
-                for (int nt = 0; nt < NT; ++nt) {
-                    const double* b = Bw5 + (nt * 8 + g) * LDK;
-                    bq5[nt][0] = b[2 * q];
-                    bq5[nt][1] = b[2 * q + 1];
-                    if (NT == 2) {
-                        if (lp.g1_shfl) {            // contracted index of k-step 2 in the order 8 10 9 11
-                            bq5[nt][2] = b[8 + ((q & 1) << 1) + (q >> 1)];
-                            bq5[nt][NKS1 - 1] = 0.0;
-                        } else {
-                            bq5[nt][2] = b[8 + 2 * q];
-                            bq5[nt][NKS1 - 1] = b[9 + 2 * q];
-                        }
+                for (int row = tid; row < lp.mt_max * 8; row += LINE_CONSUMERS) {
+                    if (row < rows1) {
+                        const int s = row / K3, c3 = row - s * K3;
+                        rowtab[row] = make_int2((s * P3 + q3b + c3) * NXF, c3 * P4 * NXF);
+                        rowsc[row] = make_int2(s, c3);
+                    } else {
+                        rowtab[row] = make_int2(SLOTS * P3 * NXF, 0);
+                        rowsc[row] = make_int2(-1, 0);
                     }
                 }
-                const int rows1 = nslots * K3, MT1 = (rows1 + 7) >> 3, ntasks = MT1 * K4;
-                for (int task = warp; task < ntasks; task += LINE_WARPS) {
-                    const int c4 = task / MT1, mt = task - c4 * MT1;
-                    const bool valid = mt * 8 + g < rows1;
-                    const int row = valid ? mt * 8 + g : 0;
-                    const int s = row / K3, c3 = row - s * K3;
-                    const double* up = U + ((long)(s * P3 + q3b + c3)) * NXF + q;
-                    const double* sp = S3s + ((long)(c3 * P4 + q4b + c4)) * NXF + q;
-                    const double* yp = Ys + ((long)(c4 * NT8 + g)) * NXF + q;
+            }
+            consumer_bar();
+            if (sh[nl].x == 0) continue;             // no shell of this line is in range and non-empty (uniform)
+
+            const int mt0 = warp % MT1, c40 = warp / MT1, dm = LINE_WARPS % MT1, dc = LINE_WARPS / MT1;
+            const int ntiles2 = MT1 * n5;
+
+            for (int o45 = 0; o45 < nl; ++o45) {
+                const int2 shd = sh[o45];
+                const int K4 = shd.x, q4b = shd.y;
+                if (K4 == 0) continue;               // uniform
+                mbar_wait(bar0 + 8 * st, st ? pf1 : pf0);
+                if (st) pf1 ^= 1; else pf0 ^= 1;
+                const double* Zc = Zs + st * zstage;
+
+                // ---- P1: T4[r,c4][i5] = sum_x (U S3) Z, C fragments stored in fragment order ----
+                for (int mt = mt0, c4 = c40; c4 < K4;) {
+                    const int2 ro = rowtab[mt * 8 + g];
+                    const double* up = U + ro.x + q;
+                    const double* sp = S3s + ro.y + (q4b + c4) * NXF + q;
+                    const double* zp = Zc + (c4 * NT8 + g) * NXF + q;
                     double c[NT][2];
 #pragma unroll
                     for (int nt = 0; nt < NT; ++nt) c[nt][0] = c[nt][1] = 0.0;
-                    // k-steps of x that the triads (k2 j13 x) of the tile's rows and (k4 l35 x) leave (warp uniform)
-                    int ks_lo, ks_hi;
-                    {
-                        const int sf = (mt * 8) / K3, sl = min(mt * 8 + 7, rows1 - 1) / K3;
-                        const int ka = k2f + 2 * sf, kb = k2f + 2 * sl;
-                        int tlo = (ka <= j13 && j13 <= kb) ? 0 : min(abs(ka - j13), abs(kb - j13)), thi = kb + j13;
-                        const int k4 = S.kmin4 + 2 * c4;
-                        tlo = max(tlo, abs(k4 - l35));
-                        thi = min(thi, k4 + l35);
-                        const int vlo = tlo > x0 ? (tlo - x0 + 1) >> 1 : 0;
-                        const int vhi = thi >= x0 ? min(nxs - 1, (thi - x0) >> 1) : -1;
-                        ks_lo = vlo >> 2;
-                        ks_hi = vhi >= vlo ? vhi >> 2 : ks_lo - 1;
+                    for (int ks = 0; ks < KSX; ++ks) {
+                        const double av = up[4 * ks] * sp[4 * ks];
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) line_dmma(c[nt][0], c[nt][1], av, zp[nt * 8 * NXF + 4 * ks]);
                     }
-                    for (int ks = ks_lo; ks <= ks_hi; ++ks) {
-                        const double av = valid ? up[4 * ks] * sp[4 * ks] : 0.0;
+                    double* t4 = T4 + mt * n5 * TS4 + st_thread + ((c4 >> 2) << 5) + (c4 & 3);
 #pragma unroll
-                        for (int nt = 0; nt < NT; ++nt) line_dmma(c[nt][0], c[nt][1], av, yp[(long)nt * 8 * NXF + 4 * ks]);
+                    for (int nt = 0; nt < NT; ++nt) {
+                        const int i5 = nt * 8 + 2 * q;
+                        if (i5 < n5) t4[(nt * 8) * TS4] = c[nt][0];
+                        if (i5 + 1 < n5) t4[(nt * 8 + 1) * TS4] = c[nt][1];
                     }
-                    // G1: the C fragment (row g; columns 2q, 2q+1 of each n-tile) is the A fragment of k-steps whose
-                    // contracted index runs 2q | 2q+1 | 8+2q (or 8 10 9 11) | 9+2q
-                    double d[NT][2];
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) d[nt][0] = d[nt][1] = 0.0;
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) line_dmma(d[nt][0], d[nt][1], c[0][0], bq5[nt][0]);
-#pragma unroll
-                    for (int nt = 0; nt < NT; ++nt) line_dmma(d[nt][0], d[nt][1], c[0][1], bq5[nt][1]);
-                    if (NT == 2 && K5 > 8) {
-                        if (lp.g1_shfl) {
-                            const double t = __shfl_sync(0xffffffffu, c[NT - 1][1], (lane & ~3) + (q & 1));
-                            const double av = q < 2 ? c[NT - 1][0] : t;
-#pragma unroll
-                            for (int nt = 0; nt < NT; ++nt) line_dmma(d[nt][0], d[nt][1], av, bq5[nt][2]);
-                        } else {
-#pragma unroll
-                            for (int nt = 0; nt < NT; ++nt) line_dmma(d[nt][0], d[nt][1], c[NT - 1][0], bq5[nt][2]);
-#pragma unroll
-                            for (int nt = 0; nt < NT; ++nt) line_dmma(d[nt][0], d[nt][1], c[NT - 1][1], bq5[nt][NKS1 - 1]);
-                        }
-                    }
-                    if (valid) {
-                        double* t4 = T4 + ((long)(s * K3 + c3) * n5) * LDK + c4;
-#pragma unroll
-                        for (int nt = 0; nt < NT; ++nt) {
-                            const int i5 = nt * 8 + 2 * q;
-                            if (i5 < n5) t4[(long)i5 * LDK] = d[nt][0];
-                            if (i5 + 1 < n5) t4[(long)(i5 + 1) * LDK] = d[nt][1];
-                        }
+                    mt += dm;
+                    c4 += dc;
+                    if (mt >= MT1) {
+                        mt -= MT1;
+                        ++c4;
                     }
                 }
-            }
-            __syncthreads();
+                consumer_bar();
 
-            // ---- P2: G2 (contract k4) accumulated in registers over the line; the next shell's operands are fetched
-            //      meanwhile ----
-            LineShell Sn;
-            long next = shell + 1;
-            while (next < s_end && !line_shell(P, next, o23, o24, o25, Sn)) ++next;
-            LinePF pf;
-            if (next < s_end) line_pf_load<NT>(lp, Sn, tid, h0, nxs, xg0, S1s, pf);
-            {
-                double bq4[NT][4];
-                const double* bw = Bw4 + pb * NT8 * LDK;
+                // ---- P2: T3 += sum_c4 T4 . (2k4+1) B4, accumulated in registers over the line ----
+                {
+                    const double* bw = Bw4s + st * bstage + g * LDK4 + q;
+                    const int ks4 = (K4 + 3) >> 2;
+                    for (int ks = 0; ks < ks4; ++ks) {
+                        double bq[NT];
 #pragma unroll
-                for (int nt = 0; nt < NT; ++nt)
-#pragma unroll
-                    for (int ks = 0; ks < 4; ++ks) bq4[nt][ks] = (4 * ks < LDK) ? bw[(nt * 8 + g) * LDK + 4 * ks + q] : 0.0;
-                const int ks4 = (K4 + 3) >> 2, ntiles2 = (nslots * K3 * n5 + 7) >> 3;
-#pragma unroll
-                for (int ks = 0; ks < 4; ++ks)
-                    if (ks < ks4) {
+                        for (int nt = 0; nt < NT; ++nt) bq[nt] = bw[nt * 8 * LDK4 + 4 * ks];
 #pragma unroll
                         for (int j = 0; j < TPW; ++j) {
-                            const int tile = warp + LINE_WARPS * j;
-                            if (tile < ntiles2) {
-                                const double av = T4[(long)(tile * 8 + g) * LDK + q + 4 * ks];
+                            if (warp + LINE_WARPS * j < ntiles2) {
+                                const double av = T4[tbase[j] + (ks << 5)];
 #pragma unroll
-                                for (int nt = 0; nt < NT; ++nt) line_dmma(acc3[j][nt][0], acc3[j][nt][1], av, bq4[nt][ks]);
+                                for (int nt = 0; nt < NT; ++nt) line_dmma(acc3[j][nt][0], acc3[j][nt][1], av, bq[nt]);
                             }
                         }
                     }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar0 + 16 + 8 * st);      // this warp is done with the stage
+                st ^= 1;
+                consumer_bar();
             }
-            if (next < s_end) line_pf_store<NT>(lp, Sn, tid, Ys, Bw5, Bw4 + (pb ^ 1) * NT8 * LDK, pf);
-            pb ^= 1;
-            __syncthreads();
-            shell = next;
-            S = Sn;
+
+            // ---- G3 (once per line): T2 sums += sum_c3 T3 . (2k3+1) B3 ----
+            {
+#pragma unroll
+                for (int j = 0; j < TPW; ++j) {
+                    const int tl = warp + LINE_WARPS * j;
+                    if (tl < ntiles2) {
+                        const int mt = tl / n5, i5 = tl - mt * n5;
+                        const int2 sc = rowsc[mt * 8 + g];
+                        if (sc.x >= 0) {
+                            const int kof = ((sc.y >> 2) << 5) + (sc.y & 3);
+#pragma unroll
+                            for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                                for (int b = 0; b < 2; ++b) {
+                                    const int i4 = nt * 8 + 2 * q + b;
+                                    if (i4 < n4) {
+                                        const int m3 = (sc.x * n4 + i4) * n5 + i5;
+                                        T4[(m3 >> 3) * TS3 + kof + ((m3 & 7) << 2)] = acc3[j][nt][b];
+                                    }
+                                }
+                        }
+                    }
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) acc3[j][nt][0] = acc3[j][nt][1] = 0.0;
+                }
+                consumer_bar();
+                const int rows3 = nslots * n45, ntiles3 = (rows3 + 7) >> 3, ks3 = (K3 + 3) >> 2;
+#pragma unroll
+                for (int j = 0; j < TPW; ++j) {
+                    const int tile = warp + LINE_WARPS * j;
+                    if (tile < ntiles3) {
+                        double c[NT][2];
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) c[nt][0] = c[nt][1] = 0.0;
+                        for (int ks = 0; ks < ks3; ++ks) {
+                            const double av = T4[tile * TS3 + (ks << 5) + lane];
+#pragma unroll
+                            for (int nt = 0; nt < NT; ++nt)
+                                line_dmma(c[nt][0], c[nt][1], av, Bw3[(nt * 8 + g) * LDK3 + 4 * ks + q]);
+                        }
+                        const int r = tile * 8 + g;
+                        if (r < rows3) {
+                            const int s = r / n45, m = r - s * n45;
+                            double* x2 = X2 + (long)s * R + m;
+#pragma unroll
+                            for (int nt = 0; nt < NT; ++nt) {
+                                const int i3 = nt * 8 + 2 * q;
+                                if (i3 < n3) x2[(long)i3 * n45] += c[nt][0];
+                                if (i3 + 1 < n3) x2[(long)(i3 + 1) * n45] += c[nt][1];
+                            }
+                        }
+                    }
+                }
+                consumer_bar();
+            }
         }
-        if (cur_line >= 0) flush_line(K3);
 
         // ---- G4 (once per unit): contract k2; the unit's tensor goes to partial[unit] ----
-        for (int z = tid; z < n2 * R; z += LINE_THREADS) {
+        for (int z = tid; z < n2 * R; z += LINE_CONSUMERS) {
             const int i2 = z / R, r = z - i2 * R;
             double sum = 0.0;
             for (int s = 0; s < nslots; ++s) sum = fma(Bw2[i2 * SLOTS + s], X2[(long)s * R + r], sum);
@@ -500,6 +548,7 @@ struct LinePlan {
     int NT, TPW;
     LineParams lp;
     size_t smem;
+    long z_doubles, b4_doubles;
 };
 
 static int line_max_nxs(const SfDims& D)
@@ -524,57 +573,66 @@ static LinePlan line_plan(const SfDims& D)
         if (D.k_max[e] > kmax) kmax = D.k_max[e];
         if (D.k_max[e] == 0) return pl;
     }
-    if (nmax > 16 || kmax > 16) return pl;
-    const int nxs_all = line_max_nxs(D);
+    if (nmax > 16 || kmax > 16 || D.nl > 32) return pl;
+    const int nxs = line_max_nxs(D);
+    if (nxs > 28) return pl;
     LineParams& lp = pl.lp;
-    pl.NT = (nmax <= 8 && kmax <= 8) ? 1 : 2;
+    pl.NT = nmax <= 8 ? 1 : 2;
     const int NT8 = pl.NT * 8;
-    lp.LDK = kmax <= 12 ? 12 : 20;
-    lp.g1_shfl = (pl.NT == 2 && kmax <= 12) ? 1 : 0;
+    lp.NXF = nxs <= 4 ? 4 : nxs <= 12 ? 12 : nxs <= 20 ? 20 : 28;
+    lp.KS3 = (D.k_max[1] + 3) / 4;
+    lp.KS4 = (D.k_max[2] + 3) / 4;
+    lp.LDK3 = 4 * lp.KS3;
+    lp.LDK4 = 4 * lp.KS4;
+    lp.TS4 = 32 * lp.KS4 + 4;
+    lp.TS3 = 32 * lp.KS3;
+    lp.zslab = NT8 * lp.NXF;
     lp.jsum = 0;
     for (int s = 0; s < 10; ++s) lp.jsum += D.two_j[s];
     const int n2 = D.n_i[1], n3 = D.n_i[2], n4 = D.n_i[3], n5 = D.n_i[4];
-    const int P3 = D.n_k_pad[1], P4 = D.n_k_pad[2], P5 = D.n_k_pad[3];
-    static const int tpws[] = {1, 2, 4, 6, 8};
+    const int P3 = D.n_k_pad[1], P4 = D.n_k_pad[2];
+    const long slabs = (long)D.nl * D.n_i[0] * D.nl * D.nl;
+    pl.z_doubles = slabs * P4 * lp.zslab;
+    pl.b4_doubles = (long)D.nl * D.nl * D.nl * NT8 * lp.LDK4;
+    if (pl.z_doubles * 8 > (16L << 30)) return pl;
     for (int nb = 1; nb <= D.k_max[0]; ++nb) {
         const int slots = (D.k_max[0] + nb - 1) / nb;
-        // x values a unit can see: the triad (i1 l25 x) cut by the triads (k2 j13 x) of `slots` consecutive k2
-        int nxs = D.two_j[J13] + slots;
-        if (nxs_all < nxs) nxs = nxs_all;
-        if (nxs > 28) continue;
-        lp.NXF = nxs <= 4 ? 4 : nxs <= 12 ? 12 : nxs <= 20 ? 20 : 28;
-        if (D.k_max[2] * NT8 * lp.NXF > LINE_PFY * LINE_THREADS) continue;
-        int rows = D.k_max[1] * n5 > n4 * n5 ? D.k_max[1] * n5 : n4 * n5;
-        rows *= slots;
-        const int tiles = (rows + 7) / 8, tpw = (tiles + LINE_WARPS - 1) / LINE_WARPS;
-        int TPW = 0;
-        for (int t : tpws)
-            if (t >= tpw) {
-                TPW = t;
-                break;
-            }
-        if (!TPW) continue;
-        int off = (tiles * 8 + 8) * lp.LDK;
+        const int mt_max = (slots * D.k_max[1] + 7) / 8;
+        const int tiles2 = mt_max * n5, tiles3 = (slots * n4 * n5 + 7) / 8;
+        const int tiles = tiles2 > tiles3 ? tiles2 : tiles3;
+        const int TPW = (tiles + LINE_WARPS - 1) / LINE_WARPS;
+        if (TPW > 8) continue;
+        int off = tiles2 * lp.TS4 + 8;
+        if (tiles3 * lp.TS3 > off) off = tiles3 * lp.TS3;
+        off = (off + 1) & ~1;
         lp.offX2 = off;
         off += slots * n3 * n4 * n5;
         off = (off + 1) & ~1;
         lp.offU = off;
-        off += (slots * P3 + 8) * lp.NXF;
+        off += (slots * P3 + 1) * lp.NXF;
         lp.offS3 = off;
-        off += (D.k_max[1] * P4 + 8) * lp.NXF;
-        lp.offY = off;
-        off += (D.k_max[2] * NT8 + 8) * lp.NXF;
-        lp.offS1 = off;
-        off += P5 * lp.NXF;
-        lp.offBw = off;
-        off += 4 * NT8 * lp.LDK;
-        lp.offB2 = off;
+        off += D.k_max[1] * P4 * lp.NXF;
+        off = (off + 1) & ~1;
+        lp.offZ = off;
+        off += 2 * D.k_max[2] * lp.zslab;
+        lp.offBw4 = off;
+        off += 2 * NT8 * lp.LDK4;
+        lp.offBw3 = off;
+        off += NT8 * lp.LDK3;
+        lp.offBw2 = off;
         off += n2 * slots;
         off = (off + 1) & ~1;
+        lp.offRow = off;
+        off += 2 * mt_max * 8;
+        lp.offSh = off;
+        off += 2 * (D.nl + 1);
+        lp.offBar = off;
+        off += 4;
         lp.n_smem = off;
-        if (sizeof(double) * (size_t)off > 224 * 1024) continue;
+        if (sizeof(double) * (size_t)off > 226 * 1024) continue;
         pl.TPW = TPW;
         lp.slots = slots;
+        lp.mt_max = mt_max;
         lp.n_batches = nb;
         pl.smem = sizeof(double) * (size_t)off;
         pl.ok = true;
@@ -590,7 +648,7 @@ static int launch_line(const LinePlan& pl, int grid, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_vertex_line<NT, TPW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_vertex_line<NT, TPW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024) != cudaSuccess)
             return SF_ECUDA;
         attr_set = true;
     }
@@ -613,7 +671,7 @@ int sf_vertex_line(const SfDims& D, const SfProblem& P, long shell_lo, long shel
     lp.shell_lo = shell_lo;
     lp.shell_hi = shell_hi;
     const long nl3 = (long)D.nl * D.nl * D.nl;
-    const int n1 = D.n_i[0];
+    const int n1 = D.n_i[0], NT8 = pl.NT * 8;
     if (shell_hi > shell_lo) {
         lp.blk0 = shell_lo / nl3;
         lp.n_blocks = (int)((shell_hi - 1) / nl3 - lp.blk0 + 1);
@@ -632,18 +690,23 @@ int sf_vertex_line(const SfDims& D, const SfProblem& P, long shell_lo, long shel
     lp.n_units = (int)(base_units * lp.n_sub);
     const long slice = D.n_out / n1;
     double* partial = (double*)sf_scratch(17, sizeof(double) * (size_t)(lp.n_units > 0 ? lp.n_units : 1) * slice);
-    unsigned int* counter = (unsigned int*)sf_scratch(18, 256);
-    if (!partial || !counter) return SF_ENOMEM;
+    double* Zg = (double*)sf_scratch(19, sizeof(double) * (size_t)pl.z_doubles);
+    double* Bw4g = (double*)sf_scratch(20, sizeof(double) * (size_t)pl.b4_doubles);
+    if (!partial || !Zg || !Bw4g) return SF_ENOMEM;
     lp.partial = partial;
-    lp.counter = counter;
+    lp.Zg = Zg;
+    lp.Bw4g = Bw4g;
     if (lp.n_units > 0) {
-        SF_CUDA_OK(cudaMemsetAsync(counter, 0, sizeof(unsigned int), st));
+        const long slabs = (long)D.nl * n1 * D.nl * D.nl;
+        k_line_prep_z<<<(unsigned)(slabs * D.n_k_pad[2]), lp.zslab, 0, st>>>(P, NT8, lp.NXF, Zg);
+        k_line_prep_b4<<<(unsigned)nl3, 128, 0, st>>>(P, NT8, lp.LDK4, Bw4g);
+        sf_count_launch(2);
         const int grid = lp.n_units < n_sm ? lp.n_units : n_sm;
         int rc = SF_EARG;
 #define SF_SHAPE(a, b) \
     if (pl.NT == a && pl.TPW == b) rc = launch_line<a, b>(pl, grid, st);
-        SF_SHAPE(1, 1) SF_SHAPE(1, 2) SF_SHAPE(1, 4) SF_SHAPE(1, 6) SF_SHAPE(1, 8)
-        SF_SHAPE(2, 1) SF_SHAPE(2, 2) SF_SHAPE(2, 4) SF_SHAPE(2, 6) SF_SHAPE(2, 8)
+        SF_SHAPE(1, 1) SF_SHAPE(1, 2) SF_SHAPE(1, 3) SF_SHAPE(1, 4) SF_SHAPE(1, 5) SF_SHAPE(1, 6) SF_SHAPE(1, 7) SF_SHAPE(1, 8)
+        SF_SHAPE(2, 1) SF_SHAPE(2, 2) SF_SHAPE(2, 3) SF_SHAPE(2, 4) SF_SHAPE(2, 5) SF_SHAPE(2, 6) SF_SHAPE(2, 7) SF_SHAPE(2, 8)
 #undef SF_SHAPE
         if (rc != SF_OK) return rc;
         sf_count_launch(1);
