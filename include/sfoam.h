@@ -127,10 +127,18 @@ long sf_launch_count(int reset);
 int sf_set_timing(int on);
 int sf_last_stage_ms(double ms[3]);
 
-/* Path selection for steps 5-7.  0 = automatic: the fused on-chip path when one i1-slice of the tensor fits the SM
- * (accumulators in registers, intermediates in shared memory), the staged path (intermediates through global memory,
- * split along i1 when needed: PAPER.md:184-186) otherwise.  1 = staged, 2 = fused (the vertex calls then return
- * SF_EARG for tensors the fused path cannot hold).  sf_last_path() = path the last vertex call took (1 or 2). */
+/* Path selection for steps 5-7.  All paths compute the same sum of eq. (3); they differ in the
+ * order of the additions only.
+ *   0 = automatic: the fastest path that supports the problem's sizes (4, else 3, else 2, else 1)
+ *   1 = staged: per batch of shells, {15j} assembly and the four mode products as separate kernels with intermediates
+ *       in global memory, split along i1 when needed; any size
+ *   2 = fused: one kernel per chunk of shells, accumulators in registers, intermediates in shared memory
+ *   3 = line: persistent per-shell kernel (x-sum of eq. (5) and the k4 product per shell, k3 / k2 products per line /
+ *       block of shells by linearity); every intertwiner range <= 16 values
+ *   4 = factorised: the sums over the virtual spins are taken one spin at a time with x kept open (Q = sum_l45,
+ *       R = sum_{l34 l35}, A' = sum_l23, A = sum_{l24 l25}); same terms, far fewer operations
+ * The vertex calls return SF_EARG when the selected path cannot hold the problem.  sf_last_path() = path the last
+ * vertex call took (1..4). */
 int sf_set_path(int path);
 int sf_last_path(void);
 /* Bytes of global scratch the staged path may use for its two ping-pong buffers (default 6 GiB). */

@@ -6,7 +6,7 @@
 
 #include "sf_internal.h"
 
-#define SF_NSCRATCH 24
+#define SF_NSCRATCH 40
 enum { SLOT_ACC = 0, SLOT_BUF0 = 1, SLOT_BUF1 = 2, SLOT_S = 3 /*..7*/, SLOT_KR = 8 /*..11*/, SLOT_HB = 12 /*..15*/,
        SLOT_HOUT = 16, SLOT_PART = 17, SLOT_MISC = 18 };
 
@@ -131,7 +131,7 @@ extern "C" int sf_last_stage_ms(double ms[3])
 // 0 = automatic (fused on-chip path when the tensor fits, staged path otherwise), 1 = staged, 2 = fused
 extern "C" int sf_set_path(int path)
 {
-    if (path < 0 || path > 3) return SF_EARG;
+    if (path < 0 || path > 4) return SF_EARG;
     g_ctx.path = path;
     return SF_OK;
 }
@@ -228,11 +228,13 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
 
     // steps 5-7
     const bool line_ok = sf_vertex_line_supported(D), fused_ok = sf_vertex_fused_supported(D);
-    if ((g_ctx.path == 2 && !fused_ok) || (g_ctx.path == 3 && !line_ok)) return SF_EARG;
+    const bool factor_ok = sf_vertex_factor_supported(D);
+    if ((g_ctx.path == 2 && !fused_ok) || (g_ctx.path == 3 && !line_ok) || (g_ctx.path == 4 && !factor_ok)) return SF_EARG;
     int path = g_ctx.path;
-    if (path == 0) path = line_ok ? 3 : fused_ok ? 2 : 1;
+    if (path == 0) path = factor_ok ? 4 : line_ok ? 3 : fused_ok ? 2 : 1;
     g_ctx.last_path = path;
-    rc = path == 3   ? sf_vertex_line(D, P, shell_lo, shell_hi, out, st)
+    rc = path == 4   ? sf_vertex_factor(D, P, shell_lo, shell_hi, out, st)
+         : path == 3 ? sf_vertex_line(D, P, shell_lo, shell_hi, out, st)
          : path == 2 ? sf_vertex_fused(D, P, shell_lo, shell_hi, out, st)
                      : sf_vertex_staged(D, P, shell_lo, shell_hi, out, st);
     if (rc != SF_OK) return rc;

@@ -96,6 +96,8 @@ int sf_vertex_fused(const SfDims& D, const SfProblem& P, long shell_lo, long she
 bool sf_vertex_fused_supported(const SfDims& D);
 int sf_vertex_line(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
 bool sf_vertex_line_supported(const SfDims& D);
+int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
+bool sf_vertex_factor_supported(const SfDims& D);
 
 // scratch allocator owned by the context: grows on demand, freed by sf_finalize.  slot = small integer id.
 void* sf_scratch(int slot, size_t bytes);

@@ -1,0 +1,886 @@
+// sf_vertex_factor.cu -- the factorised path of steps 5-7 of the vertex-tensor algorithm.
+//
+// Eq. (3) with the {15j} of eq. (5) written out is one big multilinear sum
+//
+//   A[i1..i5] = N(i) sum_{l23..l45} sum_{k2..k5} sum_x  (-1)^R (2x+1) S1 S2 S3 S4 S5  Bw2 Bw3 Bw4 Bw5 ,   Bw_a = (2k_a+1) B_a
+//
+// in which every booster depends on three of the six virtual spins only and every {6j} tensor S_n
+// of step 4 on at most three.  The paper's loop (steps 5-6) builds the {15j} of
+// one shell and contracts it with that shell's four boosters; by linearity the same sum can be taken one virtual spin
+// at a time, keeping the recoupling spin x open.  The order used here, all FP64:
+//
+//   Z [l25 i1 l35 l45; k4 x i5]        = sum_k5   S2 S1 Bw5                      (k_fz_z: two {6j} of eq. (5) and the edge-5 product)
+//   Q [.. l24 l34; k4 x i5 i4]         = sum_l45  Z Bw4                          (k_fz_qp, first half: the shells of a line l45 = j..j+Dl)
+//   P [l24 l25 i1; k3 x; l34 l35; i5 i4] = sum_k4 S3 Q                           (k_fz_qp, second half: third {6j}, edge-4 mode product)
+//   R [l24 l25 i1; k3 x; l23 i3; i5 i4]  = sum_{l34 l35} Bw3 P                   (k_fz_gemm<FzMapR>: edge-3 mode product + shell sum)
+//   G [l23 l24 l25 i1; k3 x; i2]       = sum_k2   Bw2 (-1)^.. (2x+1) S5 S4       (k_fz_g: last two {6j}, edge-2 booster)
+//   A'[l24 l25; i1 i2 i3 i4 i5]        = sum_{k3 x l23} G R                      (k_fz_gemm<FzMapA>: sum over x of eq. (5), edge-2 product)
+//   A [i1..i5]                         = N(i) sum_{l24 l25} A'                   (k_fz_reduce: fixed order, step 6(iv) + eq. (3))
+//
+// Every term of the paper's sum is still there, exactly once; only the order of the additions differs, so the result
+// agrees with the per-shell paths (sf_vertex_line.cu) to rounding.  The {6j} tensors are exactly 0 where a triad
+// fails (sf_slices.cu) and the weighted boosters are masked to each triple's own k-range (reading G9), so the dense
+// index ranges used below add only exact zeros.  All sums run in a fixed order: bitwise reproducible.
+//
+// Every product is an FP64 tensor-core MMA (mma.sync m8n8k4 f64, SASS DMMA.8x8x4).  The two big contractions (R, A')
+// are gather-GEMMs: C[m][n] = sum_k A[k][m] B[k][n] with per-index offset tables built from the spin ranges, so the
+// irregular ranges of the spin-foam sum (step 2) turn into plain index lists.
+//
+// A sub-range of the canonical shell order (sf_vertex_amplitude_range) is split into at most 11 boxes of virtual-spin
+// offsets (digit decomposition in base Dl+1); the factorisation applies to each box.
+#include <stdio.h>
+#include <string.h>
+
+#include "sf_internal.h"
+
+// a box of shell offsets, order (o23 o24 o25 o34 o35 o45); o = lo .. lo + cnt - 1
+struct FzBox {
+    int lo[6], cnt[6];
+};
+
+struct FzParams {
+    SfProblem P;
+    FzBox box;
+    int a_lo, a_cnt;            // the boundary intertwiners i1 of this pass (a1 = a_lo .. a_lo + a_cnt - 1)
+    int V;                      // largest number of x values of any (i1, l25): triad (i1 l25 x) of eq. (5)
+    int NP;                     // n5 * n4 rounded up to even: row length of P and R
+    int jsum;                   // sum of the ten boundary spins (2j units)
+    int W3p, W4p, LDQ, LDS3, VG;   // k_fz_qp shared-memory shape
+    const int2* w3A;            // [o34][o35] window (lo, cnt) of q3 allowed by the pair (l34 l35)
+    const int2* w3B;            // [o23]      window of q3 allowed by the pair (j13 l23)
+    const int2* w4A;            // [o24][o34] window of q4 allowed by the pair (l24 l34)
+    const int2* w4B;            // [o45]      window of q4 allowed by the pair (l45 j14)
+    int2 hull4B;                // union of w4B over the box: (lo, hi exclusive)
+    const double* Z;            // [b25][a1][b35][b45][q4][v][i5]
+    const double* Bw4T;         // [q4][b45][b24][b34][i4]
+    const double* Bw3T;         // [q3][b34][b35][b23][i3]
+    const double* S3T;          // [b24][b34][b35][xx][q3][q4], sign (-1)^o34 folded in
+    const double* G;            // [b24][b25][a1][q3][v][b23][i2]
+    double* Pq;                 // [ac][b24][b25][q3][v][b34][b35][NP]
+    double* Rq;                 // [ac][b24][b25][q3][v][b23][i3][NP]
+    double* Apart;              // [part][a1][i2][i3][i4][i5]
+    long part0;                 // first partial tensor of this box
+};
+
+// window (lo, cnt) of q = (k - k_base) / 2 inside [0, n_pad) allowed by the triangle |a - b| <= k <= a + b
+__host__ __device__ inline int2 fz_window(int a, int b, int two_k_base, int n_pad)
+{
+    int lo_k = a > b ? a - b : b - a;
+    const int hi_k = a + b;
+    int2 w;
+    w.x = 0;
+    w.y = 0;
+    if ((lo_k - two_k_base) & 1) return w;
+    int qlo = (lo_k - two_k_base) / 2, qhi = (hi_k - two_k_base) / 2;
+    if (qlo < 0) qlo = 0;
+    if (qhi > n_pad - 1) qhi = n_pad - 1;
+    if (qhi < qlo) return w;
+    w.x = qlo;
+    w.y = qhi - qlo + 1;
+    return w;
+}
+
+// x values of the triad (i1 l25 x): first x, count, index of the first in the S arrays' x layout
+__host__ __device__ inline void fz_xrange(const int two_i1_min, int two_j25, int two_x_base, int a1, int o25, int& x0,
+                                          int& nxs, int& xg0)
+{
+    const int i1 = two_i1_min + 2 * a1, l25 = two_j25 + 2 * o25;
+    x0 = i1 > l25 ? i1 - l25 : l25 - i1;
+    nxs = ((i1 + l25 - x0) >> 1) + 1;
+    xg0 = (x0 - two_x_base) >> 1;
+}
+
+__device__ __forceinline__ void fz_dmma(double& c0, double& c1, double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};\n"
+        : "+d"(c0), "+d"(c1)
+        : "d"(a), "d"(b));
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// small precomputations (step 2 windows, weighted / transposed operands)
+// ---------------------------------------------------------------------------------------------------------
+__global__ void k_fz_windows(SfProblem P, int2* w3A, int2* w3B, int2* w4A, int2* w4B)
+{
+    const int nl = P.nl, t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int* j = P.two_j;
+    if (t < nl * nl) {
+        const int u = t / nl, v = t % nl;
+        w3A[t] = fz_window(j[J34] + 2 * u, j[J35] + 2 * v, P.two_k_base[1], P.n_k_pad[1]);
+        w4A[t] = fz_window(j[J24] + 2 * u, j[J34] + 2 * v, P.two_k_base[2], P.n_k_pad[2]);
+    }
+    if (t < nl) {
+        w3B[t] = fz_window(j[J13], j[J23] + 2 * t, P.two_k_base[1], P.n_k_pad[1]);
+        w4B[t] = fz_window(j[J45] + 2 * t, j[J14], P.two_k_base[2], P.n_k_pad[2]);
+    }
+}
+
+// Z[b25][a1][b35][b45][q4][v][i5] = (-1)^(o25+o35+o45+q4) sum_{k5 valid} (-1)^q5 {j14 k5 x; l35 k4 l45} {i1 l25 x; k5 j14 j15} (2k5+1) B5[t5][i5][q5]
+// one CTA per (b25, a1, b35, b45)
+__global__ void __launch_bounds__(256) k_fz_z(FzParams p, double* __restrict__ Z)
+{
+    const SfProblem& P = p.P;
+    const int nl = P.nl, n1 = P.n_i[0], n5 = P.n_i[4], P4 = P.n_k_pad[2], P5 = P.n_k_pad[3], NX = P.n_x_pad, V = p.V;
+    const int c35 = p.box.cnt[4], c45 = p.box.cnt[5];
+    long b = blockIdx.x;
+    const int b45 = (int)(b % c45); b /= c45;
+    const int b35 = (int)(b % c35); b /= c35;
+    const int a1 = (int)(b % n1);
+    const int b25 = (int)(b / n1);
+    const int o25 = p.box.lo[2] + b25, o35 = p.box.lo[4] + b35, o45 = p.box.lo[5] + b45;
+    int x0, nxs, xg0;
+    fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
+    const int t5 = (o25 * nl + o35) * nl + o45;
+    const SfKRange r5 = P.kr[3][t5];
+    const int q5b = (r5.two_k_min - P.two_k_base[3]) >> 1;
+    double* z = Z + (long)blockIdx.x * P4 * V * n5;
+    for (int e = threadIdx.x; e < P4 * nxs * n5; e += blockDim.x) {
+        const int i5 = e % n5, r = e / n5, v = r % nxs, q4 = r / nxs;
+        const double* s2 = P.S[1] + ((((long)(o35 * nl + o45) * P4 + q4) * P5 + q5b) * NX) + xg0 + v;
+        const double* s1 = P.S[0] + (((long)(o25 * n1 + a1) * P5 + q5b) * NX) + xg0 + v;
+        const double* b5 = P.B[3] + ((long)t5 * n5 + i5) * P5 + q5b;
+        double val = 0.0;
+        for (int c = 0; c < r5.n_k; ++c) {
+            double term = s2[(long)c * NX] * s1[(long)c * NX] * ((double)(r5.two_k_min + 2 * c + 1) * b5[c]);
+            if ((q5b + c) & 1) term = -term;
+            val += term;
+        }
+        if ((o25 + o35 + o45 + q4) & 1) val = -val;
+        z[(q4 * V + v) * n5 + i5] = val;
+    }
+}
+
+// Bw4T[q4][b45][b24][b34][i4] = (2k4+1) B4[(o45 o24 o34)][i4][q4] inside the triple's k-range, 0 outside
+__global__ void __launch_bounds__(256) k_fz_b4t(FzParams p, long n, double* __restrict__ out)
+{
+    const SfProblem& P = p.P;
+    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int nl = P.nl, n4 = P.n_i[3], P4 = P.n_k_pad[2];
+    const int c24 = p.box.cnt[1], c34 = p.box.cnt[3], c45 = p.box.cnt[5];
+    long r = e;
+    const int i4 = (int)(r % n4); r /= n4;
+    const int b34 = (int)(r % c34); r /= c34;
+    const int b24 = (int)(r % c24); r /= c24;
+    const int b45 = (int)(r % c45);
+    const int q4 = (int)(r / c45);
+    const int t4 = ((p.box.lo[5] + b45) * nl + p.box.lo[1] + b24) * nl + p.box.lo[3] + b34;
+    const SfKRange r4 = P.kr[2][t4];
+    const int c = q4 - ((r4.two_k_min - P.two_k_base[2]) >> 1);
+    double val = 0.0;
+    if (c >= 0 && c < r4.n_k) val = (double)(r4.two_k_min + 2 * c + 1) * P.B[2][((long)t4 * n4 + i4) * P4 + q4];
+    out[e] = val;
+}
+
+// Bw3T[q3][b34][b35][b23][i3] = (2k3+1) B3[(o34 o35 o23)][i3][q3] inside the triple's k-range, 0 outside
+__global__ void __launch_bounds__(256) k_fz_b3t(FzParams p, long n, double* __restrict__ out)
+{
+    const SfProblem& P = p.P;
+    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int nl = P.nl, n3 = P.n_i[2], P3 = P.n_k_pad[1];
+    const int c23 = p.box.cnt[0], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
+    long r = e;
+    const int i3 = (int)(r % n3); r /= n3;
+    const int b23 = (int)(r % c23); r /= c23;
+    const int b35 = (int)(r % c35); r /= c35;
+    const int b34 = (int)(r % c34);
+    const int q3 = (int)(r / c34);
+    const int t3 = ((p.box.lo[3] + b34) * nl + p.box.lo[4] + b35) * nl + p.box.lo[0] + b23;
+    const SfKRange r3 = P.kr[1][t3];
+    const int c = q3 - ((r3.two_k_min - P.two_k_base[1]) >> 1);
+    double val = 0.0;
+    if (c >= 0 && c < r3.n_k) val = (double)(r3.two_k_min + 2 * c + 1) * P.B[1][((long)t3 * n3 + i3) * P3 + q3];
+    out[e] = val;
+}
+
+// S3T[b24][b34][b35][xx][q3][q4] = (-1)^o34 {k4 l35 x; k3 l24 l34}
+__global__ void __launch_bounds__(256) k_fz_s3t(FzParams p, long n, double* __restrict__ out)
+{
+    const SfProblem& P = p.P;
+    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int nl = P.nl, P3 = P.n_k_pad[1], P4 = P.n_k_pad[2], NX = P.n_x_pad;
+    const int c34 = p.box.cnt[3], c35 = p.box.cnt[4];
+    long r = e;
+    const int q4 = (int)(r % P4); r /= P4;
+    const int q3 = (int)(r % P3); r /= P3;
+    const int xx = (int)(r % NX); r /= NX;
+    const int b35 = (int)(r % c35); r /= c35;
+    const int b34 = (int)(r % c34);
+    const int b24 = (int)(r / c34);
+    const int o24 = p.box.lo[1] + b24, o34 = p.box.lo[3] + b34, o35 = p.box.lo[4] + b35;
+    const double val = P.S[2][(((((long)o24 * nl + o34) * nl + o35) * P3 + q3) * P4 + q4) * NX + xx];
+    out[e] = (o34 & 1) ? -val : val;
+}
+
+// G[b24][b25][a1][q3][v][b23][i2] = sum_{k2 valid} (2k2+1) B2[(o23 o24 o25)][i2][q2] (-1)^(h0+o23+o24+q2+q3) (2x+1)
+//                                   {k2 j13 x; i1 l25 j12} {l24 k3 x; j13 k2 l23}
+// h0 = (sum of boundary spins + i1 + sum of the k bases) / 2: with the signs folded into Z and S3T this is the
+// (-1)^R of eq. (5), 2R = sum of all fifteen labels (reading G1)
+__global__ void __launch_bounds__(256) k_fz_g(FzParams p, long n, double* __restrict__ out)
+{
+    const SfProblem& P = p.P;
+    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int nl = P.nl, n1 = P.n_i[0], n2 = P.n_i[1], P2 = P.n_k_pad[0], P3 = P.n_k_pad[1], NX = P.n_x_pad, V = p.V;
+    const int c23 = p.box.cnt[0], c25 = p.box.cnt[2];
+    long r = e;
+    const int i2 = (int)(r % n2); r /= n2;
+    const int b23 = (int)(r % c23); r /= c23;
+    const int v = (int)(r % V); r /= V;
+    const int q3 = (int)(r % P3); r /= P3;
+    const int a1 = (int)(r % n1); r /= n1;
+    const int b25 = (int)(r % c25);
+    const int b24 = (int)(r / c25);
+    const int o23 = p.box.lo[0] + b23, o24 = p.box.lo[1] + b24, o25 = p.box.lo[2] + b25;
+    int x0, nxs, xg0;
+    fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
+    double val = 0.0;
+    if (v < nxs) {
+        const int blk = (o23 * nl + o24) * nl + o25;
+        const SfKRange r2 = P.kr[0][blk];
+        const int q2b = (r2.two_k_min - P.two_k_base[0]) >> 1;
+        const int i1 = P.two_i_min[0] + 2 * a1;
+        const int h0 = (p.jsum + i1 + P.two_k_base[0] + P.two_k_base[1] + P.two_k_base[2] + P.two_k_base[3]) >> 1;
+        const double* s5 = P.S[4] + (((long)o25 * n1 + a1) * P2 + q2b) * NX + xg0 + v;
+        const double* s4 = P.S[3] + ((((long)o23 * nl + o24) * P2 + q2b) * P3 + q3) * NX + xg0 + v;
+        const double* b2 = P.B[0] + ((long)blk * n2 + i2) * P2 + q2b;
+        for (int c = 0; c < r2.n_k; ++c) {
+            double term = (double)(r2.two_k_min + 2 * c + 1) * b2[c] * s5[(long)c * NX] * s4[(long)c * P3 * NX];
+            if ((q2b + c) & 1) term = -term;
+            val += term;
+        }
+        val *= (double)(x0 + 2 * v + 1);
+        if ((h0 + o23 + o24 + q3) & 1) val = -val;
+    }
+    out[e] = val;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// k_fz_qp: Q = sum_l45 Z Bw4 and P = sum_k4 S3 Q for one (i1, l25, l35, l24, l34), a few x at a time
+// ---------------------------------------------------------------------------------------------------------
+// Q phase, per k4:  C[(v i5)][i4] = sum_l45 Z[l45][k4][(v i5)] Bw4T[k4][l45][i4]        (A and B fragments straight from L1/L2)
+// P phase, per v:   P[k3][(i5 i4)] = sum_k4 S3[k3][k4] Q[k4][(i5 i4)]                   (both operands in shared memory)
+#define FZ_QP_THREADS 256
+__global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
+{
+    extern __shared__ __align__(16) double smem[];
+    const SfProblem& P = p.P;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
+    const int nl = P.nl, n1 = P.n_i[0], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5;
+    const int P3 = P.n_k_pad[1], P4 = P.n_k_pad[2], NX = P.n_x_pad, V = p.V, NP = p.NP;
+    const int c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4], c45 = p.box.cnt[5];
+    const int W3p = p.W3p, W4p = p.W4p, LDQ = p.LDQ, LDS3 = p.LDS3, VG = p.VG;
+    long it = blockIdx.x;
+    const int b34 = (int)(it % c34); it /= c34;
+    const int b24 = (int)(it % c24); it /= c24;
+    const int b35 = (int)(it % c35); it /= c35;
+    const int b25 = (int)(it % c25);
+    const int ac = (int)(it / c25);
+    const int a1 = p.a_lo + ac;
+    const int o24 = p.box.lo[1] + b24, o25 = p.box.lo[2] + b25, o34 = p.box.lo[3] + b34, o35 = p.box.lo[4] + b35;
+    int x0, nxs, xg0;
+    fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
+    const int2 w3 = p.w3A[o34 * nl + o35];           // every k3 the pair (l34 l35) allows gets a row of P
+    if (w3.y == 0) return;
+    const int2 w4a = p.w4A[o24 * nl + o34];
+    const int lo4 = max(w4a.x, p.hull4B.x);
+    const int w4 = max(0, min(w4a.x + w4a.y, p.hull4B.y) - lo4);
+    const int W4r = (w4 + 3) & ~3;
+    double* Qs = smem;                               // [VG][W4p][LDQ]
+    double* S3s = smem + VG * W4p * LDQ;             // [VG][W3p][LDS3]
+    for (int z = tid; z < VG * W4p * LDQ; z += FZ_QP_THREADS) Qs[z] = 0.0;   // k-padding rows must be exact zeros
+    const int MT3 = (w3.y + 7) >> 3, NT = (n54 + 7) >> 3, NT4 = (n4 + 7) >> 3, KS45 = (c45 + 3) >> 2;
+    const long sZ = (long)P4 * V * n5;
+    const double* Zb = p.Z + ((((long)b25 * n1 + a1) * c35 + b35) * c45) * sZ;
+    const double* S3b = p.S3T + ((((long)b24 * c34 + b34) * c35 + b35) * NX + xg0) * (long)(P3 * P4);
+    const long c2434 = (long)c24 * c34;
+    const double* B4b = p.Bw4T + ((long)b24 * c34 + b34) * n4;
+    const long prow = (long)c34 * c35 * NP;          // stride of v in P
+    double* Pb = p.Pq + ((((long)ac * c24 + b24) * c25 + b25) * P3) * V * prow + ((long)b34 * c35 + b35) * NP;
+
+    for (int v0 = 0; v0 < nxs; v0 += VG) {
+        const int nv = min(VG, nxs - v0), rows = nv * n5, MT = (rows + 7) >> 3;
+        __syncthreads();                             // the previous P phase has read Qs and S3s
+        for (int e = tid; e < nv * W3p * W4p; e += FZ_QP_THREADS) {
+            const int r4 = e % W4p, r = e / W4p, r3 = r % W3p, vv = r / W3p;
+            double val = 0.0;
+            if (r3 < w3.y && r4 < w4) val = __ldg(S3b + ((long)(v0 + vv) * P3 + w3.x + r3) * P4 + lo4 + r4);
+            S3s[(vv * W3p + r3) * LDS3 + r4] = val;
+        }
+        // ---- Q phase ----
+        for (int r4 = warp; r4 < w4; r4 += FZ_QP_THREADS / 32) {
+            const int q4 = lo4 + r4;
+            const double* zq = Zb + ((long)q4 * V + v0) * n5;
+            for (int nt = 0; nt < NT4; ++nt) {
+                const int i4 = nt * 8 + g;
+                double bf[8];
+#pragma unroll
+                for (int ks = 0; ks < 8; ++ks) {
+                    const int b45 = 4 * ks + q;
+                    bf[ks] = (ks < KS45 && b45 < c45 && i4 < n4) ? __ldg(B4b + ((long)q4 * c45 + b45) * c2434 * n4 + i4) : 0.0;
+                }
+                for (int mt = 0; mt < MT; ++mt) {
+                    const int m = mt * 8 + g;
+                    double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks) {
+                        if (ks < KS45) {
+                            const int b45 = 4 * ks + q;
+                            const double a = (m < rows && b45 < c45) ? __ldg(zq + b45 * sZ + m) : 0.0;
+                            fz_dmma(c0, c1, a, bf[ks]);
+                        }
+                    }
+                    if (m < rows) {
+                        const int vv = m / n5, i5 = m - vv * n5, j4 = nt * 8 + 2 * q;
+                        double* dst = Qs + (vv * W4p + r4) * LDQ + i5 * n4 + j4;
+                        if (j4 < n4) dst[0] = c0;
+                        if (j4 + 1 < n4) dst[1] = c1;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        // ---- P phase ----
+        for (int task = warp; task < nv * MT3 * NT; task += FZ_QP_THREADS / 32) {
+            const int nt = task % NT, t2 = task / NT, mt3 = t2 % MT3, vv = t2 / MT3;
+            const double* ap = S3s + (vv * W3p + mt3 * 8 + g) * LDS3 + q;
+            const double* bp = Qs + (vv * W4p + q) * LDQ + nt * 8 + g;
+            double c0 = 0.0, c1 = 0.0;
+            for (int ks = 0; ks < W4r; ks += 4) fz_dmma(c0, c1, ap[ks], bp[ks * LDQ]);
+            const int r3 = mt3 * 8 + g, n = nt * 8 + 2 * q;
+            if (r3 < w3.y && n < n54) {
+                double* dst = Pb + ((long)(w3.x + r3) * V + v0 + vv) * prow + n;
+                *reinterpret_cast<double2*>(dst) = make_double2(c0, c1);   // NP is even: n + 1 < NP, rows 16-byte aligned
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// k_fz_gemm: gather-GEMM  C[offCm[m] + offCn[n]] = sum_kk A[offAk[kk] + offAm[m]] B[offBk[kk] + offBn[n]]
+// ---------------------------------------------------------------------------------------------------------
+struct FzGemmHdr {
+    int M, N, K;
+    long baseA, baseB, baseC;
+};
+
+__device__ __forceinline__ unsigned fz_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void fz_cp_async8(unsigned dst, const void* src, int bytes)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void fz_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void fz_cp_wait()
+{
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+// ordered compaction by warp 0: kk-th accepted candidate gets (fa(cand), fb(cand)); returns the count in *K
+template <class Pred, class FA, class FB>
+__device__ __forceinline__ void fz_compact(int ncand, Pred pred, FA fa, FB fb, int* offAk, int* offBk, int* K)
+{
+    if (threadIdx.x >= 32) return;
+    const int lane = threadIdx.x;
+    int cnt = 0;
+    for (int base = 0; base < ncand; base += 32) {
+        const int c = base + lane;
+        const bool ok = c < ncand && pred(c);
+        const unsigned mask = __ballot_sync(0xffffffffu, ok);
+        if (ok) {
+            const int pos = cnt + __popc(mask & ((1u << lane) - 1u));
+            offAk[pos] = fa(c);
+            offBk[pos] = fb(c);
+        }
+        cnt += __popc(mask);
+    }
+    if (lane == 0) *K = cnt;
+}
+
+// R[l24 l25 i1; k3 x; l23 i3; (i5 i4)] = sum over the pairs (l34 l35) that allow k3 of Bw3T[k3][(l34 l35)][(l23 i3)] P[..][(l34 l35)][(i5 i4)]
+// rows m = (l23 i3) over the l23 whose pair (j13 l23) allows k3
+struct FzMapR {
+    static __device__ const double* srcA(const FzParams& p) { return p.Bw3T; }
+    static __device__ const double* srcB(const FzParams& p) { return p.Pq; }
+    static __device__ double* dstC(const FzParams& p) { return p.Rq; }
+    static __host__ __device__ long items(const FzParams& p, int BM, int BN)
+    {
+        const long ntn = (p.P.n_i[3] * p.P.n_i[4] + BN - 1) / BN, ntm = (p.box.cnt[0] * p.P.n_i[2] + BM - 1) / BM;
+        return ntn * ntm * p.V * p.P.n_k_pad[1] * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
+    }
+    static __device__ void setup(const FzParams& p, long item, int BM, int BN, FzGemmHdr* h, int* offAm, int* offCm,
+                                 int* offBn, int* offCn, int* offAk, int* offBk)
+    {
+        const SfProblem& P = p.P;
+        const int nl = P.nl, n3 = P.n_i[2], n54 = P.n_i[3] * P.n_i[4], P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
+        const int c23 = p.box.cnt[0], c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
+        const int ntn = (n54 + BN - 1) / BN, ntm = (c23 * n3 + BM - 1) / BM;
+        const int nt = (int)(item % ntn); item /= ntn;
+        const int mt = (int)(item % ntm); item /= ntm;
+        const int v = (int)(item % V); item /= V;
+        const int q3 = (int)(item % P3); item /= P3;
+        const int b25 = (int)(item % c25); item /= c25;
+        const int b24 = (int)(item % c24);
+        const int ac = (int)(item / c24);
+        int x0, nxs, xg0;
+        fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, p.a_lo + ac, p.box.lo[2] + b25, x0, nxs, xg0);
+        int blo = -1, bcnt = 0;
+        for (int b = 0; b < c23; ++b) {
+            const int2 w = p.w3B[p.box.lo[0] + b];
+            if (q3 >= w.x && q3 < w.x + w.y) {
+                if (blo < 0) blo = b;
+                ++bcnt;
+            }
+        }
+        const int m0 = mt * BM, M = v < nxs ? min(BM, bcnt * n3 - m0) : 0, N = min(BN, n54 - nt * BN);
+        if (threadIdx.x == 0) {
+            h->M = M;
+            h->N = N;
+            h->K = 0;
+            const long slab = ((((long)ac * c24 + b24) * c25 + b25) * P3 + q3) * V + v;
+            h->baseA = (long)q3 * c34 * c35 * c23 * n3 + (long)blo * n3 + m0;
+            h->baseB = slab * c34 * c35 * NP + (long)nt * BN;
+            h->baseC = ((slab * c23 + blo) * n3 + m0) * NP + (long)nt * BN;
+        }
+        if (M <= 0) return;
+        for (int m = threadIdx.x; m < BM; m += blockDim.x) {
+            offAm[m] = m;
+            offCm[m] = m * NP;
+        }
+        for (int n = threadIdx.x; n < BN; n += blockDim.x) offBn[n] = offCn[n] = n;
+        const int lo34 = p.box.lo[3], lo35 = p.box.lo[4];
+        fz_compact(
+            c34 * c35,
+            [&](int c) {
+                const int2 w = p.w3A[(lo34 + c / c35) * nl + lo35 + c % c35];
+                return q3 >= w.x && q3 < w.x + w.y;
+            },
+            [&](int c) { return c * c23 * n3; }, [&](int c) { return c * NP; }, offAk, offBk, &h->K);
+    }
+};
+
+// A'[l24 l25; i1; i2; (i3 i4 i5)] = sum over (k3, x, l23) with k3 allowed by (j13 l23) of G[..][(k3 x l23)][i2] R[..][(k3 x l23)][(i3, i5 i4)]
+struct FzMapA {
+    static __device__ const double* srcA(const FzParams& p) { return p.G; }
+    static __device__ const double* srcB(const FzParams& p) { return p.Rq; }
+    static __device__ double* dstC(const FzParams& p) { return p.Apart; }
+    static __host__ __device__ long items(const FzParams& p, int BM, int BN)
+    {
+        const long ntn = ((long)p.P.n_i[2] * p.P.n_i[3] * p.P.n_i[4] + BN - 1) / BN, ntm = (p.P.n_i[1] + BM - 1) / BM;
+        return ntn * ntm * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
+    }
+    static __device__ void setup(const FzParams& p, long item, int BM, int BN, FzGemmHdr* h, int* offAm, int* offCm,
+                                 int* offBn, int* offCn, int* offAk, int* offBk)
+    {
+        const SfProblem& P = p.P;
+        const int n1 = P.n_i[0], n2 = P.n_i[1], n3 = P.n_i[2], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5, n345 = n3 * n54;
+        const int P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
+        const int c23 = p.box.cnt[0], c24 = p.box.cnt[1], c25 = p.box.cnt[2];
+        const int ntn = (n345 + BN - 1) / BN, ntm = (n2 + BM - 1) / BM;
+        const int nt = (int)(item % ntn); item /= ntn;
+        const int mt = (int)(item % ntm); item /= ntm;
+        const int b25 = (int)(item % c25); item /= c25;
+        const int b24 = (int)(item % c24);
+        const int ac = (int)(item / c24);
+        const int a1 = p.a_lo + ac;
+        int x0, nxs, xg0;
+        fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, p.box.lo[2] + b25, x0, nxs, xg0);
+        const int m0 = mt * BM, n0 = nt * BN, M = min(BM, n2 - m0), N = min(BN, n345 - n0);
+        if (threadIdx.x == 0) {
+            h->M = M;
+            h->N = N;
+            h->K = 0;
+            h->baseA = ((((long)b24 * c25 + b25) * n1 + a1) * P3 * V * c23) * n2;
+            h->baseB = (((long)ac * c24 + b24) * c25 + b25) * ((long)P3 * V * c23 * n3 * NP);
+            h->baseC = ((p.part0 + (long)b24 * c25 + b25) * n1 + a1) * ((long)n2 * n345);
+        }
+        for (int m = threadIdx.x; m < BM; m += blockDim.x) {
+            offAm[m] = m0 + m;
+            offCm[m] = (m0 + m) * n345;
+        }
+        for (int n = threadIdx.x; n < BN; n += blockDim.x) {
+            const int ng = n0 + n, i3 = ng / n54, r = ng - i3 * n54, i5 = r / n4, i4 = r - i5 * n4;
+            offBn[n] = i3 * NP + r;
+            offCn[n] = (i3 * n4 + i4) * n5 + i5;
+        }
+        const int lo23 = p.box.lo[0];
+        fz_compact(
+            P3 * nxs * c23,
+            [&](int c) {
+                const int2 w = p.w3B[lo23 + c % c23];
+                const int q3 = c / (nxs * c23);
+                return q3 >= w.x && q3 < w.x + w.y;
+            },
+            [&](int c) {
+                const int b23 = c % c23, r = c / c23, v = r % nxs, q3 = r / nxs;
+                return ((q3 * V + v) * c23 + b23) * n2;
+            },
+            [&](int c) {
+                const int b23 = c % c23, r = c / c23, v = r % nxs, q3 = r / nxs;
+                return ((q3 * V + v) * c23 + b23) * n3 * NP;
+            },
+            offAk, offBk, &h->K);
+    }
+};
+
+#define FZ_KC 16
+#define FZ_STAGES 3
+template <class Map, int WGM, int WGN, int TM, int TN>
+__global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int kcap)
+{
+    constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8, NTH = WGM * WGN * 32, LDA = BM + 8, LDB = BN + 8;
+    extern __shared__ __align__(16) double smem[];
+    __shared__ FzGemmHdr hdr;
+    double* As = smem;                               // [FZ_STAGES][FZ_KC][LDA], [k][m]
+    double* Bs = As + FZ_STAGES * FZ_KC * LDA;       // [FZ_STAGES][FZ_KC][LDB], [k][n]
+    int* offAm = (int*)(Bs + FZ_STAGES * FZ_KC * LDB);
+    int* offCm = offAm + BM;
+    int* offBn = offCm + BM;
+    int* offCn = offBn + BN;
+    int* offAk = offCn + BN;
+    int* offBk = offAk + kcap;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
+    const int wm = warp / WGN, wn = warp % WGN;
+    Map::setup(p, blockIdx.x, BM, BN, &hdr, offAm, offCm, offBn, offCn, offAk, offBk);
+    __syncthreads();
+    const int M = hdr.M, N = hdr.N, K = hdr.K;
+    if (M <= 0) return;
+    const double* A0 = Map::srcA(p);
+    const double* B0 = Map::srcB(p);
+    const double* A = A0 + hdr.baseA;
+    const double* B = B0 + hdr.baseB;
+    double* C = Map::dstC(p) + hdr.baseC;
+    const int nchunks = (K + FZ_KC - 1) / FZ_KC;
+    auto load_chunk = [&](int c) {
+        if (c < nchunks) {
+            const int s = c % FZ_STAGES, k0 = c * FZ_KC;
+            for (int e = tid; e < FZ_KC * BM; e += NTH) {
+                const int kr = e / BM, m = e % BM, k = k0 + kr;
+                const bool ok = m < M && k < K;
+                fz_cp_async8(fz_smem_u32(As + (s * FZ_KC + kr) * LDA + m), ok ? A + offAk[k] + offAm[m] : A0, ok ? 8 : 0);
+            }
+            for (int e = tid; e < FZ_KC * BN; e += NTH) {
+                const int kr = e / BN, n = e % BN, k = k0 + kr;
+                const bool ok = n < N && k < K;
+                fz_cp_async8(fz_smem_u32(Bs + (s * FZ_KC + kr) * LDB + n), ok ? B + offBk[k] + offBn[n] : B0, ok ? 8 : 0);
+            }
+        }
+        fz_cp_commit();
+    };
+    double acc[TM][TN][2];
+#pragma unroll
+    for (int i = 0; i < TM; ++i)
+#pragma unroll
+        for (int j = 0; j < TN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    const bool active = wm * TM * 8 < M && wn * TN * 8 < N;
+#pragma unroll
+    for (int c = 0; c < FZ_STAGES - 1; ++c) load_chunk(c);
+    for (int c = 0; c < nchunks; ++c) {
+        fz_cp_wait<FZ_STAGES - 2>();
+        __syncthreads();                             // chunk c has landed; every warp is done with chunk c - 1
+        load_chunk(c + FZ_STAGES - 1);               // refills the stage chunk c - 1 used
+        if (active) {
+            const double* as = As + (c % FZ_STAGES) * FZ_KC * LDA + q * LDA + wm * TM * 8 + g;
+            const double* bs = Bs + (c % FZ_STAGES) * FZ_KC * LDB + q * LDB + wn * TN * 8 + g;
+#pragma unroll
+            for (int ks = 0; ks < FZ_KC / 4; ++ks) {
+                double a[TM], b[TN];
+#pragma unroll
+                for (int i = 0; i < TM; ++i) a[i] = as[ks * 4 * LDA + 8 * i];
+#pragma unroll
+                for (int j = 0; j < TN; ++j) b[j] = bs[ks * 4 * LDB + 8 * j];
+#pragma unroll
+                for (int i = 0; i < TM; ++i)
+#pragma unroll
+                    for (int j = 0; j < TN; ++j) fz_dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+            }
+        }
+    }
+    fz_cp_wait<0>();
+    if (!active) return;
+#pragma unroll
+    for (int i = 0; i < TM; ++i) {
+        const int m = wm * TM * 8 + 8 * i + g;
+        if (m >= M) continue;
+        double* cm = C + offCm[m];
+#pragma unroll
+        for (int j = 0; j < TN; ++j) {
+            const int n = wn * TN * 8 + 8 * j + 2 * q;
+            if (n < N) cm[offCn[n]] = acc[i][j][0];
+            if (n + 1 < N) cm[offCn[n + 1]] = acc[i][j][1];
+        }
+    }
+}
+
+// kernel (d): out[a1][i2][r] = prod_e sqrt(2 i_e + 1) * sum over the partial tensors, in order, of Apart[part][a1][i2][r]
+// (step 6(iv) + the normalisation of eq. (3))
+__global__ void __launch_bounds__(256) k_fz_reduce(SfProblem P, long n_parts, long n_out, const double* __restrict__ partial,
+                                                   double* __restrict__ out)
+{
+    const long z = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (z >= n_out) return;
+    double s = 0.0;
+    for (long b = 0; b < n_parts; ++b) s += partial[b * n_out + z];
+    long r = z;
+    double d = 1.0;
+    for (int n = 4; n >= 0; --n) {
+        d *= (double)(P.two_i_min[n] + 2 * (int)(r % P.n_i[n]) + 1);
+        r /= P.n_i[n];
+    }
+    out[z] = s * sqrt(d);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------
+// [lo, hi) of the canonical shell order (o45 fastest, eq. (9)) as a disjoint union of boxes, in order
+static void fz_boxes(int nl, long lo, long hi, int digit, FzBox prefix, FzBox* out, int* n)
+{
+    if (lo >= hi) return;
+    long w = 1;
+    for (int d = digit + 1; d < 6; ++d) w *= nl;      // shells per value of this digit
+    if (lo == 0 && hi == w * nl) {
+        for (int d = digit; d < 6; ++d) {
+            prefix.lo[d] = 0;
+            prefix.cnt[d] = nl;
+        }
+        out[(*n)++] = prefix;
+        return;
+    }
+    const int a = (int)(lo / w), b = (int)((hi - 1) / w);
+    if (digit == 5) {
+        prefix.lo[5] = a;
+        prefix.cnt[5] = b - a + 1;
+        out[(*n)++] = prefix;
+        return;
+    }
+    if (a == b) {
+        prefix.lo[digit] = a;
+        prefix.cnt[digit] = 1;
+        fz_boxes(nl, lo - a * w, hi - a * w, digit + 1, prefix, out, n);
+        return;
+    }
+    int first_full = a, last_full = b;               // digits whose whole sub-range is inside [lo, hi)
+    if (lo != a * w) {
+        prefix.lo[digit] = a;
+        prefix.cnt[digit] = 1;
+        fz_boxes(nl, lo - a * w, w, digit + 1, prefix, out, n);
+        first_full = a + 1;
+    }
+    if (hi != (b + 1) * w) last_full = b - 1;
+    if (last_full >= first_full) {
+        FzBox m = prefix;
+        m.lo[digit] = first_full;
+        m.cnt[digit] = last_full - first_full + 1;
+        for (int d = digit + 1; d < 6; ++d) {
+            m.lo[d] = 0;
+            m.cnt[d] = nl;
+        }
+        out[(*n)++] = m;
+    }
+    if (hi != (b + 1) * w) {
+        prefix.lo[digit] = b;
+        prefix.cnt[digit] = 1;
+        fz_boxes(nl, 0, hi - b * w, digit + 1, prefix, out, n);
+    }
+}
+
+struct FzShape {
+    bool ok;
+    int V, NP, W3p, W4p, LDQ, LDS3, VG;
+    size_t qp_smem;
+};
+
+static FzShape fz_shape(const SfDims& D)
+{
+    FzShape s;
+    memset(&s, 0, sizeof s);
+    for (int e = 0; e < 4; ++e)
+        if (D.k_max[e] == 0) return s;
+    if (D.nl > 32) return s;
+    for (int a = 0; a < D.n_i[0]; ++a)
+        for (int o = 0; o < D.nl; ++o) {
+            int x0, nxs, xg0;
+            fz_xrange(D.two_i_min[0], D.two_j[J25], D.two_x_base, a, o, x0, nxs, xg0);
+            if (nxs > s.V) s.V = nxs;
+        }
+    const int n54 = D.n_i[3] * D.n_i[4];
+    s.NP = (n54 + 1) & ~1;
+    int w3 = 0, w4 = 0;
+    for (int u = 0; u < D.nl; ++u)
+        for (int v = 0; v < D.nl; ++v) {
+            const int2 a = fz_window(D.two_j[J34] + 2 * u, D.two_j[J35] + 2 * v, D.two_k_base[1], D.n_k_pad[1]);
+            const int2 b = fz_window(D.two_j[J24] + 2 * u, D.two_j[J34] + 2 * v, D.two_k_base[2], D.n_k_pad[2]);
+            if (a.y > w3) w3 = a.y;
+            if (b.y > w4) w4 = b.y;
+        }
+    s.W3p = (w3 + 7) & ~7;
+    s.W4p = (w4 + 3) & ~3;
+    if (s.W3p == 0 || s.W4p == 0) return s;
+    s.LDQ = ((n54 + 15) & ~15) + 8;                   // = 8 mod 16: conflict-free B fragments
+    s.LDS3 = (s.W4p % 8 == 0) ? s.W4p + 4 : s.W4p;    // = 4 mod 8: conflict-free A fragments
+    // x values per pass: fill the 8-row tiles of (v, i5) as well as possible inside ~100 KB (two CTAs per SM)
+    int best = 0;
+    double best_fill = 0.0;
+    for (int vg = 1; vg <= s.V; ++vg) {
+        const size_t bytes = sizeof(double) * ((size_t)vg * s.W4p * s.LDQ + (size_t)vg * s.W3p * s.LDS3);
+        if (bytes > 100 * 1024) break;
+        const int rows = vg * D.n_i[4];
+        const double fill = (double)rows / (((rows + 7) / 8) * 8);
+        if (fill > best_fill + 1e-9) {
+            best_fill = fill;
+            best = vg;
+        }
+    }
+    if (best == 0) return s;
+    s.VG = best;
+    s.qp_smem = sizeof(double) * ((size_t)s.VG * s.W4p * s.LDQ + (size_t)s.VG * s.W3p * s.LDS3);
+    // int offsets inside one gather-GEMM item
+    const double slab = (double)D.n_k_pad[1] * s.V * D.nl * D.n_i[2] * s.NP;
+    if (slab > 2.0e9 || (double)D.n_out / D.n_i[0] > 2.0e9) return s;
+    s.ok = true;
+    return s;
+}
+
+bool sf_vertex_factor_supported(const SfDims& D) { return fz_shape(D).ok; }
+
+template <class Map, int WGM, int WGN, int TM, int TN>
+static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
+{
+    constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8;
+    const size_t smem = sizeof(double) * FZ_STAGES * FZ_KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 2 * (size_t)kcap);
+    if (smem > 226 * 1024) return SF_EARG;
+    static size_t attr = 0;
+    if (smem > attr) {
+        if (cudaFuncSetAttribute(k_fz_gemm<Map, WGM, WGN, TM, TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return SF_ECUDA;
+        attr = smem;
+    }
+    const long items = Map::items(p, BM, BN);
+    if (items <= 0) return SF_OK;
+    if (items > 2147483647L) return SF_EARG;
+    k_fz_gemm<Map, WGM, WGN, TM, TN><<<(unsigned)items, WGM * WGN * 32, smem, st>>>(p, kcap);
+    sf_count_launch(1);
+    return SF_OK;
+}
+
+enum { FZ_SLOT_WIN = 24, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART };
+
+int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st)
+{
+    const FzShape sh = fz_shape(D);
+    if (!sh.ok) return SF_EARG;
+    const int nl = D.nl, n1 = D.n_i[0], n2 = D.n_i[1], n3 = D.n_i[2], n4 = D.n_i[3], n5 = D.n_i[4];
+    const int P3 = D.n_k_pad[1], P4 = D.n_k_pad[2];
+    const long slice = D.n_out / n1;
+
+    FzBox boxes[16];
+    int nbox = 0;
+    FzBox none;
+    memset(&none, 0, sizeof none);
+    fz_boxes(nl, shell_lo, shell_hi, 0, none, boxes, &nbox);
+    long parts = 0;
+    for (int b = 0; b < nbox; ++b) parts += (long)boxes[b].cnt[1] * boxes[b].cnt[2];
+
+    FzParams p;
+    memset(&p, 0, sizeof p);
+    p.P = P;
+    p.V = sh.V;
+    p.NP = sh.NP;
+    p.W3p = sh.W3p;
+    p.W4p = sh.W4p;
+    p.LDQ = sh.LDQ;
+    p.LDS3 = sh.LDS3;
+    p.VG = sh.VG;
+    for (int s = 0; s < 10; ++s) p.jsum += D.two_j[s];
+
+    int2* win = (int2*)sf_scratch(FZ_SLOT_WIN, sizeof(int2) * (2 * (size_t)nl * nl + 2 * nl));
+    double* Apart = (double*)sf_scratch(FZ_SLOT_PART, sizeof(double) * (size_t)(parts > 0 ? parts : 1) * D.n_out);
+    if (!win || !Apart) return SF_ENOMEM;
+    int2 *w3A = win, *w4A = win + nl * nl, *w3B = win + 2 * nl * nl, *w4B = w3B + nl;
+    p.w3A = w3A;
+    p.w3B = w3B;
+    p.w4A = w4A;
+    p.w4B = w4B;
+    p.Apart = Apart;
+    if (nbox > 0) {
+        k_fz_windows<<<(nl * nl + 127) / 128, 128, 0, st>>>(P, w3A, w3B, w4A, w4B);
+        sf_count_launch(1);
+    }
+    static bool qp_attr = false;
+    if (!qp_attr) {
+        if (cudaFuncSetAttribute(k_fz_qp, cudaFuncAttributeMaxDynamicSharedMemorySize, 101 * 1024) != cudaSuccess) return SF_ECUDA;
+        qp_attr = true;
+    }
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return SF_ECUDA;
+
+    long part0 = 0;
+    for (int bi = 0; bi < nbox; ++bi) {
+        const FzBox& bx = boxes[bi];
+        p.box = bx;
+        p.part0 = part0;
+        const long c23 = bx.cnt[0], c24 = bx.cnt[1], c25 = bx.cnt[2], c34 = bx.cnt[3], c35 = bx.cnt[4], c45 = bx.cnt[5];
+        int lo = 1 << 30, hi = 0;
+        for (int o = bx.lo[5]; o < bx.lo[5] + bx.cnt[5]; ++o) {
+            const int2 w = fz_window(D.two_j[J45] + 2 * o, D.two_j[J14], D.two_k_base[2], P4);
+            if (w.y > 0) {
+                if (w.x < lo) lo = w.x;
+                if (w.x + w.y > hi) hi = w.x + w.y;
+            }
+        }
+        p.hull4B = make_int2(lo < hi ? lo : 0, lo < hi ? hi : 0);
+
+        const long nZ = c25 * n1 * c35 * c45 * ((long)P4 * sh.V * n5);
+        const long nB4 = (long)P4 * c45 * c24 * c34 * n4, nB3 = (long)P3 * c34 * c35 * c23 * n3;
+        const long nS3 = c24 * c34 * c35 * D.n_x_pad * P3 * P4;
+        const long nG = c24 * c25 * n1 * P3 * sh.V * c23 * n2;
+        const long pP = c24 * c25 * P3 * sh.V * c34 * c35 * sh.NP;     // per i1
+        const long pR = c24 * c25 * P3 * sh.V * c23 * n3 * sh.NP;
+        // i1 values per pass: P and R of a pass inside ~1/3 of the device memory
+        const double budget = (double)total_b / 3.0;
+        long na = (long)(budget / (8.0 * (double)(pP + pR)));
+        if (na < 1) return SF_ENOMEM;
+        if (na > n1) na = n1;
+        double* Z = (double*)sf_scratch(FZ_SLOT_Z, sizeof(double) * (size_t)nZ);
+        double* B4 = (double*)sf_scratch(FZ_SLOT_B4, sizeof(double) * (size_t)nB4);
+        double* B3 = (double*)sf_scratch(FZ_SLOT_B3, sizeof(double) * (size_t)nB3);
+        double* S3 = (double*)sf_scratch(FZ_SLOT_S3, sizeof(double) * (size_t)nS3);
+        double* G = (double*)sf_scratch(FZ_SLOT_G, sizeof(double) * (size_t)nG);
+        double* Pq = (double*)sf_scratch(FZ_SLOT_P, sizeof(double) * (size_t)(pP * na));
+        double* Rq = (double*)sf_scratch(FZ_SLOT_R, sizeof(double) * (size_t)(pR * na));
+        if (!Z || !B4 || !B3 || !S3 || !G || !Pq || !Rq) return SF_ENOMEM;
+        p.Z = Z;
+        p.Bw4T = B4;
+        p.Bw3T = B3;
+        p.S3T = S3;
+        p.G = G;
+        p.Pq = Pq;
+        p.Rq = Rq;
+        p.a_lo = 0;
+        p.a_cnt = n1;
+        k_fz_z<<<(unsigned)(c25 * n1 * c35 * c45), 256, 0, st>>>(p, Z);
+        k_fz_b4t<<<(unsigned)((nB4 + 255) / 256), 256, 0, st>>>(p, nB4, B4);
+        k_fz_b3t<<<(unsigned)((nB3 + 255) / 256), 256, 0, st>>>(p, nB3, B3);
+        k_fz_s3t<<<(unsigned)((nS3 + 255) / 256), 256, 0, st>>>(p, nS3, S3);
+        k_fz_g<<<(unsigned)((nG + 255) / 256), 256, 0, st>>>(p, nG, G);
+        sf_count_launch(5);
+        for (int a_lo = 0; a_lo < n1; a_lo += (int)na) {
+            p.a_lo = a_lo;
+            p.a_cnt = (int)(a_lo + na <= n1 ? na : n1 - a_lo);
+            k_fz_qp<<<(unsigned)((long)p.a_cnt * c25 * c35 * c24 * c34), FZ_QP_THREADS, sh.qp_smem, st>>>(p);
+            sf_count_launch(1);
+            int rc = fz_launch_gemm<FzMapR, 4, 2, 4, 4>(p, (int)(c34 * c35), st);
+            if (rc != SF_OK) return rc;
+            rc = fz_launch_gemm<FzMapA, 1, 8, 2, 4>(p, (int)(P3 * sh.V * c23), st);
+            if (rc != SF_OK) return rc;
+        }
+        part0 += c24 * c25;
+    }
+    sf_timing_mark(2, st);
+    k_fz_reduce<<<(unsigned)((D.n_out + 255) / 256), 256, 0, st>>>(P, parts, D.n_out, Apart, out);
+    sf_count_launch(1);
+    return cudaGetLastError() == cudaSuccess ? SF_OK : SF_ECUDA;
+}

@@ -1,6 +1,7 @@
 """GPU parity of the vertex tensor (steps 4-7 of the algorithm) against the oracle, through the
 C ABI, on the five workloads of BASELINE.json (small ones in full, large ones on shell sub-ranges the oracle finishes
-in seconds), for both the staged and the fused path, plus edge cases, additivity, determinism and error behaviour.
+in seconds), for the staged, the per-shell line and the factorised path (the automatic choice), plus edge cases,
+additivity, determinism and error behaviour.
 """
 import itertools
 import random
@@ -17,7 +18,8 @@ from gpu_common import TOL, abi_dims, assert_parity, boosters_for, run_gpu, run_
 
 pytestmark = pytest.mark.gpu
 
-PATHS = [pytest.param(1, id="staged"), pytest.param(0, id="auto")]
+PATHS = [pytest.param(1, id="staged"), pytest.param(3, id="line"), pytest.param(0, id="auto")]
+TAKEN = {1: 1, 3: 3, 0: 4}      # automatic selection takes the factorised path wherever it fits
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -45,7 +47,7 @@ def _full(cfg, what):
 def test_config0_full(path):
     worst, Ag, Ao = _full(wl.CONFIGS[0], "config 0")
     assert Ag.shape == (3,) * 5 and np.abs(Ao).max() > 0
-    assert sf.sf_last_path() == (1 if path == 1 else 3)      # automatic selection takes the on-chip line path here
+    assert sf.sf_last_path() == TAKEN[path]
 
 
 @pytest.mark.parametrize("two_j", [1, 2, 3, 4, 6, 9, 12])
@@ -96,7 +98,39 @@ def test_config3_scattered_shells(path):
     Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, lo + 9, Bdev=Bdev)
     Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, lo + 9)
     assert_parity(Ag, Ao, Aabs, what="config 3 short range")
-    assert sf.sf_last_path() == (1 if path == 1 else 3)
+    assert sf.sf_last_path() == TAKEN[path]
+
+
+def test_config3_blocks_and_ragged_ranges():
+    """The headline workload at its bench launch configuration (automatic path = factorised), on ranges that are whole
+    boxes of virtual spins (all (l34 l35 l45) of one (l23 l24 l25): 1331 shells) and on ragged ranges that the
+    library splits into up to 11 boxes."""
+    cfg = wl.CONFIGS[3]
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    nl3 = 11 ** 3
+    for lo, hi in [(nl3 * 700, nl3 * 701), (nl3 * 1330, nl3 * 1331), (nl3 * 5 + 777, nl3 * 6 + 1500),
+                   (11 ** 5 * 4 - 40, 11 ** 5 * 4 + 2000)]:
+        Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+        assert sf.sf_last_path() == 4
+        Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, hi)
+        assert_parity(Ag, Ao, Aabs, what=f"config 3 shells [{lo},{hi})")
+
+
+def test_paths_agree_on_a_full_tensor():
+    """Config 2, Delta_l = 4 (15 625 shells) in full: the factorised and the per-shell line path give the same tensor to
+    rounding, and both match the oracle."""
+    cfg = wl.config2(4)
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    sf.sf_set_path(4)
+    A4 = run_gpu(cfg["two_j"], cfg["two_dl"], B, Bdev=Bdev)
+    sf.sf_set_path(3)
+    A3 = run_gpu(cfg["two_j"], cfg["two_dl"], B, Bdev=Bdev)
+    sf.sf_set_path(0)
+    Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B)
+    assert_parity(A4, Ao, Aabs, what="config 2 dl=4, factorised")
+    assert_parity(A3, Ao, Aabs, what="config 2 dl=4, line")
 
 
 def _config4(lam):
@@ -107,6 +141,8 @@ def _config4(lam):
 
 @pytest.mark.parametrize("lam,n", [(1, 60), (2, 6), (3, 1)])
 def test_config4_sub_ranges(path, lam, n):
+    if path == 3 and lam > 1:
+        pytest.skip("the line path holds intertwiner ranges of at most 16 values")
     cfg = _config4(lam)
     B = boosters_for(cfg)
     lo = 7 ** 6 // 2 + 11
