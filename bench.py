@@ -31,6 +31,7 @@ if ROOT not in sys.path:
 import workloads as wl  # noqa: E402
 
 METRIC = "eprl_shells_contracted_per_s"
+PATH_NAMES = {1: "staged", 2: "fused", 3: "line", 4: "factorised"}
 UNIT = "shells/s"
 
 
@@ -182,6 +183,7 @@ def run_ours(args, cfg, rank, world, local_rank):
     n_shells = nl ** 6
 
     sf.sf_init(wl.GAMMA)
+    sf.sf_set_path(args.path)
     # one-off {6j} table (kernel (a)), outside the timed region, timed on its own
     t0 = time.perf_counter()
     sf.sf_sixj_table(args.table)
@@ -276,13 +278,13 @@ def run_ours(args, cfg, rank, world, local_rank):
                    "nonempty_shells": work["n_nonempty"], "out_shape": n_i, "boosters": "seeded N(0,1)*(1+u+v+w)^-1.5",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "256 MiB device memset between steps (inside the timed region)",
-                   "sixj_table_two_jmax": args.table, "path": {1: "staged", 2: "fused", 3: "line"}.get(last_path, "?")},
+                   "sixj_table_two_jmax": args.table, "path": PATH_NAMES.get(last_path, "?")},
         "vertex_tensors_per_s": world * args.steps / (ms * 1e-3),
         "clocks": clocks,
         "e2e": {"value": whole_job_value(n_shells, args.steps, world, e2e_s), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s / args.steps},
         "gpu_launches": launches,
-        "roofline": {"bound": "alu", "kernel": {2: "k_vertex_fused", 3: "k_vertex_line"}.get(last_path, "k_stage_*"),
+        "roofline": {"bound": "alu", "kernel": {2: "k_vertex_fused", 3: "k_vertex_line", 4: "k_fz_gemm<FzMapR>"}.get(last_path, "k_stage_*"),
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
                      "peak_source": "measured in this process: FP64 DFMA %.2f, DMMA(mma.sync m8n8k4) %.2f TFLOP/s"
                                     % (peak_dfma, peak_dmma),
@@ -321,6 +323,7 @@ def main():
     ap.add_argument("--table", type=int, default=60, help="two_jmax of the resident {6j} table (-1: none)")
     ap.add_argument("--ref-shells", type=int, default=8000, help="shells in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", type=int, default=0, help="0 automatic (fastest that fits), 1 staged, 2 fused, 3 line, 4 factorised")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

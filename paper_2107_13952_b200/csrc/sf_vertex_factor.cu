@@ -51,6 +51,8 @@ struct FzParams {
     const int2* w4A;            // [o24][o34] window of q4 allowed by the pair (l24 l34)
     const int2* w4B;            // [o45]      window of q4 allowed by the pair (l45 j14)
     int2 hull4B;                // union of w4B over the box: (lo, hi exclusive)
+    const int2* win23;          // [q3] (first b23, count) of the box's l23 whose pair (j13 l23) allows k3
+    const int* kl3;             // [q3][1 + c34 c35]: count, then the box's pairs (b34 c35 + b35) whose (l34 l35) allow k3, ascending
     const double* Z;            // [b25][a1][b35][b45][q4][v][i5]
     const double* Bw4T;         // [q4][b45][b24][b34][i4]
     const double* Bw3T;         // [q3][b34][b35][b23][i3]
@@ -257,12 +259,47 @@ __global__ void __launch_bounds__(256) k_fz_g(FzParams p, long n, double* __rest
     out[e] = val;
 }
 
+// per k3: the l23 of the box that allow it (contiguous: |k3 - j13| <= l23 <= k3 + j13) and the (l34 l35) pairs that do
+__global__ void __launch_bounds__(32) k_fz_lists(FzParams p, int2* __restrict__ win23, int* __restrict__ kl3)
+{
+    const int q3 = blockIdx.x, lane = threadIdx.x, nl = p.P.nl;
+    const int c23 = p.box.cnt[0], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
+    if (lane == 0) {
+        int blo = -1, bcnt = 0;
+        for (int b = 0; b < c23; ++b) {
+            const int2 w = p.w3B[p.box.lo[0] + b];
+            if (q3 >= w.x && q3 < w.x + w.y) {
+                if (blo < 0) blo = b;
+                ++bcnt;
+            }
+        }
+        win23[q3] = make_int2(blo < 0 ? 0 : blo, bcnt);
+    }
+    int* list = kl3 + (long)q3 * (1 + c34 * c35);
+    int cnt = 0;
+    for (int base = 0; base < c34 * c35; base += 32) {
+        const int c = base + lane;
+        bool ok = false;
+        if (c < c34 * c35) {
+            const int2 w = p.w3A[(p.box.lo[3] + c / c35) * nl + p.box.lo[4] + c % c35];
+            ok = q3 >= w.x && q3 < w.x + w.y;
+        }
+        const unsigned mask = __ballot_sync(0xffffffffu, ok);
+        if (ok) list[1 + cnt + __popc(mask & ((1u << lane) - 1u))] = c;
+        cnt += __popc(mask);
+    }
+    if (lane == 0) list[0] = cnt;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // k_fz_qp: Q = sum_l45 Z Bw4 and P = sum_k4 S3 Q for one (i1, l25, l35, l24, l34), a few x at a time
 // ---------------------------------------------------------------------------------------------------------
 // Q phase, per k4:  C[(v i5)][i4] = sum_l45 Z[l45][k4][(v i5)] Bw4T[k4][l45][i4]        (A and B fragments straight from L1/L2)
 // P phase, per v:   P[k3][(i5 i4)] = sum_k4 S3[k3][k4] Q[k4][(i5 i4)]                   (both operands in shared memory)
 #define FZ_QP_THREADS 256
+#define FZ_QKS 3      /* fast Q phase: c45 <= 12, n4 <= 16, (v, i5) rows of a pass <= 32 */
+#define FZ_QNT 2
+#define FZ_QMT 4
 __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
 {
     extern __shared__ __align__(16) double smem[];
@@ -310,49 +347,103 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
             S3s[(vv * W3p + r3) * LDS3 + r4] = val;
         }
         // ---- Q phase ----
-        for (int r4 = warp; r4 < w4; r4 += FZ_QP_THREADS / 32) {
-            const int q4 = lo4 + r4;
-            const double* zq = Zb + ((long)q4 * V + v0) * n5;
-            for (int nt = 0; nt < NT4; ++nt) {
-                const int i4 = nt * 8 + g;
-                double bf[8];
+        if (KS45 <= FZ_QKS && NT4 <= FZ_QNT && MT <= FZ_QMT) {
+            // common sizes: every fragment of a k4 is requested before the first MMA, so one round of L2 latency per k4
+            for (int r4 = warp; r4 < w4; r4 += FZ_QP_THREADS / 32) {
+                const int q4 = lo4 + r4;
+                const double* zq = Zb + ((long)q4 * V + v0) * n5;
+                const double* bq = B4b + (long)q4 * c45 * c2434 * n4;
+                double a[FZ_QMT][FZ_QKS], b[FZ_QNT][FZ_QKS];
 #pragma unroll
-                for (int ks = 0; ks < 8; ++ks) {
+                for (int ks = 0; ks < FZ_QKS; ++ks) {
                     const int b45 = 4 * ks + q;
-                    bf[ks] = (ks < KS45 && b45 < c45 && i4 < n4) ? __ldg(B4b + ((long)q4 * c45 + b45) * c2434 * n4 + i4) : 0.0;
-                }
-                for (int mt = 0; mt < MT; ++mt) {
-                    const int m = mt * 8 + g;
-                    double c0 = 0.0, c1 = 0.0;
+                    const bool kin = ks < KS45 && b45 < c45;
 #pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) {
-                        if (ks < KS45) {
-                            const int b45 = 4 * ks + q;
-                            const double a = (m < rows && b45 < c45) ? __ldg(zq + b45 * sZ + m) : 0.0;
-                            fz_dmma(c0, c1, a, bf[ks]);
+                    for (int nt = 0; nt < FZ_QNT; ++nt) {
+                        const int i4 = nt * 8 + g;
+                        b[nt][ks] = (kin && nt < NT4 && i4 < n4) ? __ldg(bq + (long)b45 * c2434 * n4 + i4) : 0.0;
+                    }
+#pragma unroll
+                    for (int mt = 0; mt < FZ_QMT; ++mt) {
+                        const int m = mt * 8 + g;
+                        a[mt][ks] = (kin && m < rows) ? __ldg(zq + b45 * sZ + m) : 0.0;
+                    }
+                }
+#pragma unroll
+                for (int mt = 0; mt < FZ_QMT; ++mt) {
+                    if (mt >= MT) break;
+                    const int m = mt * 8 + g, vv = m / n5, i5 = m - vv * n5;
+                    double* dst = Qs + (vv * W4p + r4) * LDQ + i5 * n4 + 2 * q;
+#pragma unroll
+                    for (int nt = 0; nt < FZ_QNT; ++nt) {
+                        if (nt >= NT4) break;
+                        double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                        for (int ks = 0; ks < FZ_QKS; ++ks)
+                            if (ks < KS45) fz_dmma(c0, c1, a[mt][ks], b[nt][ks]);
+                        if (m < rows) {
+                            const int j4 = nt * 8 + 2 * q;
+                            if (j4 < n4) dst[nt * 8] = c0;
+                            if (j4 + 1 < n4) dst[nt * 8 + 1] = c1;
                         }
                     }
-                    if (m < rows) {
-                        const int vv = m / n5, i5 = m - vv * n5, j4 = nt * 8 + 2 * q;
-                        double* dst = Qs + (vv * W4p + r4) * LDQ + i5 * n4 + j4;
-                        if (j4 < n4) dst[0] = c0;
-                        if (j4 + 1 < n4) dst[1] = c1;
+                }
+            }
+        } else {
+            for (int r4 = warp; r4 < w4; r4 += FZ_QP_THREADS / 32) {
+                const int q4 = lo4 + r4;
+                const double* zq = Zb + ((long)q4 * V + v0) * n5;
+                for (int nt = 0; nt < NT4; ++nt) {
+                    const int i4 = nt * 8 + g;
+                    double bf[8];
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks) {
+                        const int b45 = 4 * ks + q;
+                        bf[ks] = (ks < KS45 && b45 < c45 && i4 < n4) ? __ldg(B4b + ((long)q4 * c45 + b45) * c2434 * n4 + i4) : 0.0;
+                    }
+                    for (int mt = 0; mt < MT; ++mt) {
+                        const int m = mt * 8 + g;
+                        double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                        for (int ks = 0; ks < 8; ++ks) {
+                            if (ks < KS45) {
+                                const int b45 = 4 * ks + q;
+                                const double av = (m < rows && b45 < c45) ? __ldg(zq + b45 * sZ + m) : 0.0;
+                                fz_dmma(c0, c1, av, bf[ks]);
+                            }
+                        }
+                        if (m < rows) {
+                            const int vv = m / n5, i5 = m - vv * n5, j4 = nt * 8 + 2 * q;
+                            double* dst = Qs + (vv * W4p + r4) * LDQ + i5 * n4 + j4;
+                            if (j4 < n4) dst[0] = c0;
+                            if (j4 + 1 < n4) dst[1] = c1;
+                        }
                     }
                 }
             }
         }
         __syncthreads();
-        // ---- P phase ----
-        for (int task = warp; task < nv * MT3 * NT; task += FZ_QP_THREADS / 32) {
-            const int nt = task % NT, t2 = task / NT, mt3 = t2 % MT3, vv = t2 / MT3;
+        // ---- P phase: one A fragment feeds four column tiles (four independent accumulator chains) ----
+        const int NTQ = (NT + 3) >> 2;
+        for (int task = warp; task < nv * MT3 * NTQ; task += FZ_QP_THREADS / 32) {
+            const int ntq = task % NTQ, t2 = task / NTQ, mt3 = t2 % MT3, vv = t2 / MT3;
             const double* ap = S3s + (vv * W3p + mt3 * 8 + g) * LDS3 + q;
-            const double* bp = Qs + (vv * W4p + q) * LDQ + nt * 8 + g;
-            double c0 = 0.0, c1 = 0.0;
-            for (int ks = 0; ks < W4r; ks += 4) fz_dmma(c0, c1, ap[ks], bp[ks * LDQ]);
-            const int r3 = mt3 * 8 + g, n = nt * 8 + 2 * q;
-            if (r3 < w3.y && n < n54) {
-                double* dst = Pb + ((long)(w3.x + r3) * V + v0 + vv) * prow + n;
-                *reinterpret_cast<double2*>(dst) = make_double2(c0, c1);   // NP is even: n + 1 < NP, rows 16-byte aligned
+            const double* bp = Qs + (vv * W4p + q) * LDQ + ntq * 32 + g;
+            double c[4][2];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) c[j][0] = c[j][1] = 0.0;
+            for (int ks = 0; ks < W4r; ks += 4) {
+                const double av = ap[ks];
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (ntq * 4 + j < NT) fz_dmma(c[j][0], c[j][1], av, bp[ks * LDQ + 8 * j]);
+            }
+            const int r3 = mt3 * 8 + g;
+            if (r3 < w3.y) {
+                double* dst = Pb + ((long)(w3.x + r3) * V + v0 + vv) * prow + ntq * 32 + 2 * q;
+#pragma unroll
+                for (int j = 0; j < 4; ++j)     // NP is even: n + 1 < NP whenever n < n54, and rows are 16-byte aligned
+                    if (ntq * 32 + 8 * j + 2 * q < n54) *reinterpret_cast<double2*>(dst + 8 * j) = make_double2(c[j][0], c[j][1]);
             }
         }
     }
@@ -363,7 +454,8 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
 // ---------------------------------------------------------------------------------------------------------
 struct FzGemmHdr {
     int M, N, K;
-    long baseA, baseB, baseC;
+    int nsub;                   // products that share A and the index tables: B and C advance by sB, sC
+    long baseA, baseB, baseC, sB, sC;
 };
 
 __device__ __forceinline__ unsigned fz_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -378,29 +470,8 @@ __device__ __forceinline__ void fz_cp_wait()
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// ordered compaction by warp 0: kk-th accepted candidate gets (fa(cand), fb(cand)); returns the count in *K
-template <class Pred, class FA, class FB>
-__device__ __forceinline__ void fz_compact(int ncand, Pred pred, FA fa, FB fb, int* offAk, int* offBk, int* K)
-{
-    if (threadIdx.x >= 32) return;
-    const int lane = threadIdx.x;
-    int cnt = 0;
-    for (int base = 0; base < ncand; base += 32) {
-        const int c = base + lane;
-        const bool ok = c < ncand && pred(c);
-        const unsigned mask = __ballot_sync(0xffffffffu, ok);
-        if (ok) {
-            const int pos = cnt + __popc(mask & ((1u << lane) - 1u));
-            offAk[pos] = fa(c);
-            offBk[pos] = fb(c);
-        }
-        cnt += __popc(mask);
-    }
-    if (lane == 0) *K = cnt;
-}
-
 // R[l24 l25 i1; k3 x; l23 i3; (i5 i4)] = sum over the pairs (l34 l35) that allow k3 of Bw3T[k3][(l34 l35)][(l23 i3)] P[..][(l34 l35)][(i5 i4)]
-// rows m = (l23 i3) over the l23 whose pair (j13 l23) allows k3
+// rows m = (l23 i3) over the l23 whose pair (j13 l23) allows k3; one item = (i1, l24, l25, k3, tile), every x of (i1 l25)
 struct FzMapR {
     static __device__ const double* srcA(const FzParams& p) { return p.Bw3T; }
     static __device__ const double* srcB(const FzParams& p) { return p.Pq; }
@@ -408,41 +479,37 @@ struct FzMapR {
     static __host__ __device__ long items(const FzParams& p, int BM, int BN)
     {
         const long ntn = (p.P.n_i[3] * p.P.n_i[4] + BN - 1) / BN, ntm = (p.box.cnt[0] * p.P.n_i[2] + BM - 1) / BM;
-        return ntn * ntm * p.V * p.P.n_k_pad[1] * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
+        return ntn * ntm * p.P.n_k_pad[1] * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
     }
     static __device__ void setup(const FzParams& p, long item, int BM, int BN, FzGemmHdr* h, int* offAm, int* offCm,
-                                 int* offBn, int* offCn, int* offAk, int* offBk)
+                                 int* offBn, int* offCn, int* offAk, int* offBk, int* tmp)
     {
         const SfProblem& P = p.P;
-        const int nl = P.nl, n3 = P.n_i[2], n54 = P.n_i[3] * P.n_i[4], P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
+        const int n3 = P.n_i[2], n54 = P.n_i[3] * P.n_i[4], P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
         const int c23 = p.box.cnt[0], c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
         const int ntn = (n54 + BN - 1) / BN, ntm = (c23 * n3 + BM - 1) / BM;
         const int nt = (int)(item % ntn); item /= ntn;
         const int mt = (int)(item % ntm); item /= ntm;
-        const int v = (int)(item % V); item /= V;
         const int q3 = (int)(item % P3); item /= P3;
         const int b25 = (int)(item % c25); item /= c25;
         const int b24 = (int)(item % c24);
         const int ac = (int)(item / c24);
         int x0, nxs, xg0;
         fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, p.a_lo + ac, p.box.lo[2] + b25, x0, nxs, xg0);
-        int blo = -1, bcnt = 0;
-        for (int b = 0; b < c23; ++b) {
-            const int2 w = p.w3B[p.box.lo[0] + b];
-            if (q3 >= w.x && q3 < w.x + w.y) {
-                if (blo < 0) blo = b;
-                ++bcnt;
-            }
-        }
-        const int m0 = mt * BM, M = v < nxs ? min(BM, bcnt * n3 - m0) : 0, N = min(BN, n54 - nt * BN);
+        const int2 win = p.win23[q3];
+        const int* list = p.kl3 + (long)q3 * (1 + c34 * c35);
+        const int m0 = mt * BM, M = min(BM, win.y * n3 - m0), N = min(BN, n54 - nt * BN), K = list[0];
         if (threadIdx.x == 0) {
             h->M = M;
             h->N = N;
-            h->K = 0;
-            const long slab = ((((long)ac * c24 + b24) * c25 + b25) * P3 + q3) * V + v;
-            h->baseA = (long)q3 * c34 * c35 * c23 * n3 + (long)blo * n3 + m0;
+            h->K = K;
+            h->nsub = nxs;
+            const long slab = ((((long)ac * c24 + b24) * c25 + b25) * P3 + q3) * V;
+            h->baseA = (long)q3 * c34 * c35 * c23 * n3 + (long)win.x * n3 + m0;
             h->baseB = slab * c34 * c35 * NP + (long)nt * BN;
-            h->baseC = ((slab * c23 + blo) * n3 + m0) * NP + (long)nt * BN;
+            h->baseC = ((slab * c23 + win.x) * n3 + m0) * NP + (long)nt * BN;
+            h->sB = (long)c34 * c35 * NP;
+            h->sC = (long)c23 * n3 * NP;
         }
         if (M <= 0) return;
         for (int m = threadIdx.x; m < BM; m += blockDim.x) {
@@ -450,14 +517,11 @@ struct FzMapR {
             offCm[m] = m * NP;
         }
         for (int n = threadIdx.x; n < BN; n += blockDim.x) offBn[n] = offCn[n] = n;
-        const int lo34 = p.box.lo[3], lo35 = p.box.lo[4];
-        fz_compact(
-            c34 * c35,
-            [&](int c) {
-                const int2 w = p.w3A[(lo34 + c / c35) * nl + lo35 + c % c35];
-                return q3 >= w.x && q3 < w.x + w.y;
-            },
-            [&](int c) { return c * c23 * n3; }, [&](int c) { return c * NP; }, offAk, offBk, &h->K);
+        for (int kk = threadIdx.x; kk < K; kk += blockDim.x) {
+            const int c = list[1 + kk];
+            offAk[kk] = c * c23 * n3;
+            offBk[kk] = c * NP;
+        }
     }
 };
 
@@ -472,7 +536,7 @@ struct FzMapA {
         return ntn * ntm * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
     }
     static __device__ void setup(const FzParams& p, long item, int BM, int BN, FzGemmHdr* h, int* offAm, int* offCm,
-                                 int* offBn, int* offCn, int* offAk, int* offBk)
+                                 int* offBn, int* offCn, int* offAk, int* offBk, int* tmp)
     {
         const SfProblem& P = p.P;
         const int n1 = P.n_i[0], n2 = P.n_i[1], n3 = P.n_i[2], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5, n345 = n3 * n54;
@@ -488,13 +552,22 @@ struct FzMapA {
         int x0, nxs, xg0;
         fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, p.box.lo[2] + b25, x0, nxs, xg0);
         const int m0 = mt * BM, n0 = nt * BN, M = min(BM, n2 - m0), N = min(BN, n345 - n0);
+        // k list in the order (k3, x, l23): prefix sums over k3 of (x count) * (l23 count)
         if (threadIdx.x == 0) {
+            int run = 0;
+            for (int q3 = 0; q3 < P3; ++q3) {
+                tmp[q3] = run;
+                run += p.win23[q3].y * nxs;
+            }
+            tmp[P3] = run;
             h->M = M;
             h->N = N;
-            h->K = 0;
+            h->K = run;
+            h->nsub = 1;
             h->baseA = ((((long)b24 * c25 + b25) * n1 + a1) * P3 * V * c23) * n2;
             h->baseB = (((long)ac * c24 + b24) * c25 + b25) * ((long)P3 * V * c23 * n3 * NP);
             h->baseC = ((p.part0 + (long)b24 * c25 + b25) * n1 + a1) * ((long)n2 * n345);
+            h->sB = h->sC = 0;
         }
         for (int m = threadIdx.x; m < BM; m += blockDim.x) {
             offAm[m] = m0 + m;
@@ -505,23 +578,17 @@ struct FzMapA {
             offBn[n] = i3 * NP + r;
             offCn[n] = (i3 * n4 + i4) * n5 + i5;
         }
-        const int lo23 = p.box.lo[0];
-        fz_compact(
-            P3 * nxs * c23,
-            [&](int c) {
-                const int2 w = p.w3B[lo23 + c % c23];
-                const int q3 = c / (nxs * c23);
-                return q3 >= w.x && q3 < w.x + w.y;
-            },
-            [&](int c) {
-                const int b23 = c % c23, r = c / c23, v = r % nxs, q3 = r / nxs;
-                return ((q3 * V + v) * c23 + b23) * n2;
-            },
-            [&](int c) {
-                const int b23 = c % c23, r = c / c23, v = r % nxs, q3 = r / nxs;
-                return ((q3 * V + v) * c23 + b23) * n3 * NP;
-            },
-            offAk, offBk, &h->K);
+        __syncthreads();
+        for (int e = threadIdx.x; e < P3 * nxs; e += blockDim.x) {
+            const int q3 = e / nxs, v = e - q3 * nxs;
+            const int2 win = p.win23[q3];
+            const int at = tmp[q3] + v * win.y;
+            for (int b = 0; b < win.y; ++b) {
+                const int row = (q3 * V + v) * c23 + win.x + b;
+                offAk[at + b] = row * n2;
+                offBk[at + b] = row * n3 * NP;
+            }
+        }
     }
 };
 
@@ -539,23 +606,57 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     int* offCm = offAm + BM;
     int* offBn = offCm + BM;
     int* offCn = offBn + BN;
-    int* offAk = offCn + BN;
+    int* tmp = offCn + BN;                           // 80 ints of scratch for the setup
+    int* offAk = tmp + 80;
     int* offBk = offAk + kcap;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
     const int wm = warp / WGN, wn = warp % WGN;
-    Map::setup(p, blockIdx.x, BM, BN, &hdr, offAm, offCm, offBn, offCn, offAk, offBk);
+    Map::setup(p, blockIdx.x, BM, BN, &hdr, offAm, offCm, offBn, offCn, offAk, offBk, tmp);
     __syncthreads();
-    const int M = hdr.M, N = hdr.N, K = hdr.K;
+    const int M = hdr.M, N = hdr.N, K = hdr.K, nsub = hdr.nsub;
     if (M <= 0) return;
     const double* A0 = Map::srcA(p);
     const double* B0 = Map::srcB(p);
     const double* A = A0 + hdr.baseA;
     const double* B = B0 + hdr.baseB;
     double* C = Map::dstC(p) + hdr.baseC;
-    const int nchunks = (K + FZ_KC - 1) / FZ_KC;
-    auto load_chunk = [&](int c) {
-        if (c < nchunks) {
-            const int s = c % FZ_STAGES, k0 = c * FZ_KC;
+    const long sB = hdr.sB, sC = hdr.sC;
+    const int nchunks = (K + FZ_KC - 1) / FZ_KC, total = nsub * nchunks;
+    const bool active = wm * TM * 8 < M && wn * TN * 8 < N;
+
+    double acc[TM][TN][2];
+#pragma unroll
+    for (int i = 0; i < TM; ++i)
+#pragma unroll
+        for (int j = 0; j < TN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    auto store = [&](int sub) {                      // C fragments of one product to its rows of the destination
+        if (!active) return;
+        double* cs = C + sub * sC;
+#pragma unroll
+        for (int i = 0; i < TM; ++i) {
+            const int m = wm * TM * 8 + 8 * i + g;
+            if (m < M) {
+                double* cm = cs + offCm[m];
+#pragma unroll
+                for (int j = 0; j < TN; ++j) {
+                    const int n = wn * TN * 8 + 8 * j + 2 * q;
+                    if (n < N) cm[offCn[n]] = acc[i][j][0];
+                    if (n + 1 < N) cm[offCn[n + 1]] = acc[i][j][1];
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < TN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        }
+    };
+    if (nchunks == 0) {                              // nothing to sum: the destination rows are exact zeros
+        for (int sub = 0; sub < nsub; ++sub) store(sub);
+        return;
+    }
+    int l_sub = 0, l_c = 0;                          // next chunk to request: product l_sub, chunk l_c of it
+    auto load_chunk = [&](int gc) {
+        if (gc < total) {
+            const int s = gc % FZ_STAGES, k0 = l_c * FZ_KC;
+            const double* Bq = B + l_sub * sB;
             for (int e = tid; e < FZ_KC * BM; e += NTH) {
                 const int kr = e / BM, m = e % BM, k = k0 + kr;
                 const bool ok = m < M && k < K;
@@ -564,26 +665,25 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
             for (int e = tid; e < FZ_KC * BN; e += NTH) {
                 const int kr = e / BN, n = e % BN, k = k0 + kr;
                 const bool ok = n < N && k < K;
-                fz_cp_async8(fz_smem_u32(Bs + (s * FZ_KC + kr) * LDB + n), ok ? B + offBk[k] + offBn[n] : B0, ok ? 8 : 0);
+                fz_cp_async8(fz_smem_u32(Bs + (s * FZ_KC + kr) * LDB + n), ok ? Bq + offBk[k] + offBn[n] : B0, ok ? 8 : 0);
+            }
+            if (++l_c == nchunks) {
+                l_c = 0;
+                ++l_sub;
             }
         }
         fz_cp_commit();
     };
-    double acc[TM][TN][2];
-#pragma unroll
-    for (int i = 0; i < TM; ++i)
-#pragma unroll
-        for (int j = 0; j < TN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-    const bool active = wm * TM * 8 < M && wn * TN * 8 < N;
 #pragma unroll
     for (int c = 0; c < FZ_STAGES - 1; ++c) load_chunk(c);
-    for (int c = 0; c < nchunks; ++c) {
+    int c_in = 0, sub = 0;
+    for (int gc = 0; gc < total; ++gc) {
         fz_cp_wait<FZ_STAGES - 2>();
-        __syncthreads();                             // chunk c has landed; every warp is done with chunk c - 1
-        load_chunk(c + FZ_STAGES - 1);               // refills the stage chunk c - 1 used
+        __syncthreads();                             // chunk gc has landed; every warp is done with chunk gc - 1
+        load_chunk(gc + FZ_STAGES - 1);              // refills the stage chunk gc - 1 used
         if (active) {
-            const double* as = As + (c % FZ_STAGES) * FZ_KC * LDA + q * LDA + wm * TM * 8 + g;
-            const double* bs = Bs + (c % FZ_STAGES) * FZ_KC * LDB + q * LDB + wn * TN * 8 + g;
+            const double* as = As + (gc % FZ_STAGES) * FZ_KC * LDA + q * LDA + wm * TM * 8 + g;
+            const double* bs = Bs + (gc % FZ_STAGES) * FZ_KC * LDB + q * LDB + wn * TN * 8 + g;
 #pragma unroll
             for (int ks = 0; ks < FZ_KC / 4; ++ks) {
                 double a[TM], b[TN];
@@ -597,21 +697,13 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
                     for (int j = 0; j < TN; ++j) fz_dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
             }
         }
-    }
-    fz_cp_wait<0>();
-    if (!active) return;
-#pragma unroll
-    for (int i = 0; i < TM; ++i) {
-        const int m = wm * TM * 8 + 8 * i + g;
-        if (m >= M) continue;
-        double* cm = C + offCm[m];
-#pragma unroll
-        for (int j = 0; j < TN; ++j) {
-            const int n = wn * TN * 8 + 8 * j + 2 * q;
-            if (n < N) cm[offCn[n]] = acc[i][j][0];
-            if (n + 1 < N) cm[offCn[n + 1]] = acc[i][j][1];
+        if (++c_in == nchunks) {
+            store(sub);
+            c_in = 0;
+            ++sub;
         }
     }
+    fz_cp_wait<0>();
 }
 
 // kernel (d): out[a1][i2][r] = prod_e sqrt(2 i_e + 1) * sum over the partial tensors, in order, of Apart[part][a1][i2][r]
@@ -699,7 +791,7 @@ static FzShape fz_shape(const SfDims& D)
     memset(&s, 0, sizeof s);
     for (int e = 0; e < 4; ++e)
         if (D.k_max[e] == 0) return s;
-    if (D.nl > 32) return s;
+    if (D.nl > 32 || D.n_k_pad[1] > 78) return s;     // k_fz_gemm keeps P3 + 1 prefix sums in 80 ints
     for (int a = 0; a < D.n_i[0]; ++a)
         for (int o = 0; o < D.nl; ++o) {
             int x0, nxs, xg0;
@@ -750,7 +842,7 @@ template <class Map, int WGM, int WGN, int TM, int TN>
 static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
 {
     constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8;
-    const size_t smem = sizeof(double) * FZ_STAGES * FZ_KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 2 * (size_t)kcap);
+    const size_t smem = sizeof(double) * FZ_STAGES * FZ_KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 80 + 2 * (size_t)kcap);
     if (smem > 226 * 1024) return SF_EARG;
     static size_t attr = 0;
     if (smem > attr) {
@@ -766,7 +858,7 @@ static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
     return SF_OK;
 }
 
-enum { FZ_SLOT_WIN = 24, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART };
+enum { FZ_SLOT_WIN = 24, FZ_SLOT_LIST, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART };
 
 int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st)
 {
@@ -851,7 +943,10 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         double* G = (double*)sf_scratch(FZ_SLOT_G, sizeof(double) * (size_t)nG);
         double* Pq = (double*)sf_scratch(FZ_SLOT_P, sizeof(double) * (size_t)(pP * na));
         double* Rq = (double*)sf_scratch(FZ_SLOT_R, sizeof(double) * (size_t)(pR * na));
-        if (!Z || !B4 || !B3 || !S3 || !G || !Pq || !Rq) return SF_ENOMEM;
+        int* lists = (int*)sf_scratch(FZ_SLOT_LIST, sizeof(int2) * P3 + sizeof(int) * (size_t)P3 * (1 + c34 * c35));
+        if (!Z || !B4 || !B3 || !S3 || !G || !Pq || !Rq || !lists) return SF_ENOMEM;
+        p.win23 = (const int2*)lists;
+        p.kl3 = lists + 2 * P3;
         p.Z = Z;
         p.Bw4T = B4;
         p.Bw3T = B3;
@@ -866,7 +961,8 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         k_fz_b3t<<<(unsigned)((nB3 + 255) / 256), 256, 0, st>>>(p, nB3, B3);
         k_fz_s3t<<<(unsigned)((nS3 + 255) / 256), 256, 0, st>>>(p, nS3, S3);
         k_fz_g<<<(unsigned)((nG + 255) / 256), 256, 0, st>>>(p, nG, G);
-        sf_count_launch(5);
+        k_fz_lists<<<P3, 32, 0, st>>>(p, (int2*)lists, lists + 2 * P3);
+        sf_count_launch(6);
         for (int a_lo = 0; a_lo < n1; a_lo += (int)na) {
             p.a_lo = a_lo;
             p.a_cnt = (int)(a_lo + na <= n1 ? na : n1 - a_lo);
