@@ -99,6 +99,20 @@ __device__ __forceinline__ void fz_dmma(double& c0, double& c1, double a, double
         : "d"(a), "d"(b));
 }
 
+__device__ __forceinline__ unsigned fz_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void fz_cp_async8(unsigned dst, const void* src, int bytes)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void fz_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void fz_cp_wait()
+{
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+__device__ __forceinline__ void fz_prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 // ---------------------------------------------------------------------------------------------------------
 // small precomputations (step 2 windows, weighted / transposed operands)
 // ---------------------------------------------------------------------------------------------------------
@@ -340,12 +354,13 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
     for (int v0 = 0; v0 < nxs; v0 += VG) {
         const int nv = min(VG, nxs - v0), rows = nv * n5, MT = (rows + 7) >> 3;
         __syncthreads();                             // the previous P phase has read Qs and S3s
-        for (int e = tid; e < nv * W3p * W4p; e += FZ_QP_THREADS) {
+        for (int e = tid; e < nv * W3p * W4p; e += FZ_QP_THREADS) {      // lands under the Q phase
             const int r4 = e % W4p, r = e / W4p, r3 = r % W3p, vv = r / W3p;
-            double val = 0.0;
-            if (r3 < w3.y && r4 < w4) val = __ldg(S3b + ((long)(v0 + vv) * P3 + w3.x + r3) * P4 + lo4 + r4);
-            S3s[(vv * W3p + r3) * LDS3 + r4] = val;
+            const bool ok = r3 < w3.y && r4 < w4;
+            fz_cp_async8(fz_smem_u32(S3s + (vv * W3p + r3) * LDS3 + r4),
+                         ok ? S3b + ((long)(v0 + vv) * P3 + w3.x + r3) * P4 + lo4 + r4 : S3b, ok ? 8 : 0);
         }
+        fz_cp_commit();
         // ---- Q phase ----
         if (KS45 <= FZ_QKS && NT4 <= FZ_QNT && MT <= FZ_QMT) {
             // common sizes: every fragment of a k4 is requested before the first MMA, so one round of L2 latency per k4
@@ -422,7 +437,17 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
                 }
             }
         }
+        fz_cp_wait<0>();
         __syncthreads();
+        if (v0 + VG < nxs) {                         // the next pass's rows of Z: into L1 under this pass's P phase
+            const int rows2 = min(VG, nxs - v0 - VG) * n5, lines = (rows2 * 8 + 127) / 128 + 1;
+            for (int e = tid; e < c45 * w4 * lines; e += FZ_QP_THREADS) {
+                const int ln = e % lines, r = e / lines, r4 = r % w4, b45 = r / w4;
+                const double* row = Zb + b45 * sZ + ((long)(lo4 + r4) * V + v0 + VG) * n5;
+                const int off = ln * 16 < rows2 ? ln * 16 : rows2 - 1;
+                fz_prefetch_l1(row + off);
+            }
+        }
         // ---- P phase: one A fragment feeds four column tiles (four independent accumulator chains) ----
         const int NTQ = (NT + 3) >> 2;
         for (int task = warp; task < nv * MT3 * NTQ; task += FZ_QP_THREADS / 32) {
@@ -454,31 +479,20 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
 // ---------------------------------------------------------------------------------------------------------
 struct FzGemmHdr {
     int M, N, K;
-    int nsub;                   // products that share A and the index tables: B and C advance by sB, sC
-    long baseA, baseB, baseC, sB, sC;
+    int nsub;                   // products that share the index tables: A, B and C advance by sA, sB, sC
+    long baseA, baseB, baseC, sA, sB, sC;
 };
 
-__device__ __forceinline__ unsigned fz_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void fz_cp_async8(unsigned dst, const void* src, int bytes)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void fz_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void fz_cp_wait()
-{
-    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
-}
-
-// R[l24 l25 i1; k3 x; l23 i3; (i5 i4)] = sum over the pairs (l34 l35) that allow k3 of Bw3T[k3][(l34 l35)][(l23 i3)] P[..][(l34 l35)][(i5 i4)]
-// rows m = (l23 i3) over the l23 whose pair (j13 l23) allows k3; one item = (i1, l24, l25, k3, tile), every x of (i1 l25)
+// R[l24 l25 i1; k3 x; l23 i3; (i5 i4)] = sum over the pairs (l34 l35) that allow k3 of P[..][(l34 l35)][(i5 i4)] Bw3T[k3][(l34 l35)][(l23 i3)]
+// rows m = (i5 i4), columns n = (l23 i3) over the l23 whose pair (j13 l23) allows k3; one item = (i1, l24, l25, k3, tile),
+// every x of (i1 l25) in turn
 struct FzMapR {
-    static __device__ const double* srcA(const FzParams& p) { return p.Bw3T; }
-    static __device__ const double* srcB(const FzParams& p) { return p.Pq; }
+    static __device__ const double* srcA(const FzParams& p) { return p.Pq; }
+    static __device__ const double* srcB(const FzParams& p) { return p.Bw3T; }
     static __device__ double* dstC(const FzParams& p) { return p.Rq; }
     static __host__ __device__ long items(const FzParams& p, int BM, int BN)
     {
-        const long ntn = (p.P.n_i[3] * p.P.n_i[4] + BN - 1) / BN, ntm = (p.box.cnt[0] * p.P.n_i[2] + BM - 1) / BM;
+        const long ntm = (p.P.n_i[3] * p.P.n_i[4] + BM - 1) / BM, ntn = (p.box.cnt[0] * p.P.n_i[2] + BN - 1) / BN;
         return ntn * ntm * p.P.n_k_pad[1] * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
     }
     static __device__ void setup(const FzParams& p, long item, int BM, int BN, FzGemmHdr* h, int* offAm, int* offCm,
@@ -487,7 +501,7 @@ struct FzMapR {
         const SfProblem& P = p.P;
         const int n3 = P.n_i[2], n54 = P.n_i[3] * P.n_i[4], P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
         const int c23 = p.box.cnt[0], c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
-        const int ntn = (n54 + BN - 1) / BN, ntm = (c23 * n3 + BM - 1) / BM;
+        const int ntm = (n54 + BM - 1) / BM, ntn = (c23 * n3 + BN - 1) / BN;
         const int nt = (int)(item % ntn); item /= ntn;
         const int mt = (int)(item % ntm); item /= ntm;
         const int q3 = (int)(item % P3); item /= P3;
@@ -498,29 +512,30 @@ struct FzMapR {
         fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, p.a_lo + ac, p.box.lo[2] + b25, x0, nxs, xg0);
         const int2 win = p.win23[q3];
         const int* list = p.kl3 + (long)q3 * (1 + c34 * c35);
-        const int m0 = mt * BM, M = min(BM, win.y * n3 - m0), N = min(BN, n54 - nt * BN), K = list[0];
+        const int m0 = mt * BM, n0 = nt * BN, N = min(BN, win.y * n3 - n0), M = N > 0 ? min(BM, n54 - m0) : 0, K = list[0];
         if (threadIdx.x == 0) {
             h->M = M;
             h->N = N;
             h->K = K;
             h->nsub = nxs;
             const long slab = ((((long)ac * c24 + b24) * c25 + b25) * P3 + q3) * V;
-            h->baseA = (long)q3 * c34 * c35 * c23 * n3 + (long)win.x * n3 + m0;
-            h->baseB = slab * c34 * c35 * NP + (long)nt * BN;
-            h->baseC = ((slab * c23 + win.x) * n3 + m0) * NP + (long)nt * BN;
-            h->sB = (long)c34 * c35 * NP;
+            h->baseA = slab * c34 * c35 * NP + m0;
+            h->baseB = (long)q3 * c34 * c35 * c23 * n3 + (long)win.x * n3 + n0;
+            h->baseC = ((slab * c23 + win.x) * n3 + n0) * NP + m0;
+            h->sA = (long)c34 * c35 * NP;
+            h->sB = 0;
             h->sC = (long)c23 * n3 * NP;
         }
         if (M <= 0) return;
-        for (int m = threadIdx.x; m < BM; m += blockDim.x) {
-            offAm[m] = m;
-            offCm[m] = m * NP;
+        for (int m = threadIdx.x; m < BM; m += blockDim.x) offAm[m] = offCm[m] = m;
+        for (int n = threadIdx.x; n < BN; n += blockDim.x) {
+            offBn[n] = n;
+            offCn[n] = n * NP;
         }
-        for (int n = threadIdx.x; n < BN; n += blockDim.x) offBn[n] = offCn[n] = n;
         for (int kk = threadIdx.x; kk < K; kk += blockDim.x) {
             const int c = list[1 + kk];
-            offAk[kk] = c * c23 * n3;
-            offBk[kk] = c * NP;
+            offAk[kk] = c * NP;
+            offBk[kk] = c * c23 * n3;
         }
     }
 };
@@ -567,7 +582,7 @@ struct FzMapA {
             h->baseA = ((((long)b24 * c25 + b25) * n1 + a1) * P3 * V * c23) * n2;
             h->baseB = (((long)ac * c24 + b24) * c25 + b25) * ((long)P3 * V * c23 * n3 * NP);
             h->baseC = ((p.part0 + (long)b24 * c25 + b25) * n1 + a1) * ((long)n2 * n345);
-            h->sB = h->sC = 0;
+            h->sA = h->sB = h->sC = 0;
         }
         for (int m = threadIdx.x; m < BM; m += blockDim.x) {
             offAm[m] = m0 + m;
@@ -594,6 +609,44 @@ struct FzMapA {
 
 #define FZ_KC 16
 #define FZ_STAGES 3
+// one k-chunk of a warp tile with TNA live column tiles (tiles beyond N are skipped, not multiplied by zeros)
+template <int TM, int TN, int TNA>
+__device__ __forceinline__ void fz_chunk(double (&acc)[TM][TN][2], const double* as, const double* bs, int LDA, int LDB,
+                                         int ksn, int tma)
+{
+#pragma unroll
+    for (int ks = 0; ks < FZ_KC / 4; ++ks) {
+        if (ks < ksn) {
+            double a[TM], b[TNA];
+#pragma unroll
+            for (int i = 0; i < TM; ++i) a[i] = as[ks * 4 * LDA + 8 * i];
+#pragma unroll
+            for (int j = 0; j < TNA; ++j) b[j] = bs[ks * 4 * LDB + 8 * j];
+#pragma unroll
+            for (int i = 0; i < TM; ++i) {
+                if (i < tma) {
+#pragma unroll
+                    for (int j = 0; j < TNA; ++j) fz_dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                }
+            }
+        }
+    }
+}
+template <int TM, int TN, int TNA>
+struct FzChunk {
+    static __device__ __forceinline__ void run(double (&acc)[TM][TN][2], const double* as, const double* bs, int LDA,
+                                               int LDB, int ksn, int tma, int tna)
+    {
+        if (tna == TNA)
+            fz_chunk<TM, TN, TNA>(acc, as, bs, LDA, LDB, ksn, tma);
+        else
+            FzChunk<TM, TN, TNA - 1>::run(acc, as, bs, LDA, LDB, ksn, tma, tna);
+    }
+};
+template <int TM, int TN>
+struct FzChunk<TM, TN, 0> {
+    static __device__ __forceinline__ void run(double (&)[TM][TN][2], const double*, const double*, int, int, int, int, int) {}
+};
 template <class Map, int WGM, int WGN, int TM, int TN>
 __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int kcap)
 {
@@ -620,9 +673,14 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     const double* A = A0 + hdr.baseA;
     const double* B = B0 + hdr.baseB;
     double* C = Map::dstC(p) + hdr.baseC;
-    const long sB = hdr.sB, sC = hdr.sC;
+    const long sA = hdr.sA, sB = hdr.sB, sC = hdr.sC;
     const int nchunks = (K + FZ_KC - 1) / FZ_KC, total = nsub * nchunks;
-    const bool active = wm * TM * 8 < M && wn * TN * 8 < N;
+    int tma = 0, tna = 0;                            // live 8-row / 8-column tiles of this warp
+#pragma unroll
+    for (int i = 0; i < TM; ++i) tma += (wm * TM + i) * 8 < M;
+#pragma unroll
+    for (int j = 0; j < TN; ++j) tna += (wn * TN + j) * 8 < N;
+    const bool active = tma > 0 && tna > 0;
 
     double acc[TM][TN][2];
 #pragma unroll
@@ -656,11 +714,12 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     auto load_chunk = [&](int gc) {
         if (gc < total) {
             const int s = gc % FZ_STAGES, k0 = l_c * FZ_KC;
+            const double* Aq = A + l_sub * sA;
             const double* Bq = B + l_sub * sB;
             for (int e = tid; e < FZ_KC * BM; e += NTH) {
                 const int kr = e / BM, m = e % BM, k = k0 + kr;
                 const bool ok = m < M && k < K;
-                fz_cp_async8(fz_smem_u32(As + (s * FZ_KC + kr) * LDA + m), ok ? A + offAk[k] + offAm[m] : A0, ok ? 8 : 0);
+                fz_cp_async8(fz_smem_u32(As + (s * FZ_KC + kr) * LDA + m), ok ? Aq + offAk[k] + offAm[m] : A0, ok ? 8 : 0);
             }
             for (int e = tid; e < FZ_KC * BN; e += NTH) {
                 const int kr = e / BN, n = e % BN, k = k0 + kr;
@@ -684,18 +743,8 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
         if (active) {
             const double* as = As + (gc % FZ_STAGES) * FZ_KC * LDA + q * LDA + wm * TM * 8 + g;
             const double* bs = Bs + (gc % FZ_STAGES) * FZ_KC * LDB + q * LDB + wn * TN * 8 + g;
-#pragma unroll
-            for (int ks = 0; ks < FZ_KC / 4; ++ks) {
-                double a[TM], b[TN];
-#pragma unroll
-                for (int i = 0; i < TM; ++i) a[i] = as[ks * 4 * LDA + 8 * i];
-#pragma unroll
-                for (int j = 0; j < TN; ++j) b[j] = bs[ks * 4 * LDB + 8 * j];
-#pragma unroll
-                for (int i = 0; i < TM; ++i)
-#pragma unroll
-                    for (int j = 0; j < TN; ++j) fz_dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-            }
+            const int ksn = min(FZ_KC / 4, (K - c_in * FZ_KC + 3) >> 2);
+            FzChunk<TM, TN, TN>::run(acc, as, bs, LDA, LDB, ksn, tma, tna);
         }
         if (++c_in == nchunks) {
             store(sub);
@@ -968,7 +1017,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             p.a_cnt = (int)(a_lo + na <= n1 ? na : n1 - a_lo);
             k_fz_qp<<<(unsigned)((long)p.a_cnt * c25 * c35 * c24 * c34), FZ_QP_THREADS, sh.qp_smem, st>>>(p);
             sf_count_launch(1);
-            int rc = fz_launch_gemm<FzMapR, 4, 2, 4, 4>(p, (int)(c34 * c35), st);
+            int rc = fz_launch_gemm<FzMapR, 8, 1, 2, 8>(p, (int)(c34 * c35), st);
             if (rc != SF_OK) return rc;
             rc = fz_launch_gemm<FzMapA, 1, 8, 2, 4>(p, (int)(P3 * sh.V * c23), st);
             if (rc != SF_OK) return rc;
