@@ -104,6 +104,10 @@ __device__ __forceinline__ void fz_cp_async8(unsigned dst, const void* src, int 
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void fz_cp_async16(unsigned dst, const void* src, int bytes)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void fz_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void fz_cp_wait()
@@ -487,6 +491,7 @@ struct FzGemmHdr {
 // rows m = (i5 i4), columns n = (l23 i3) over the l23 whose pair (j13 l23) allows k3; one item = (i1, l24, l25, k3, tile),
 // every x of (i1 l25) in turn
 struct FzMapR {
+    static constexpr bool A16 = true;    // rows of P start 16-byte aligned (NP even) and m runs contiguously: copy pairs
     static __device__ const double* srcA(const FzParams& p) { return p.Pq; }
     static __device__ const double* srcB(const FzParams& p) { return p.Bw3T; }
     static __device__ double* dstC(const FzParams& p) { return p.Rq; }
@@ -542,6 +547,7 @@ struct FzMapR {
 
 // A'[l24 l25; i1; i2; (i3 i4 i5)] = sum over (k3, x, l23) with k3 allowed by (j13 l23) of G[..][(k3 x l23)][i2] R[..][(k3 x l23)][(i3, i5 i4)]
 struct FzMapA {
+    static constexpr bool A16 = false;
     static __device__ const double* srcA(const FzParams& p) { return p.G; }
     static __device__ const double* srcB(const FzParams& p) { return p.Rq; }
     static __device__ double* dstC(const FzParams& p) { return p.Apart; }
@@ -711,20 +717,34 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
         return;
     }
     int l_sub = 0, l_c = 0;                          // next chunk to request: product l_sub, chunk l_c of it
+    // every thread copies the same m (pair of m) and n of each k-row it serves: offsets and bounds are fixed per item
+    constexpr int AW = Map::A16 ? 2 : 1, ATPR = BM / AW, ARPP = NTH / ATPR, APASS = FZ_KC / ARPP;
+    constexpr int BTPR = BN, BRPP = NTH / BTPR, BPASS = FZ_KC / BRPP;
+    static_assert(NTH % ATPR == 0 && FZ_KC % ARPP == 0 && NTH % BTPR == 0 && FZ_KC % BRPP == 0, "loader shape");
+    const int am = (tid % ATPR) * AW, akr = tid / ATPR, bn = tid % BTPR, bkr = tid / BTPR;
+    const int a_bytes = 8 * max(0, min(AW, M - am)), b_bytes = bn < N ? 8 : 0;
+    const int a_off = a_bytes ? offAm[am] : 0, b_off = b_bytes ? offBn[bn] : 0;
+    const unsigned a_dst = fz_smem_u32(As + akr * LDA + am), b_dst = fz_smem_u32(Bs + bkr * LDB + bn);
     auto load_chunk = [&](int gc) {
         if (gc < total) {
             const int s = gc % FZ_STAGES, k0 = l_c * FZ_KC;
-            const double* Aq = A + l_sub * sA;
-            const double* Bq = B + l_sub * sB;
-            for (int e = tid; e < FZ_KC * BM; e += NTH) {
-                const int kr = e / BM, m = e % BM, k = k0 + kr;
-                const bool ok = m < M && k < K;
-                fz_cp_async8(fz_smem_u32(As + (s * FZ_KC + kr) * LDA + m), ok ? Aq + offAk[k] + offAm[m] : A0, ok ? 8 : 0);
+            const double* Aq = A + l_sub * sA + a_off;
+            const double* Bq = B + l_sub * sB + b_off;
+#pragma unroll
+            for (int it = 0; it < APASS; ++it) {
+                const int kr = akr + it * ARPP, k = k0 + kr;
+                const bool ok = a_bytes && k < K;
+                const unsigned dst = a_dst + 8u * (unsigned)((s * FZ_KC + it * ARPP) * LDA);
+                if (Map::A16)
+                    fz_cp_async16(dst, ok ? Aq + offAk[k] : A0, ok ? a_bytes : 0);
+                else
+                    fz_cp_async8(dst, ok ? Aq + offAk[k] : A0, ok ? 8 : 0);
             }
-            for (int e = tid; e < FZ_KC * BN; e += NTH) {
-                const int kr = e / BN, n = e % BN, k = k0 + kr;
-                const bool ok = n < N && k < K;
-                fz_cp_async8(fz_smem_u32(Bs + (s * FZ_KC + kr) * LDB + n), ok ? Bq + offBk[k] + offBn[n] : B0, ok ? 8 : 0);
+#pragma unroll
+            for (int it = 0; it < BPASS; ++it) {
+                const int kr = bkr + it * BRPP, k = k0 + kr;
+                const bool ok = b_bytes && k < K;
+                fz_cp_async8(b_dst + 8u * (unsigned)((s * FZ_KC + it * BRPP) * LDB), ok ? Bq + offBk[k] : B0, ok ? 8 : 0);
             }
             if (++l_c == nchunks) {
                 l_c = 0;
