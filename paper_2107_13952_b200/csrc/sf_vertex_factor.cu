@@ -92,6 +92,24 @@ __host__ __device__ inline void fz_xrange(const int two_i1_min, int two_j25, int
     xg0 = (x0 - two_x_base) >> 1;
 }
 
+// the x indices v (x = x0 + 2v, v < nxs) for which the triad (k l x) holds: a contiguous run (first, count).  Same
+// predicate as fz_window(l, x, ..) evaluated at k, so the rows k_fz_qp writes are the rows k_fz_gemm reads.
+__host__ __device__ inline int2 fz_vrange(int two_l, int two_k, int x0, int nxs)
+{
+    int first = -1, cnt = 0;
+    for (int v = 0; v < nxs; ++v) {
+        const int x = x0 + 2 * v, d = two_l > x ? two_l - x : x - two_l;
+        if (two_k >= d && two_k <= two_l + x && !((two_l + x + two_k) & 1)) {
+            if (first < 0) first = v;
+            ++cnt;
+        }
+    }
+    int2 r;
+    r.x = first < 0 ? 0 : first;
+    r.y = cnt;
+    return r;
+}
+
 __device__ __forceinline__ void fz_dmma(double& c0, double& c1, double a, double b)
 {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};\n"
@@ -314,13 +332,16 @@ __global__ void __launch_bounds__(32) k_fz_lists(FzParams p, int2* __restrict__ 
 // ---------------------------------------------------------------------------------------------------------
 // Q phase, per k4:  C[(v i5)][i4] = sum_l45 Z[l45][k4][(v i5)] Bw4T[k4][l45][i4]        (A and B fragments straight from L1/L2)
 // P phase, per v:   P[k3][(i5 i4)] = sum_k4 S3[k3][k4] Q[k4][(i5 i4)]                   (both operands in shared memory)
+// The triads of eq. (5) that contain x, (k4 l35 x) and (k3 l24 x), bound k4 and k3 for every x: only those k4 are
+// computed and only those rows k3 of P are written (k_fz_gemm reads exactly the same set, fz_vrange).
 #define FZ_QP_THREADS 256
 #define FZ_QKS 3      /* fast Q phase: c45 <= 12, n4 <= 16, (v, i5) rows of a pass <= 32 */
 #define FZ_QNT 2
 #define FZ_QMT 4
-__global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
+__global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p)
 {
     extern __shared__ __align__(16) double smem[];
+    constexpr int NW = FZ_QP_THREADS / 32;
     const SfProblem& P = p.P;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
     const int nl = P.nl, n1 = P.n_i[0], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5;
@@ -335,64 +356,91 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
     const int ac = (int)(it / c25);
     const int a1 = p.a_lo + ac;
     const int o24 = p.box.lo[1] + b24, o25 = p.box.lo[2] + b25, o34 = p.box.lo[3] + b34, o35 = p.box.lo[4] + b35;
+    const int l24 = P.two_j[J24] + 2 * o24, l35 = P.two_j[J35] + 2 * o35;
     int x0, nxs, xg0;
     fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
-    const int2 w3 = p.w3A[o34 * nl + o35];           // every k3 the pair (l34 l35) allows gets a row of P
+    const int2 w3 = p.w3A[o34 * nl + o35];           // the k3 the pair (l34 l35) allows
     if (w3.y == 0) return;
     const int2 w4a = p.w4A[o24 * nl + o34];
     const int lo4 = max(w4a.x, p.hull4B.x);
     const int w4 = max(0, min(w4a.x + w4a.y, p.hull4B.y) - lo4);
-    const int W4r = (w4 + 3) & ~3;
     double* Qs = smem;                               // [VG][W4p][LDQ]
     double* S3s = smem + VG * W4p * LDQ;             // [VG][W3p][LDS3]
-    for (int z = tid; z < VG * W4p * LDQ; z += FZ_QP_THREADS) Qs[z] = 0.0;   // k-padding rows must be exact zeros
+    for (int z = tid; z < VG * W4p * LDQ; z += FZ_QP_THREADS) Qs[z] = 0.0;   // rows never written must stay finite
     const int MT3 = (w3.y + 7) >> 3, NT = (n54 + 7) >> 3, NT4 = (n4 + 7) >> 3, KS45 = (c45 + 3) >> 2;
-    const long sZ = (long)P4 * V * n5;
-    const double* Zb = p.Z + ((((long)b25 * n1 + a1) * c35 + b35) * c45) * sZ;
+    const int sZ = P4 * V * n5;
+    const double* Zb = p.Z + ((((long)b25 * n1 + a1) * c35 + b35) * c45) * (long)sZ;
     const double* S3b = p.S3T + ((((long)b24 * c34 + b34) * c35 + b35) * NX + xg0) * (long)(P3 * P4);
-    const long c2434 = (long)c24 * c34;
+    const int c2434n4 = c24 * c34 * n4;
     const double* B4b = p.Bw4T + ((long)b24 * c34 + b34) * n4;
     const long prow = (long)c34 * c35 * NP;          // stride of v in P
     double* Pb = p.Pq + ((((long)ac * c24 + b24) * c25 + b25) * P3) * V * prow + ((long)b34 * c35 + b35) * NP;
+    const bool fast = KS45 <= FZ_QKS && NT4 <= FZ_QNT && ((VG * n5 + 7) >> 3) <= FZ_QMT;
+    // item constants of the fast Q phase: offsets of this lane's B fragments inside one k4 block of Bw4T (-1: zero)
+    int bofs[FZ_QNT][FZ_QKS];
+#pragma unroll
+    for (int nt = 0; nt < FZ_QNT; ++nt)
+#pragma unroll
+        for (int ks = 0; ks < FZ_QKS; ++ks) {
+            const int b45 = 4 * ks + q, i4 = nt * 8 + g;
+            bofs[nt][ks] = (ks < KS45 && b45 < c45 && nt < NT4 && i4 < n4) ? b45 * c2434n4 + i4 : -1;
+        }
 
     for (int v0 = 0; v0 < nxs; v0 += VG) {
         const int nv = min(VG, nxs - v0), rows = nv * n5, MT = (rows + 7) >> 3;
+        // k4 of this pass: union over its x of the triad (k4 l35 x), inside the item's window
+        int g4lo = w4, g4hi = 0;
+        for (int vv = 0; vv < nv; ++vv) {
+            const int2 w = fz_window(l35, x0 + 2 * (v0 + vv), P.two_k_base[2], P4);
+            const int lo = max(w.x, lo4) - lo4, hi = min(w.x + w.y, lo4 + w4) - lo4;
+            if (w.y > 0 && hi > lo) {
+                g4lo = min(g4lo, lo);
+                g4hi = max(g4hi, hi);
+            }
+        }
+        if (g4hi <= g4lo) g4lo = g4hi = 0;
+        const int k4a = g4lo & ~3, k4b = (g4hi + 3) & ~3;
         __syncthreads();                             // the previous P phase has read Qs and S3s
-        for (int e = tid; e < nv * W3p * W4p; e += FZ_QP_THREADS) {      // lands under the Q phase
-            const int r4 = e % W4p, r = e / W4p, r3 = r % W3p, vv = r / W3p;
-            const bool ok = r3 < w3.y && r4 < w4;
-            fz_cp_async8(fz_smem_u32(S3s + (vv * W3p + r3) * LDS3 + r4),
-                         ok ? S3b + ((long)(v0 + vv) * P3 + w3.x + r3) * P4 + lo4 + r4 : S3b, ok ? 8 : 0);
+        for (int row = warp; row < nv * W3p; row += NW) {                 // lands under the Q phase
+            const int vv = row / W3p, r3 = row - vv * W3p;
+            const double* src = S3b + ((long)(v0 + vv) * P3 + w3.x + r3) * P4 + lo4;
+            for (int r4 = lane; r4 < W4p; r4 += 32) {
+                const bool ok = r3 < w3.y && r4 < w4;
+                fz_cp_async8(fz_smem_u32(S3s + row * LDS3 + r4), ok ? src + r4 : S3b, ok ? 8 : 0);
+            }
         }
         fz_cp_commit();
         // ---- Q phase ----
-        if (KS45 <= FZ_QKS && NT4 <= FZ_QNT && MT <= FZ_QMT) {
+        if (fast) {
             // common sizes: every fragment of a k4 is requested before the first MMA, so one round of L2 latency per k4
-            for (int r4 = warp; r4 < w4; r4 += FZ_QP_THREADS / 32) {
-                const int q4 = lo4 + r4;
-                const double* zq = Zb + ((long)q4 * V + v0) * n5;
-                const double* bq = B4b + (long)q4 * c45 * c2434 * n4;
-                double a[FZ_QMT][FZ_QKS], b[FZ_QNT][FZ_QKS];
+            int zofs[FZ_QMT][FZ_QKS], qofs[FZ_QMT];
+#pragma unroll
+            for (int mt = 0; mt < FZ_QMT; ++mt) {
+                const int m = mt * 8 + g, vv = m / n5, i5 = m - vv * n5;
+                const bool okm = mt < MT && m < rows;
+                qofs[mt] = okm ? vv * W4p * LDQ + i5 * n4 + 2 * q : -1;
 #pragma unroll
                 for (int ks = 0; ks < FZ_QKS; ++ks) {
                     const int b45 = 4 * ks + q;
-                    const bool kin = ks < KS45 && b45 < c45;
+                    zofs[mt][ks] = (okm && ks < KS45 && b45 < c45) ? b45 * sZ + m : -1;
+                }
+            }
+            for (int r4 = g4lo + warp; r4 < g4hi; r4 += NW) {
+                const int q4 = lo4 + r4;
+                const double* zq = Zb + ((long)q4 * V + v0) * n5;
+                const double* bq = B4b + (long)q4 * c45 * c2434n4;
+                double a[FZ_QMT][FZ_QKS], b[FZ_QNT][FZ_QKS];
 #pragma unroll
-                    for (int nt = 0; nt < FZ_QNT; ++nt) {
-                        const int i4 = nt * 8 + g;
-                        b[nt][ks] = (kin && nt < NT4 && i4 < n4) ? __ldg(bq + (long)b45 * c2434 * n4 + i4) : 0.0;
-                    }
+                for (int ks = 0; ks < FZ_QKS; ++ks) {
 #pragma unroll
-                    for (int mt = 0; mt < FZ_QMT; ++mt) {
-                        const int m = mt * 8 + g;
-                        a[mt][ks] = (kin && m < rows) ? __ldg(zq + b45 * sZ + m) : 0.0;
-                    }
+                    for (int nt = 0; nt < FZ_QNT; ++nt) b[nt][ks] = bofs[nt][ks] >= 0 ? __ldg(bq + bofs[nt][ks]) : 0.0;
+#pragma unroll
+                    for (int mt = 0; mt < FZ_QMT; ++mt) a[mt][ks] = zofs[mt][ks] >= 0 ? __ldg(zq + zofs[mt][ks]) : 0.0;
                 }
 #pragma unroll
                 for (int mt = 0; mt < FZ_QMT; ++mt) {
                     if (mt >= MT) break;
-                    const int m = mt * 8 + g, vv = m / n5, i5 = m - vv * n5;
-                    double* dst = Qs + (vv * W4p + r4) * LDQ + i5 * n4 + 2 * q;
+                    double* dst = Qs + qofs[mt] + r4 * LDQ;
 #pragma unroll
                     for (int nt = 0; nt < FZ_QNT; ++nt) {
                         if (nt >= NT4) break;
@@ -400,7 +448,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
 #pragma unroll
                         for (int ks = 0; ks < FZ_QKS; ++ks)
                             if (ks < KS45) fz_dmma(c0, c1, a[mt][ks], b[nt][ks]);
-                        if (m < rows) {
+                        if (qofs[mt] >= 0) {
                             const int j4 = nt * 8 + 2 * q;
                             if (j4 < n4) dst[nt * 8] = c0;
                             if (j4 + 1 < n4) dst[nt * 8 + 1] = c1;
@@ -409,7 +457,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
                 }
             }
         } else {
-            for (int r4 = warp; r4 < w4; r4 += FZ_QP_THREADS / 32) {
+            for (int r4 = g4lo + warp; r4 < g4hi; r4 += NW) {
                 const int q4 = lo4 + r4;
                 const double* zq = Zb + ((long)q4 * V + v0) * n5;
                 for (int nt = 0; nt < NT4; ++nt) {
@@ -418,7 +466,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
 #pragma unroll
                     for (int ks = 0; ks < 8; ++ks) {
                         const int b45 = 4 * ks + q;
-                        bf[ks] = (ks < KS45 && b45 < c45 && i4 < n4) ? __ldg(B4b + ((long)q4 * c45 + b45) * c2434 * n4 + i4) : 0.0;
+                        bf[ks] = (ks < KS45 && b45 < c45 && i4 < n4) ? __ldg(B4b + ((long)q4 * c45 + b45) * c2434n4 + i4) : 0.0;
                     }
                     for (int mt = 0; mt < MT; ++mt) {
                         const int m = mt * 8 + g;
@@ -427,7 +475,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
                         for (int ks = 0; ks < 8; ++ks) {
                             if (ks < KS45) {
                                 const int b45 = 4 * ks + q;
-                                const double av = (m < rows && b45 < c45) ? __ldg(zq + b45 * sZ + m) : 0.0;
+                                const double av = (m < rows && b45 < c45) ? __ldg(zq + (long)b45 * sZ + m) : 0.0;
                                 fz_dmma(c0, c1, av, bf[ks]);
                             }
                         }
@@ -444,31 +492,35 @@ __global__ void __launch_bounds__(FZ_QP_THREADS) k_fz_qp(const FzParams p)
         fz_cp_wait<0>();
         __syncthreads();
         if (v0 + VG < nxs) {                         // the next pass's rows of Z: into L1 under this pass's P phase
-            const int rows2 = min(VG, nxs - v0 - VG) * n5, lines = (rows2 * 8 + 127) / 128 + 1;
-            for (int e = tid; e < c45 * w4 * lines; e += FZ_QP_THREADS) {
-                const int ln = e % lines, r = e / lines, r4 = r % w4, b45 = r / w4;
-                const double* row = Zb + b45 * sZ + ((long)(lo4 + r4) * V + v0 + VG) * n5;
-                const int off = ln * 16 < rows2 ? ln * 16 : rows2 - 1;
-                fz_prefetch_l1(row + off);
+            const int rows2 = min(VG, nxs - v0 - VG) * n5;
+            for (int pr = tid; pr < c45 * w4; pr += FZ_QP_THREADS) {
+                const int b45 = pr / w4, r4 = pr - b45 * w4;
+                const double* row = Zb + (long)b45 * sZ + ((long)(lo4 + r4) * V + v0 + VG) * n5;
+                for (int off = 0; off < rows2; off += 16) fz_prefetch_l1(row + off);
+                fz_prefetch_l1(row + rows2 - 1);
             }
         }
         // ---- P phase: one A fragment feeds four column tiles (four independent accumulator chains) ----
         const int NTQ = (NT + 3) >> 2;
-        for (int task = warp; task < nv * MT3 * NTQ; task += FZ_QP_THREADS / 32) {
+        for (int task = warp; task < nv * MT3 * NTQ; task += NW) {
             const int ntq = task % NTQ, t2 = task / NTQ, mt3 = t2 % MT3, vv = t2 / MT3;
+            // rows k3 the triad (k3 l24 x) allows for this x
+            const int2 wx = fz_window(l24, x0 + 2 * (v0 + vv), P.two_k_base[1], P3);
+            const int rlo = max(wx.x, w3.x) - w3.x, rhi = wx.y > 0 ? min(wx.x + wx.y, w3.x + w3.y) - w3.x : 0;
+            if (mt3 * 8 >= rhi || mt3 * 8 + 8 <= rlo) continue;
             const double* ap = S3s + (vv * W3p + mt3 * 8 + g) * LDS3 + q;
             const double* bp = Qs + (vv * W4p + q) * LDQ + ntq * 32 + g;
             double c[4][2];
 #pragma unroll
             for (int j = 0; j < 4; ++j) c[j][0] = c[j][1] = 0.0;
-            for (int ks = 0; ks < W4r; ks += 4) {
+            for (int ks = k4a; ks < k4b; ks += 4) {
                 const double av = ap[ks];
 #pragma unroll
                 for (int j = 0; j < 4; ++j)
                     if (ntq * 4 + j < NT) fz_dmma(c[j][0], c[j][1], av, bp[ks * LDQ + 8 * j]);
             }
             const int r3 = mt3 * 8 + g;
-            if (r3 < w3.y) {
+            if (r3 >= rlo && r3 < rhi) {
                 double* dst = Pb + ((long)(w3.x + r3) * V + v0 + vv) * prow + ntq * 32 + 2 * q;
 #pragma unroll
                 for (int j = 0; j < 4; ++j)     // NP is even: n + 1 < NP whenever n < n54, and rows are 16-byte aligned
@@ -517,13 +569,16 @@ struct FzMapR {
         fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, p.a_lo + ac, p.box.lo[2] + b25, x0, nxs, xg0);
         const int2 win = p.win23[q3];
         const int* list = p.kl3 + (long)q3 * (1 + c34 * c35);
-        const int m0 = mt * BM, n0 = nt * BN, N = min(BN, win.y * n3 - n0), M = N > 0 ? min(BM, n54 - m0) : 0, K = list[0];
+        // the x for which the triad (k3 l24 x) of eq. (5) holds: the only rows of P that k_fz_qp wrote
+        const int2 vr = fz_vrange(P.two_j[J24] + 2 * (p.box.lo[1] + b24), P.two_k_base[1] + 2 * q3, x0, nxs);
+        const int m0 = mt * BM, n0 = nt * BN, N = min(BN, win.y * n3 - n0), K = list[0];
+        const int M = (N > 0 && vr.y > 0) ? min(BM, n54 - m0) : 0;
         if (threadIdx.x == 0) {
             h->M = M;
             h->N = N;
             h->K = K;
-            h->nsub = nxs;
-            const long slab = ((((long)ac * c24 + b24) * c25 + b25) * P3 + q3) * V;
+            h->nsub = vr.y;
+            const long slab = ((((long)ac * c24 + b24) * c25 + b25) * P3 + q3) * V + vr.x;
             h->baseA = slab * c34 * c35 * NP + m0;
             h->baseB = (long)q3 * c34 * c35 * c23 * n3 + (long)win.x * n3 + n0;
             h->baseC = ((slab * c23 + win.x) * n3 + n0) * NP + m0;
@@ -573,12 +628,19 @@ struct FzMapA {
         int x0, nxs, xg0;
         fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, p.box.lo[2] + b25, x0, nxs, xg0);
         const int m0 = mt * BM, n0 = nt * BN, M = min(BM, n2 - m0), N = min(BN, n345 - n0);
-        // k list in the order (k3, x, l23): prefix sums over k3 of (x count) * (l23 count)
+        // k list in the order (k3, x, l23): the x of each k3 (triad (k3 l24 x)), then prefix sums of (x count) * (l23 count)
+        const int l24 = P.two_j[J24] + 2 * (p.box.lo[1] + b24);
+        for (int q3 = threadIdx.x; q3 < P3; q3 += blockDim.x) {
+            const int2 vr = fz_vrange(l24, P.two_k_base[1] + 2 * q3, x0, nxs);
+            tmp[80 + q3] = vr.x;
+            tmp[160 + q3] = vr.y;
+        }
+        __syncthreads();
         if (threadIdx.x == 0) {
             int run = 0;
             for (int q3 = 0; q3 < P3; ++q3) {
                 tmp[q3] = run;
-                run += p.win23[q3].y * nxs;
+                run += p.win23[q3].y * tmp[160 + q3];
             }
             tmp[P3] = run;
             h->M = M;
@@ -601,9 +663,11 @@ struct FzMapA {
         }
         __syncthreads();
         for (int e = threadIdx.x; e < P3 * nxs; e += blockDim.x) {
-            const int q3 = e / nxs, v = e - q3 * nxs;
+            const int q3 = e / nxs, vi = e - q3 * nxs;
+            if (vi >= tmp[160 + q3]) continue;
+            const int v = tmp[80 + q3] + vi;
             const int2 win = p.win23[q3];
-            const int at = tmp[q3] + v * win.y;
+            const int at = tmp[q3] + vi * win.y;
             for (int b = 0; b < win.y; ++b) {
                 const int row = (q3 * V + v) * c23 + win.x + b;
                 offAk[at + b] = row * n2;
@@ -665,8 +729,8 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     int* offCm = offAm + BM;
     int* offBn = offCm + BM;
     int* offCn = offBn + BN;
-    int* tmp = offCn + BN;                           // 80 ints of scratch for the setup
-    int* offAk = tmp + 80;
+    int* tmp = offCn + BN;                           // 240 ints of scratch for the setup
+    int* offAk = tmp + 240;
     int* offBk = offAk + kcap;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
     const int wm = warp / WGN, wn = warp % WGN;
@@ -911,7 +975,7 @@ template <class Map, int WGM, int WGN, int TM, int TN>
 static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
 {
     constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8;
-    const size_t smem = sizeof(double) * FZ_STAGES * FZ_KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 80 + 2 * (size_t)kcap);
+    const size_t smem = sizeof(double) * FZ_STAGES * FZ_KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 240 + 2 * (size_t)kcap);
     if (smem > 226 * 1024) return SF_EARG;
     static size_t attr = 0;
     if (smem > attr) {
