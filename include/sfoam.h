@@ -126,6 +126,15 @@ long sf_launch_count(int reset);
  * [2] accumulation (step 6(iv) + normalisation).  Enabling timing makes the vertex calls synchronous. */
 int sf_set_timing(int on);
 int sf_last_stage_ms(double ms[3]);
+/* Factorised path only (sf_set_path): CUDA-event times of its kernels, summed over the launches of the last vertex call made
+ * with sf_set_timing(1): ms[0] k_fz_qp (sums over l45 and k4), ms[1] k_fz_gemm<FzMapR> (sum over l34 l35, edge-3 product),
+ * ms[2] k_fz_gemm<FzMapA> (sum over x, k3, l23, edge-2 product), ms[3] the precomputations (Z, weighted boosters, G). */
+int sf_last_kernel_ms(double ms[4]);
+/* sf_set_counting(1): the factorised kernels count the FP64 MMA instructions (DMMA.8x8x4, 512 flop each) they issue, padding
+ * included; sf_last_dmma returns the counts of the last vertex call, same order as ms[0..2] above.  Measurement only: the
+ * call becomes synchronous and slightly slower; the result is unchanged. */
+int sf_set_counting(int on);
+int sf_last_dmma(double n[3]);
 
 /* Path selection for steps 5-7.  All paths compute the same sum of eq. (3); they differ in the
  * order of the additions only.

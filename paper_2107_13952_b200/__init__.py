@@ -119,6 +119,26 @@ def sf_last_stage_ms():
     return list(ms)
 
 
+def sf_last_kernel_ms():
+    """Factorised path: event times (ms) of [k_fz_qp, k_fz_gemm<FzMapR>, k_fz_gemm<FzMapA>, precomputations] of the last
+    vertex call made with sf_set_timing(True)."""
+    ms = (ctypes.c_double * 4)()
+    _check(_lib().sf_last_kernel_ms(ms), "sf_last_kernel_ms")
+    return list(ms)
+
+
+def sf_set_counting(on):
+    _check(_lib().sf_set_counting(int(bool(on))), "sf_set_counting")
+
+
+def sf_last_dmma():
+    """Factorised path: DMMA.8x8x4 warp instructions issued by [k_fz_qp, k_fz_gemm<FzMapR>, k_fz_gemm<FzMapA>] in the last
+    vertex call made with sf_set_counting(True)."""
+    n = (ctypes.c_double * 3)()
+    _check(_lib().sf_last_dmma(n), "sf_last_dmma")
+    return list(n)
+
+
 def sf_set_path(path):
     """0 = automatic, 1 = staged (general sizes), 2 = first fused on-chip path, 3 = line path (on-chip, register
     accumulation over lines of shells); 2 and 3 raise SF_EARG at call time for shapes they do not hold."""

@@ -19,6 +19,7 @@ struct SfContext {
     int path = 0;          // 0 auto, 1 staged, 2 fused
     int last_path = 0;
     bool timing = false;
+    bool counting = false;
     cudaEvent_t ev[4] = {};
     double stage_ms[3] = {};
 };
@@ -46,6 +47,9 @@ void* sf_scratch(int slot, size_t bytes)
     g_ctx.scratch_bytes[slot] = bytes;
     return p;
 }
+
+bool sf_timing_on(void) { return g_ctx.timing; }
+bool sf_counting_on(void) { return g_ctx.counting; }
 
 void sf_timing_mark(int idx, cudaStream_t st)
 {
@@ -120,6 +124,11 @@ extern "C" long sf_launch_count(int reset)
 extern "C" int sf_set_timing(int on)
 {
     g_ctx.timing = on != 0;
+    return SF_OK;
+}
+extern "C" int sf_set_counting(int on)
+{
+    g_ctx.counting = on != 0;
     return SF_OK;
 }
 extern "C" int sf_last_stage_ms(double ms[3])

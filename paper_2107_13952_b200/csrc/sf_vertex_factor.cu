@@ -62,6 +62,7 @@ struct FzParams {
     double* Rq;                 // [ac][b24][b25][q3][v][b23][i3][NP]
     double* Apart;              // [part][a1][i2][i3][i4][i5]
     long part0;                 // first partial tensor of this box
+    unsigned long long* cnt;    // measurement only (sf_set_counting): DMMA instructions issued by k_fz_qp, R, A'; else null
 };
 
 // window (lo, cnt) of q = (k - k_base) / 2 inside [0, n_pad) allowed by the triangle |a - b| <= k <= a + b
@@ -386,6 +387,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p)
             bofs[nt][ks] = (ks < KS45 && b45 < c45 && nt < NT4 && i4 < n4) ? b45 * c2434n4 + i4 : -1;
         }
 
+    unsigned ndm = 0;                                // DMMA instructions of this warp (reported when p.cnt is set)
     for (int v0 = 0; v0 < nxs; v0 += VG) {
         const int nv = min(VG, nxs - v0), rows = nv * n5, MT = (rows + 7) >> 3;
         // k4 of this pass: union over its x of the triad (k4 l35 x), inside the item's window
@@ -429,6 +431,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p)
                 const int q4 = lo4 + r4;
                 const double* zq = Zb + ((long)q4 * V + v0) * n5;
                 const double* bq = B4b + (long)q4 * c45 * c2434n4;
+                ndm += MT * NT4 * KS45;
                 double a[FZ_QMT][FZ_QKS], b[FZ_QNT][FZ_QKS];
 #pragma unroll
                 for (int ks = 0; ks < FZ_QKS; ++ks) {
@@ -460,6 +463,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p)
             for (int r4 = g4lo + warp; r4 < g4hi; r4 += NW) {
                 const int q4 = lo4 + r4;
                 const double* zq = Zb + ((long)q4 * V + v0) * n5;
+                ndm += MT * NT4 * KS45;
                 for (int nt = 0; nt < NT4; ++nt) {
                     const int i4 = nt * 8 + g;
                     double bf[8];
@@ -513,6 +517,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p)
             double c[4][2];
 #pragma unroll
             for (int j = 0; j < 4; ++j) c[j][0] = c[j][1] = 0.0;
+            ndm += ((k4b - k4a) >> 2) * min(4, NT - ntq * 4);
             for (int ks = k4a; ks < k4b; ks += 4) {
                 const double av = ap[ks];
 #pragma unroll
@@ -528,6 +533,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p)
             }
         }
     }
+    if (p.cnt && lane == 0) atomicAdd(p.cnt, (unsigned long long)ndm);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -543,7 +549,8 @@ struct FzGemmHdr {
 // rows m = (i5 i4), columns n = (l23 i3) over the l23 whose pair (j13 l23) allows k3; one item = (i1, l24, l25, k3, tile),
 // every x of (i1 l25) in turn
 struct FzMapR {
-    static constexpr bool A16 = true;    // rows of P start 16-byte aligned (NP even) and m runs contiguously: copy pairs
+    static constexpr bool A16 = true;
+    static constexpr int CNT = 1;    // rows of P start 16-byte aligned (NP even) and m runs contiguously: copy pairs
     static __device__ const double* srcA(const FzParams& p) { return p.Pq; }
     static __device__ const double* srcB(const FzParams& p) { return p.Bw3T; }
     static __device__ double* dstC(const FzParams& p) { return p.Rq; }
@@ -603,6 +610,7 @@ struct FzMapR {
 // A'[l24 l25; i1; i2; (i3 i4 i5)] = sum over (k3, x, l23) with k3 allowed by (j13 l23) of G[..][(k3 x l23)][i2] R[..][(k3 x l23)][(i3, i5 i4)]
 struct FzMapA {
     static constexpr bool A16 = false;
+    static constexpr int CNT = 2;
     static __device__ const double* srcA(const FzParams& p) { return p.G; }
     static __device__ const double* srcB(const FzParams& p) { return p.Rq; }
     static __device__ double* dstC(const FzParams& p) { return p.Apart; }
@@ -820,6 +828,7 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
 #pragma unroll
     for (int c = 0; c < FZ_STAGES - 1; ++c) load_chunk(c);
     int c_in = 0, sub = 0;
+    unsigned ndm = 0;                                // DMMA instructions of this warp (reported when p.cnt is set)
     for (int gc = 0; gc < total; ++gc) {
         fz_cp_wait<FZ_STAGES - 2>();
         __syncthreads();                             // chunk gc has landed; every warp is done with chunk gc - 1
@@ -829,6 +838,7 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
             const double* bs = Bs + (gc % FZ_STAGES) * FZ_KC * LDB + q * LDB + wn * TN * 8 + g;
             const int ksn = min(FZ_KC / 4, (K - c_in * FZ_KC + 3) >> 2);
             FzChunk<TM, TN, TN>::run(acc, as, bs, LDA, LDB, ksn, tma, tna);
+            ndm += tma * tna * ksn;
         }
         if (++c_in == nchunks) {
             store(sub);
@@ -837,6 +847,7 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
         }
     }
     fz_cp_wait<0>();
+    if (p.cnt && lane == 0) atomicAdd(p.cnt + Map::CNT, (unsigned long long)ndm);
 }
 
 // kernel (d): out[a1][i2][r] = prod_e sqrt(2 i_e + 1) * sum over the partial tensors, in order, of Apart[part][a1][i2][r]
@@ -991,7 +1002,43 @@ static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
     return SF_OK;
 }
 
-enum { FZ_SLOT_WIN = 24, FZ_SLOT_LIST, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART };
+// ---- measurement: per-kernel CUDA-event times (sf_set_timing) and issued DMMA instructions (sf_set_counting) ----
+#define FZ_MAX_EV 256
+static cudaEvent_t g_fz_ev[FZ_MAX_EV];
+static int g_fz_ev_made = 0, g_fz_ev_used = 0, g_fz_ev_class[FZ_MAX_EV / 2];
+static double g_fz_ms[4], g_fz_dmma[3];
+
+static void fz_ev_begin(int cls, cudaStream_t st)
+{
+    if (!sf_timing_on() || g_fz_ev_used + 2 > FZ_MAX_EV) return;
+    while (g_fz_ev_made < g_fz_ev_used + 2) cudaEventCreate(&g_fz_ev[g_fz_ev_made++]);
+    g_fz_ev_class[g_fz_ev_used / 2] = cls;
+    cudaEventRecord(g_fz_ev[g_fz_ev_used], st);
+}
+static void fz_ev_end(cudaStream_t st)
+{
+    if (!sf_timing_on() || g_fz_ev_used + 2 > FZ_MAX_EV) return;
+    cudaEventRecord(g_fz_ev[g_fz_ev_used + 1], st);
+    g_fz_ev_used += 2;
+}
+/* ms[0..3] = k_fz_qp, k_fz_gemm<FzMapR>, k_fz_gemm<FzMapA>, the precomputations: summed over the launches of the last
+ * factorised vertex call made with sf_set_timing(1) */
+extern "C" int sf_last_kernel_ms(double ms[4])
+{
+    if (!ms) return SF_EARG;
+    memcpy(ms, g_fz_ms, sizeof g_fz_ms);
+    return SF_OK;
+}
+/* n[0..2] = DMMA.8x8x4 warp instructions issued by k_fz_qp, k_fz_gemm<FzMapR>, k_fz_gemm<FzMapA> in the last factorised
+ * vertex call made with sf_set_counting(1) (512 flop each) */
+extern "C" int sf_last_dmma(double n[3])
+{
+    if (!n) return SF_EARG;
+    memcpy(n, g_fz_dmma, sizeof g_fz_dmma);
+    return SF_OK;
+}
+
+enum { FZ_SLOT_CNT = 23, FZ_SLOT_WIN = 24, FZ_SLOT_LIST, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART };
 
 int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st)
 {
@@ -1042,6 +1089,12 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     size_t free_b = 0, total_b = 0;
     if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return SF_ECUDA;
 
+    g_fz_ev_used = 0;
+    if (sf_counting_on()) {
+        p.cnt = (unsigned long long*)sf_scratch(FZ_SLOT_CNT, 3 * sizeof(unsigned long long));
+        if (!p.cnt) return SF_ENOMEM;
+        SF_CUDA_OK(cudaMemsetAsync(p.cnt, 0, 3 * sizeof(unsigned long long), st));
+    }
     long part0 = 0;
     for (int bi = 0; bi < nbox; ++bi) {
         const FzBox& bx = boxes[bi];
@@ -1089,6 +1142,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         p.Rq = Rq;
         p.a_lo = 0;
         p.a_cnt = n1;
+        fz_ev_begin(3, st);
         k_fz_z<<<(unsigned)(c25 * n1 * c35 * c45), 256, 0, st>>>(p, Z);
         k_fz_b4t<<<(unsigned)((nB4 + 255) / 256), 256, 0, st>>>(p, nB4, B4);
         k_fz_b3t<<<(unsigned)((nB3 + 255) / 256), 256, 0, st>>>(p, nB3, B3);
@@ -1096,14 +1150,21 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         k_fz_g<<<(unsigned)((nG + 255) / 256), 256, 0, st>>>(p, nG, G);
         k_fz_lists<<<P3, 32, 0, st>>>(p, (int2*)lists, lists + 2 * P3);
         sf_count_launch(6);
+        fz_ev_end(st);
         for (int a_lo = 0; a_lo < n1; a_lo += (int)na) {
             p.a_lo = a_lo;
             p.a_cnt = (int)(a_lo + na <= n1 ? na : n1 - a_lo);
+            fz_ev_begin(0, st);
             k_fz_qp<<<(unsigned)((long)p.a_cnt * c25 * c35 * c24 * c34), FZ_QP_THREADS, sh.qp_smem, st>>>(p);
             sf_count_launch(1);
+            fz_ev_end(st);
+            fz_ev_begin(1, st);
             int rc = fz_launch_gemm<FzMapR, 8, 1, 2, 8>(p, (int)(c34 * c35), st);
+            fz_ev_end(st);
             if (rc != SF_OK) return rc;
+            fz_ev_begin(2, st);
             rc = fz_launch_gemm<FzMapA, 1, 8, 2, 4>(p, (int)(P3 * sh.V * c23), st);
+            fz_ev_end(st);
             if (rc != SF_OK) return rc;
         }
         part0 += c24 * c25;
@@ -1111,5 +1172,20 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     sf_timing_mark(2, st);
     k_fz_reduce<<<(unsigned)((D.n_out + 255) / 256), 256, 0, st>>>(P, parts, D.n_out, Apart, out);
     sf_count_launch(1);
-    return cudaGetLastError() == cudaSuccess ? SF_OK : SF_ECUDA;
+    if (cudaGetLastError() != cudaSuccess) return SF_ECUDA;
+    if (sf_timing_on() || sf_counting_on()) {        // measurement modes make the call synchronous
+        SF_CUDA_OK(cudaStreamSynchronize(st));
+        memset(g_fz_ms, 0, sizeof g_fz_ms);
+        for (int e = 0; e + 1 < g_fz_ev_used; e += 2) {
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, g_fz_ev[e], g_fz_ev[e + 1]);
+            g_fz_ms[g_fz_ev_class[e / 2]] += ms;
+        }
+        if (p.cnt) {
+            unsigned long long h[3];
+            SF_CUDA_OK(cudaMemcpy(h, p.cnt, sizeof h, cudaMemcpyDeviceToHost));
+            for (int k = 0; k < 3; ++k) g_fz_dmma[k] = (double)h[k];
+        }
+    }
+    return SF_OK;
 }
