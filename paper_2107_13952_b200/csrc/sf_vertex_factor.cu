@@ -550,7 +550,7 @@ struct FzGemmHdr {
 // every x of (i1 l25) in turn
 struct FzMapR {
     static constexpr bool A16 = true;
-    static constexpr int CNT = 1;    // rows of P start 16-byte aligned (NP even) and m runs contiguously: copy pairs
+    static constexpr int CNT = 1, KC = 32, ST = 2;    // rows of P start 16-byte aligned (NP even) and m runs contiguously: copy pairs
     static __device__ const double* srcA(const FzParams& p) { return p.Pq; }
     static __device__ const double* srcB(const FzParams& p) { return p.Bw3T; }
     static __device__ double* dstC(const FzParams& p) { return p.Rq; }
@@ -610,7 +610,7 @@ struct FzMapR {
 // A'[l24 l25; i1; i2; (i3 i4 i5)] = sum over (k3, x, l23) with k3 allowed by (j13 l23) of G[..][(k3 x l23)][i2] R[..][(k3 x l23)][(i3, i5 i4)]
 struct FzMapA {
     static constexpr bool A16 = false;
-    static constexpr int CNT = 2;
+    static constexpr int CNT = 2, KC = 16, ST = 3;
     static __device__ const double* srcA(const FzParams& p) { return p.G; }
     static __device__ const double* srcB(const FzParams& p) { return p.Rq; }
     static __device__ double* dstC(const FzParams& p) { return p.Apart; }
@@ -685,15 +685,13 @@ struct FzMapA {
     }
 };
 
-#define FZ_KC 16
-#define FZ_STAGES 3
 // one k-chunk of a warp tile with TNA live column tiles (tiles beyond N are skipped, not multiplied by zeros)
-template <int TM, int TN, int TNA>
+template <int TM, int TN, int TNA, int KC>
 __device__ __forceinline__ void fz_chunk(double (&acc)[TM][TN][2], const double* as, const double* bs, int LDA, int LDB,
                                          int ksn, int tma)
 {
 #pragma unroll
-    for (int ks = 0; ks < FZ_KC / 4; ++ks) {
+    for (int ks = 0; ks < KC / 4; ++ks) {
         if (ks < ksn) {
             double a[TM], b[TNA];
 #pragma unroll
@@ -710,30 +708,31 @@ __device__ __forceinline__ void fz_chunk(double (&acc)[TM][TN][2], const double*
         }
     }
 }
-template <int TM, int TN, int TNA>
+template <int TM, int TN, int TNA, int KC>
 struct FzChunk {
     static __device__ __forceinline__ void run(double (&acc)[TM][TN][2], const double* as, const double* bs, int LDA,
                                                int LDB, int ksn, int tma, int tna)
     {
         if (tna == TNA)
-            fz_chunk<TM, TN, TNA>(acc, as, bs, LDA, LDB, ksn, tma);
+            fz_chunk<TM, TN, TNA, KC>(acc, as, bs, LDA, LDB, ksn, tma);
         else
-            FzChunk<TM, TN, TNA - 1>::run(acc, as, bs, LDA, LDB, ksn, tma, tna);
+            FzChunk<TM, TN, TNA - 1, KC>::run(acc, as, bs, LDA, LDB, ksn, tma, tna);
     }
 };
-template <int TM, int TN>
-struct FzChunk<TM, TN, 0> {
+template <int TM, int TN, int KC>
+struct FzChunk<TM, TN, 0, KC> {
     static __device__ __forceinline__ void run(double (&)[TM][TN][2], const double*, const double*, int, int, int, int, int) {}
 };
 template <class Map, int WGM, int WGN, int TM, int TN>
 __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int kcap)
 {
     constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8, NTH = WGM * WGN * 32, LDA = BM + 8, LDB = BN + 8;
+    constexpr int KC = Map::KC, ST = Map::ST;        // k-chunk depth and ring stages
     extern __shared__ __align__(16) double smem[];
     __shared__ FzGemmHdr hdr;
-    double* As = smem;                               // [FZ_STAGES][FZ_KC][LDA], [k][m]
-    double* Bs = As + FZ_STAGES * FZ_KC * LDA;       // [FZ_STAGES][FZ_KC][LDB], [k][n]
-    int* offAm = (int*)(Bs + FZ_STAGES * FZ_KC * LDB);
+    double* As = smem;                               // [ST][KC][LDA], [k][m]
+    double* Bs = As + ST * KC * LDA;       // [ST][KC][LDB], [k][n]
+    int* offAm = (int*)(Bs + ST * KC * LDB);
     int* offCm = offAm + BM;
     int* offBn = offCm + BM;
     int* offCn = offBn + BN;
@@ -752,7 +751,7 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     const double* B = B0 + hdr.baseB;
     double* C = Map::dstC(p) + hdr.baseC;
     const long sA = hdr.sA, sB = hdr.sB, sC = hdr.sC;
-    const int nchunks = (K + FZ_KC - 1) / FZ_KC, total = nsub * nchunks;
+    const int nchunks = (K + KC - 1) / KC, total = nsub * nchunks;
     int tma = 0, tna = 0;                            // live 8-row / 8-column tiles of this warp
 #pragma unroll
     for (int i = 0; i < TM; ++i) tma += (wm * TM + i) * 8 < M;
@@ -790,23 +789,23 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     }
     int l_sub = 0, l_c = 0;                          // next chunk to request: product l_sub, chunk l_c of it
     // every thread copies the same m (pair of m) and n of each k-row it serves: offsets and bounds are fixed per item
-    constexpr int AW = Map::A16 ? 2 : 1, ATPR = BM / AW, ARPP = NTH / ATPR, APASS = FZ_KC / ARPP;
-    constexpr int BTPR = BN, BRPP = NTH / BTPR, BPASS = FZ_KC / BRPP;
-    static_assert(NTH % ATPR == 0 && FZ_KC % ARPP == 0 && NTH % BTPR == 0 && FZ_KC % BRPP == 0, "loader shape");
+    constexpr int AW = Map::A16 ? 2 : 1, ATPR = BM / AW, ARPP = NTH / ATPR, APASS = KC / ARPP;
+    constexpr int BTPR = BN, BRPP = NTH / BTPR, BPASS = KC / BRPP;
+    static_assert(NTH % ATPR == 0 && KC % ARPP == 0 && NTH % BTPR == 0 && KC % BRPP == 0, "loader shape");
     const int am = (tid % ATPR) * AW, akr = tid / ATPR, bn = tid % BTPR, bkr = tid / BTPR;
     const int a_bytes = 8 * max(0, min(AW, M - am)), b_bytes = bn < N ? 8 : 0;
     const int a_off = a_bytes ? offAm[am] : 0, b_off = b_bytes ? offBn[bn] : 0;
     const unsigned a_dst = fz_smem_u32(As + akr * LDA + am), b_dst = fz_smem_u32(Bs + bkr * LDB + bn);
     auto load_chunk = [&](int gc) {
         if (gc < total) {
-            const int s = gc % FZ_STAGES, k0 = l_c * FZ_KC;
+            const int s = gc % ST, k0 = l_c * KC;
             const double* Aq = A + l_sub * sA + a_off;
             const double* Bq = B + l_sub * sB + b_off;
 #pragma unroll
             for (int it = 0; it < APASS; ++it) {
                 const int kr = akr + it * ARPP, k = k0 + kr;
                 const bool ok = a_bytes && k < K;
-                const unsigned dst = a_dst + 8u * (unsigned)((s * FZ_KC + it * ARPP) * LDA);
+                const unsigned dst = a_dst + 8u * (unsigned)((s * KC + it * ARPP) * LDA);
                 if (Map::A16)
                     fz_cp_async16(dst, ok ? Aq + offAk[k] : A0, ok ? a_bytes : 0);
                 else
@@ -816,7 +815,7 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
             for (int it = 0; it < BPASS; ++it) {
                 const int kr = bkr + it * BRPP, k = k0 + kr;
                 const bool ok = b_bytes && k < K;
-                fz_cp_async8(b_dst + 8u * (unsigned)((s * FZ_KC + it * BRPP) * LDB), ok ? Bq + offBk[k] : B0, ok ? 8 : 0);
+                fz_cp_async8(b_dst + 8u * (unsigned)((s * KC + it * BRPP) * LDB), ok ? Bq + offBk[k] : B0, ok ? 8 : 0);
             }
             if (++l_c == nchunks) {
                 l_c = 0;
@@ -826,18 +825,18 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
         fz_cp_commit();
     };
 #pragma unroll
-    for (int c = 0; c < FZ_STAGES - 1; ++c) load_chunk(c);
+    for (int c = 0; c < ST - 1; ++c) load_chunk(c);
     int c_in = 0, sub = 0;
     unsigned ndm = 0;                                // DMMA instructions of this warp (reported when p.cnt is set)
     for (int gc = 0; gc < total; ++gc) {
-        fz_cp_wait<FZ_STAGES - 2>();
+        fz_cp_wait<ST - 2>();
         __syncthreads();                             // chunk gc has landed; every warp is done with chunk gc - 1
-        load_chunk(gc + FZ_STAGES - 1);              // refills the stage chunk gc - 1 used
+        load_chunk(gc + ST - 1);              // refills the stage chunk gc - 1 used
         if (active) {
-            const double* as = As + (gc % FZ_STAGES) * FZ_KC * LDA + q * LDA + wm * TM * 8 + g;
-            const double* bs = Bs + (gc % FZ_STAGES) * FZ_KC * LDB + q * LDB + wn * TN * 8 + g;
-            const int ksn = min(FZ_KC / 4, (K - c_in * FZ_KC + 3) >> 2);
-            FzChunk<TM, TN, TN>::run(acc, as, bs, LDA, LDB, ksn, tma, tna);
+            const double* as = As + (gc % ST) * KC * LDA + q * LDA + wm * TM * 8 + g;
+            const double* bs = Bs + (gc % ST) * KC * LDB + q * LDB + wn * TN * 8 + g;
+            const int ksn = min(KC / 4, (K - c_in * KC + 3) >> 2);
+            FzChunk<TM, TN, TN, KC>::run(acc, as, bs, LDA, LDB, ksn, tma, tna);
             ndm += tma * tna * ksn;
         }
         if (++c_in == nchunks) {
@@ -986,7 +985,7 @@ template <class Map, int WGM, int WGN, int TM, int TN>
 static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
 {
     constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8;
-    const size_t smem = sizeof(double) * FZ_STAGES * FZ_KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 240 + 2 * (size_t)kcap);
+    const size_t smem = sizeof(double) * Map::ST * Map::KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 240 + 2 * (size_t)kcap);
     if (smem > 226 * 1024) return SF_EARG;
     static size_t attr = 0;
     if (smem > attr) {
