@@ -332,14 +332,16 @@ __global__ void __launch_bounds__(32) k_fz_lists(FzParams p, int2* __restrict__ 
 // k_fz_qp: Q = sum_l45 Z Bw4 and P = sum_k4 S3 Q for one (i1, l25, l35, l24, l34), a few x at a time
 // ---------------------------------------------------------------------------------------------------------
 // Q phase, per k4:  C[(v i5)][i4] = sum_l45 Z[l45][k4][(v i5)] Bw4T[k4][l45][i4]        (A and B fragments straight from L1/L2)
-// P phase, per v:   P[k3][(i5 i4)] = sum_k4 S3[k3][k4] Q[k4][(i5 i4)]                   (both operands in shared memory)
+// P phase, per v:   P[k3][(i5 i4)] = sum_k4 S3[k3][k4] Q[k4][(i5 i4)]                   (S3 from L1/L2, Q from shared memory)
+// Persistent: a CTA walks the items with stride gridDim.x; its fragment offsets are computed once.
 // The triads of eq. (5) that contain x, (k4 l35 x) and (k3 l24 x), bound k4 and k3 for every x: only those k4 are
 // computed and only those rows k3 of P are written (k_fz_gemm reads exactly the same set, fz_vrange).
 #define FZ_QP_THREADS 256
 #define FZ_QKS 3      /* fast Q phase: c45 <= 12, n4 <= 16, (v, i5) rows of a pass <= 32 */
 #define FZ_QNT 2
 #define FZ_QMT 4
-__global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p)
+#define FZ_PKS 6      /* fast P phase: k4 windows of at most 24 values */
+__global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, long n_items)
 {
     extern __shared__ __align__(16) double smem[];
     constexpr int NW = FZ_QP_THREADS / 32;
@@ -348,188 +350,204 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p)
     const int nl = P.nl, n1 = P.n_i[0], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5;
     const int P3 = P.n_k_pad[1], P4 = P.n_k_pad[2], NX = P.n_x_pad, V = p.V, NP = p.NP;
     const int c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4], c45 = p.box.cnt[5];
-    const int W3p = p.W3p, W4p = p.W4p, LDQ = p.LDQ, LDS3 = p.LDS3, VG = p.VG;
-    long it = blockIdx.x;
-    const int b34 = (int)(it % c34); it /= c34;
-    const int b24 = (int)(it % c24); it /= c24;
-    const int b35 = (int)(it % c35); it /= c35;
-    const int b25 = (int)(it % c25);
-    const int ac = (int)(it / c25);
-    const int a1 = p.a_lo + ac;
-    const int o24 = p.box.lo[1] + b24, o25 = p.box.lo[2] + b25, o34 = p.box.lo[3] + b34, o35 = p.box.lo[4] + b35;
-    const int l24 = P.two_j[J24] + 2 * o24, l35 = P.two_j[J35] + 2 * o35;
-    int x0, nxs, xg0;
-    fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
-    const int2 w3 = p.w3A[o34 * nl + o35];           // the k3 the pair (l34 l35) allows
-    if (w3.y == 0) return;
-    const int2 w4a = p.w4A[o24 * nl + o34];
-    const int lo4 = max(w4a.x, p.hull4B.x);
-    const int w4 = max(0, min(w4a.x + w4a.y, p.hull4B.y) - lo4);
-    double* Qs = smem;                               // [VG][W4p][LDQ]
-    double* S3s = smem + VG * W4p * LDQ;             // [VG][W3p][LDS3]
-    for (int z = tid; z < VG * W4p * LDQ; z += FZ_QP_THREADS) Qs[z] = 0.0;   // rows never written must stay finite
-    const int MT3 = (w3.y + 7) >> 3, NT = (n54 + 7) >> 3, NT4 = (n4 + 7) >> 3, KS45 = (c45 + 3) >> 2;
-    const int sZ = P4 * V * n5;
-    const double* Zb = p.Z + ((((long)b25 * n1 + a1) * c35 + b35) * c45) * (long)sZ;
-    const double* S3b = p.S3T + ((((long)b24 * c34 + b34) * c35 + b35) * NX + xg0) * (long)(P3 * P4);
-    const int c2434n4 = c24 * c34 * n4;
-    const double* B4b = p.Bw4T + ((long)b24 * c34 + b34) * n4;
+    const int W4p = p.W4p, LDQ = p.LDQ, VG = p.VG;
+    const int NT = (n54 + 7) >> 3, NT4 = (n4 + 7) >> 3, KS45 = (c45 + 3) >> 2, NTQ = (NT + 3) >> 2;
+    const int sZ = P4 * V * n5, c2434n4 = c24 * c34 * n4;
     const long prow = (long)c34 * c35 * NP;          // stride of v in P
-    double* Pb = p.Pq + ((((long)ac * c24 + b24) * c25 + b25) * P3) * V * prow + ((long)b34 * c35 + b35) * NP;
-    const bool fast = KS45 <= FZ_QKS && NT4 <= FZ_QNT && ((VG * n5 + 7) >> 3) <= FZ_QMT;
-    // item constants of the fast Q phase: offsets of this lane's B fragments inside one k4 block of Bw4T (-1: zero)
-    int bofs[FZ_QNT][FZ_QKS];
+    const bool fastq = KS45 <= FZ_QKS && NT4 <= FZ_QNT && ((VG * n5 + 7) >> 3) <= FZ_QMT;
+    const bool fastp = W4p <= 4 * FZ_PKS;
+    double* Qs = smem;                               // [VG][W4p][LDQ]
+    for (int z = tid; z < VG * W4p * LDQ; z += FZ_QP_THREADS) Qs[z] = 0.0;   // rows never written must stay finite
+    // constants of the CTA: this lane's fragment offsets inside one k4 block of Bw4T / of Z, its C rows in Qs (-1: none)
+    int bofs[FZ_QNT][FZ_QKS], zofs[FZ_QMT][FZ_QKS], qrow[FZ_QMT];
 #pragma unroll
-    for (int nt = 0; nt < FZ_QNT; ++nt)
+    for (int ks = 0; ks < FZ_QKS; ++ks) {
+        const int b45 = 4 * ks + q;
+        const bool kin = ks < KS45 && b45 < c45;
 #pragma unroll
-        for (int ks = 0; ks < FZ_QKS; ++ks) {
-            const int b45 = 4 * ks + q, i4 = nt * 8 + g;
-            bofs[nt][ks] = (ks < KS45 && b45 < c45 && nt < NT4 && i4 < n4) ? b45 * c2434n4 + i4 : -1;
+        for (int nt = 0; nt < FZ_QNT; ++nt) {
+            const int i4 = nt * 8 + g;
+            bofs[nt][ks] = (kin && nt < NT4 && i4 < n4) ? b45 * c2434n4 + i4 : -1;
         }
-
+#pragma unroll
+        for (int mt = 0; mt < FZ_QMT; ++mt) zofs[mt][ks] = kin ? b45 * sZ + mt * 8 + g : -1;
+    }
+#pragma unroll
+    for (int mt = 0; mt < FZ_QMT; ++mt) {
+        const int m = mt * 8 + g, vv = m / n5, i5 = m - vv * n5;
+        qrow[mt] = vv * W4p * LDQ + i5 * n4 + 2 * q;
+    }
     unsigned ndm = 0;                                // DMMA instructions of this warp (reported when p.cnt is set)
-    for (int v0 = 0; v0 < nxs; v0 += VG) {
-        const int nv = min(VG, nxs - v0), rows = nv * n5, MT = (rows + 7) >> 3;
-        // k4 of this pass: union over its x of the triad (k4 l35 x), inside the item's window
-        int g4lo = w4, g4hi = 0;
-        for (int vv = 0; vv < nv; ++vv) {
-            const int2 w = fz_window(l35, x0 + 2 * (v0 + vv), P.two_k_base[2], P4);
-            const int lo = max(w.x, lo4) - lo4, hi = min(w.x + w.y, lo4 + w4) - lo4;
-            if (w.y > 0 && hi > lo) {
-                g4lo = min(g4lo, lo);
-                g4hi = max(g4hi, hi);
-            }
-        }
-        if (g4hi <= g4lo) g4lo = g4hi = 0;
-        const int k4a = g4lo & ~3, k4b = (g4hi + 3) & ~3;
-        __syncthreads();                             // the previous P phase has read Qs and S3s
-        for (int row = warp; row < nv * W3p; row += NW) {                 // lands under the Q phase
-            const int vv = row / W3p, r3 = row - vv * W3p;
-            const double* src = S3b + ((long)(v0 + vv) * P3 + w3.x + r3) * P4 + lo4;
-            for (int r4 = lane; r4 < W4p; r4 += 32) {
-                const bool ok = r3 < w3.y && r4 < w4;
-                fz_cp_async8(fz_smem_u32(S3s + row * LDS3 + r4), ok ? src + r4 : S3b, ok ? 8 : 0);
-            }
-        }
-        fz_cp_commit();
-        // ---- Q phase ----
-        if (fast) {
-            // common sizes: every fragment of a k4 is requested before the first MMA, so one round of L2 latency per k4
-            int zofs[FZ_QMT][FZ_QKS], qofs[FZ_QMT];
-#pragma unroll
-            for (int mt = 0; mt < FZ_QMT; ++mt) {
-                const int m = mt * 8 + g, vv = m / n5, i5 = m - vv * n5;
-                const bool okm = mt < MT && m < rows;
-                qofs[mt] = okm ? vv * W4p * LDQ + i5 * n4 + 2 * q : -1;
-#pragma unroll
-                for (int ks = 0; ks < FZ_QKS; ++ks) {
-                    const int b45 = 4 * ks + q;
-                    zofs[mt][ks] = (okm && ks < KS45 && b45 < c45) ? b45 * sZ + m : -1;
+
+    for (long item = blockIdx.x; item < n_items; item += gridDim.x) {
+        long it = item;
+        const int b34 = (int)(it % c34); it /= c34;
+        const int b24 = (int)(it % c24); it /= c24;
+        const int b35 = (int)(it % c35); it /= c35;
+        const int b25 = (int)(it % c25);
+        const int ac = (int)(it / c25);
+        const int a1 = p.a_lo + ac;
+        const int o24 = p.box.lo[1] + b24, o25 = p.box.lo[2] + b25, o34 = p.box.lo[3] + b34, o35 = p.box.lo[4] + b35;
+        const int l24 = P.two_j[J24] + 2 * o24, l35 = P.two_j[J35] + 2 * o35;
+        int x0, nxs, xg0;
+        fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
+        const int2 w3 = p.w3A[o34 * nl + o35];       // the k3 the pair (l34 l35) allows
+        if (w3.y == 0) continue;
+        const int2 w4a = p.w4A[o24 * nl + o34];
+        const int lo4 = max(w4a.x, p.hull4B.x);
+        const int w4 = max(0, min(w4a.x + w4a.y, p.hull4B.y) - lo4);
+        const int MT3 = (w3.y + 7) >> 3;
+        const double* Zb = p.Z + ((((long)b25 * n1 + a1) * c35 + b35) * c45) * (long)sZ;
+        const double* S3b = p.S3T + ((((long)b24 * c34 + b34) * c35 + b35) * NX + xg0) * (long)(P3 * P4) + (long)w3.x * P4 + lo4;
+        const double* B4b = p.Bw4T + ((long)b24 * c34 + b34) * n4;
+        double* Pb = p.Pq + ((((long)ac * c24 + b24) * c25 + b25) * P3) * V * prow + ((long)b34 * c35 + b35) * NP;
+
+        for (int v0 = 0; v0 < nxs; v0 += VG) {
+            const int nv = min(VG, nxs - v0), rows = nv * n5, MT = (rows + 7) >> 3;
+            // k4 of this pass: union over its x of the triad (k4 l35 x), inside the item's window
+            int g4lo = w4, g4hi = 0;
+            for (int vv = 0; vv < nv; ++vv) {
+                const int2 w = fz_window(l35, x0 + 2 * (v0 + vv), P.two_k_base[2], P4);
+                const int lo = max(w.x, lo4) - lo4, hi = min(w.x + w.y, lo4 + w4) - lo4;
+                if (w.y > 0 && hi > lo) {
+                    g4lo = min(g4lo, lo);
+                    g4hi = max(g4hi, hi);
                 }
             }
-            for (int r4 = g4lo + warp; r4 < g4hi; r4 += NW) {
-                const int q4 = lo4 + r4;
-                const double* zq = Zb + ((long)q4 * V + v0) * n5;
-                const double* bq = B4b + (long)q4 * c45 * c2434n4;
-                ndm += MT * NT4 * KS45;
-                double a[FZ_QMT][FZ_QKS], b[FZ_QNT][FZ_QKS];
+            if (g4hi <= g4lo) g4lo = g4hi = 0;
+            const int k4a = g4lo & ~3, k4b = (g4hi + 3) & ~3;
+            __syncthreads();                         // the previous P phase has read Qs
+            // ---- Q phase ----
+            if (fastq) {
+                // common sizes: every fragment of a k4 is requested before the first MMA: one round of latency per k4
+                for (int r4 = g4lo + warp; r4 < g4hi; r4 += NW) {
+                    const int q4 = lo4 + r4;
+                    const double* zq = Zb + ((long)q4 * V + v0) * n5;
+                    const double* bq = B4b + (long)q4 * c45 * c2434n4;
+                    ndm += MT * NT4 * KS45;
+                    double a[FZ_QMT][FZ_QKS], b[FZ_QNT][FZ_QKS];
 #pragma unroll
-                for (int ks = 0; ks < FZ_QKS; ++ks) {
+                    for (int ks = 0; ks < FZ_QKS; ++ks) {
 #pragma unroll
-                    for (int nt = 0; nt < FZ_QNT; ++nt) b[nt][ks] = bofs[nt][ks] >= 0 ? __ldg(bq + bofs[nt][ks]) : 0.0;
+                        for (int nt = 0; nt < FZ_QNT; ++nt) b[nt][ks] = bofs[nt][ks] >= 0 ? __ldg(bq + bofs[nt][ks]) : 0.0;
 #pragma unroll
-                    for (int mt = 0; mt < FZ_QMT; ++mt) a[mt][ks] = zofs[mt][ks] >= 0 ? __ldg(zq + zofs[mt][ks]) : 0.0;
-                }
+                        for (int mt = 0; mt < FZ_QMT; ++mt)
+                            a[mt][ks] = (zofs[mt][ks] >= 0 && mt * 8 + g < rows) ? __ldg(zq + zofs[mt][ks]) : 0.0;
+                    }
 #pragma unroll
-                for (int mt = 0; mt < FZ_QMT; ++mt) {
-                    if (mt >= MT) break;
-                    double* dst = Qs + qofs[mt] + r4 * LDQ;
+                    for (int mt = 0; mt < FZ_QMT; ++mt) {
+                        if (mt >= MT) break;
+                        double* dst = Qs + qrow[mt] + r4 * LDQ;
+                        const bool okm = mt * 8 + g < rows;
 #pragma unroll
-                    for (int nt = 0; nt < FZ_QNT; ++nt) {
-                        if (nt >= NT4) break;
-                        double c0 = 0.0, c1 = 0.0;
+                        for (int nt = 0; nt < FZ_QNT; ++nt) {
+                            if (nt >= NT4) break;
+                            double c0 = 0.0, c1 = 0.0;
 #pragma unroll
-                        for (int ks = 0; ks < FZ_QKS; ++ks)
-                            if (ks < KS45) fz_dmma(c0, c1, a[mt][ks], b[nt][ks]);
-                        if (qofs[mt] >= 0) {
+                            for (int ks = 0; ks < FZ_QKS; ++ks)
+                                if (ks < KS45) fz_dmma(c0, c1, a[mt][ks], b[nt][ks]);
                             const int j4 = nt * 8 + 2 * q;
-                            if (j4 < n4) dst[nt * 8] = c0;
-                            if (j4 + 1 < n4) dst[nt * 8 + 1] = c1;
+                            if (okm && j4 < n4) dst[nt * 8] = c0;
+                            if (okm && j4 + 1 < n4) dst[nt * 8 + 1] = c1;
                         }
                     }
                 }
-            }
-        } else {
-            for (int r4 = g4lo + warp; r4 < g4hi; r4 += NW) {
-                const int q4 = lo4 + r4;
-                const double* zq = Zb + ((long)q4 * V + v0) * n5;
-                ndm += MT * NT4 * KS45;
-                for (int nt = 0; nt < NT4; ++nt) {
-                    const int i4 = nt * 8 + g;
-                    double bf[8];
-#pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) {
-                        const int b45 = 4 * ks + q;
-                        bf[ks] = (ks < KS45 && b45 < c45 && i4 < n4) ? __ldg(B4b + ((long)q4 * c45 + b45) * c2434n4 + i4) : 0.0;
-                    }
-                    for (int mt = 0; mt < MT; ++mt) {
-                        const int m = mt * 8 + g;
-                        double c0 = 0.0, c1 = 0.0;
+            } else {
+                for (int r4 = g4lo + warp; r4 < g4hi; r4 += NW) {
+                    const int q4 = lo4 + r4;
+                    const double* zq = Zb + ((long)q4 * V + v0) * n5;
+                    ndm += MT * NT4 * KS45;
+                    for (int nt = 0; nt < NT4; ++nt) {
+                        const int i4 = nt * 8 + g;
+                        double bf[8];
 #pragma unroll
                         for (int ks = 0; ks < 8; ++ks) {
-                            if (ks < KS45) {
-                                const int b45 = 4 * ks + q;
-                                const double av = (m < rows && b45 < c45) ? __ldg(zq + (long)b45 * sZ + m) : 0.0;
-                                fz_dmma(c0, c1, av, bf[ks]);
-                            }
+                            const int b45 = 4 * ks + q;
+                            bf[ks] = (ks < KS45 && b45 < c45 && i4 < n4) ? __ldg(B4b + ((long)q4 * c45 + b45) * c2434n4 + i4) : 0.0;
                         }
-                        if (m < rows) {
-                            const int vv = m / n5, i5 = m - vv * n5, j4 = nt * 8 + 2 * q;
-                            double* dst = Qs + (vv * W4p + r4) * LDQ + i5 * n4 + j4;
-                            if (j4 < n4) dst[0] = c0;
-                            if (j4 + 1 < n4) dst[1] = c1;
+                        for (int mt = 0; mt < MT; ++mt) {
+                            const int m = mt * 8 + g;
+                            double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                            for (int ks = 0; ks < 8; ++ks) {
+                                if (ks < KS45) {
+                                    const int b45 = 4 * ks + q;
+                                    const double av = (m < rows && b45 < c45) ? __ldg(zq + (long)b45 * sZ + m) : 0.0;
+                                    fz_dmma(c0, c1, av, bf[ks]);
+                                }
+                            }
+                            if (m < rows) {
+                                const int vv = m / n5, i5 = m - vv * n5, j4 = nt * 8 + 2 * q;
+                                double* dst = Qs + (vv * W4p + r4) * LDQ + i5 * n4 + j4;
+                                if (j4 < n4) dst[0] = c0;
+                                if (j4 + 1 < n4) dst[1] = c1;
+                            }
                         }
                     }
                 }
             }
-        }
-        fz_cp_wait<0>();
-        __syncthreads();
-        if (v0 + VG < nxs) {                         // the next pass's rows of Z: into L1 under this pass's P phase
-            const int rows2 = min(VG, nxs - v0 - VG) * n5;
-            for (int pr = tid; pr < c45 * w4; pr += FZ_QP_THREADS) {
-                const int b45 = pr / w4, r4 = pr - b45 * w4;
-                const double* row = Zb + (long)b45 * sZ + ((long)(lo4 + r4) * V + v0 + VG) * n5;
-                for (int off = 0; off < rows2; off += 16) fz_prefetch_l1(row + off);
-                fz_prefetch_l1(row + rows2 - 1);
+            __syncthreads();                         // Qs of this pass is complete
+            if (v0 + VG < nxs) {                     // the next pass's rows of Z and S3: into L1 under this pass's P phase
+                const int nv2 = min(VG, nxs - v0 - VG), rows2 = nv2 * n5;
+                for (int pr = tid; pr < c45 * w4; pr += FZ_QP_THREADS) {
+                    const int b45 = pr / w4, r4 = pr - b45 * w4;
+                    const double* row = Zb + (long)b45 * sZ + ((long)(lo4 + r4) * V + v0 + VG) * n5;
+                    for (int off = 0; off < rows2; off += 16) fz_prefetch_l1(row + off);
+                    fz_prefetch_l1(row + rows2 - 1);
+                }
+                for (int pr = tid; pr < nv2 * w3.y; pr += FZ_QP_THREADS) {
+                    const int vv = pr / w3.y, r3 = pr - vv * w3.y;
+                    const double* row = S3b + ((long)(v0 + VG + vv) * P3 + r3) * P4;
+                    for (int off = 0; off < w4; off += 16) fz_prefetch_l1(row + off);
+                    if (w4 > 0) fz_prefetch_l1(row + w4 - 1);
+                }
             }
-        }
-        // ---- P phase: one A fragment feeds four column tiles (four independent accumulator chains) ----
-        const int NTQ = (NT + 3) >> 2;
-        for (int task = warp; task < nv * MT3 * NTQ; task += NW) {
-            const int ntq = task % NTQ, t2 = task / NTQ, mt3 = t2 % MT3, vv = t2 / MT3;
-            // rows k3 the triad (k3 l24 x) allows for this x
-            const int2 wx = fz_window(l24, x0 + 2 * (v0 + vv), P.two_k_base[1], P3);
-            const int rlo = max(wx.x, w3.x) - w3.x, rhi = wx.y > 0 ? min(wx.x + wx.y, w3.x + w3.y) - w3.x : 0;
-            if (mt3 * 8 >= rhi || mt3 * 8 + 8 <= rlo) continue;
-            const double* ap = S3s + (vv * W3p + mt3 * 8 + g) * LDS3 + q;
-            const double* bp = Qs + (vv * W4p + q) * LDQ + ntq * 32 + g;
-            double c[4][2];
+            // ---- P phase: one A fragment (S3, straight from L1/L2) feeds four column tiles of Q ----
+            for (int task = warp; task < nv * MT3 * NTQ; task += NW) {
+                const int ntq = task % NTQ, t2 = task / NTQ, mt3 = t2 % MT3, vv = t2 / MT3;
+                // rows k3 the triad (k3 l24 x) allows for this x
+                const int2 wx = fz_window(l24, x0 + 2 * (v0 + vv), P.two_k_base[1], P3);
+                const int rlo = max(wx.x, w3.x) - w3.x, rhi = wx.y > 0 ? min(wx.x + wx.y, w3.x + w3.y) - w3.x : 0;
+                if (mt3 * 8 >= rhi || mt3 * 8 + 8 <= rlo) continue;
+                const int r3 = mt3 * 8 + g;
+                const bool rok = r3 < w3.y;
+                const double* ap = S3b + ((long)(v0 + vv) * P3 + r3) * P4 + q;
+                const double* bp = Qs + (vv * W4p + q) * LDQ + ntq * 32 + g;
+                const int ntl = min(4, NT - ntq * 4);
+                ndm += ((k4b - k4a) >> 2) * ntl;
+                double c[4][2];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) c[j][0] = c[j][1] = 0.0;
-            ndm += ((k4b - k4a) >> 2) * min(4, NT - ntq * 4);
-            for (int ks = k4a; ks < k4b; ks += 4) {
-                const double av = ap[ks];
+                for (int j = 0; j < 4; ++j) c[j][0] = c[j][1] = 0.0;
+                if (fastp) {
+                    double av[FZ_PKS];
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if (ntq * 4 + j < NT) fz_dmma(c[j][0], c[j][1], av, bp[ks * LDQ + 8 * j]);
-            }
-            const int r3 = mt3 * 8 + g;
-            if (r3 >= rlo && r3 < rhi) {
-                double* dst = Pb + ((long)(w3.x + r3) * V + v0 + vv) * prow + ntq * 32 + 2 * q;
+                    for (int i = 0; i < FZ_PKS; ++i) {
+                        const int ks = k4a + 4 * i;
+                        av[i] = (ks < k4b && rok && ks + q < w4) ? __ldg(ap + ks) : 0.0;
+                    }
 #pragma unroll
-                for (int j = 0; j < 4; ++j)     // NP is even: n + 1 < NP whenever n < n54, and rows are 16-byte aligned
-                    if (ntq * 32 + 8 * j + 2 * q < n54) *reinterpret_cast<double2*>(dst + 8 * j) = make_double2(c[j][0], c[j][1]);
+                    for (int i = 0; i < FZ_PKS; ++i) {
+                        const int ks = k4a + 4 * i;
+                        if (ks < k4b) {
+#pragma unroll
+                            for (int j = 0; j < 4; ++j)
+                                if (j < ntl) fz_dmma(c[j][0], c[j][1], av[i], bp[ks * LDQ + 8 * j]);
+                        }
+                    }
+                } else {
+                    for (int ks = k4a; ks < k4b; ks += 4) {
+                        const double av = (rok && ks + q < w4) ? __ldg(ap + ks) : 0.0;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+                            if (j < ntl) fz_dmma(c[j][0], c[j][1], av, bp[ks * LDQ + 8 * j]);
+                    }
+                }
+                if (r3 >= rlo && r3 < rhi) {
+                    double* dst = Pb + ((long)(w3.x + r3) * V + v0 + vv) * prow + ntq * 32 + 2 * q;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)     // NP is even: n + 1 < NP whenever n < n54, and rows are 16-byte aligned
+                        if (ntq * 32 + 8 * j + 2 * q < n54) *reinterpret_cast<double2*>(dst + 8 * j) = make_double2(c[j][0], c[j][1]);
+                }
             }
         }
     }
@@ -960,7 +978,7 @@ static FzShape fz_shape(const SfDims& D)
     int best = 0;
     double best_fill = 0.0;
     for (int vg = 1; vg <= s.V; ++vg) {
-        const size_t bytes = sizeof(double) * ((size_t)vg * s.W4p * s.LDQ + (size_t)vg * s.W3p * s.LDS3);
+        const size_t bytes = sizeof(double) * (size_t)vg * s.W4p * s.LDQ;
         if (bytes > 100 * 1024) break;
         const int rows = vg * D.n_i[4];
         const double fill = (double)rows / (((rows + 7) / 8) * 8);
@@ -971,7 +989,7 @@ static FzShape fz_shape(const SfDims& D)
     }
     if (best == 0) return s;
     s.VG = best;
-    s.qp_smem = sizeof(double) * ((size_t)s.VG * s.W4p * s.LDQ + (size_t)s.VG * s.W3p * s.LDS3);
+    s.qp_smem = sizeof(double) * (size_t)s.VG * s.W4p * s.LDQ;
     // int offsets inside one gather-GEMM item
     const double slab = (double)D.n_k_pad[1] * s.V * D.nl * D.n_i[2] * s.NP;
     if (slab > 2.0e9 || (double)D.n_out / D.n_i[0] > 2.0e9) return s;
@@ -1085,6 +1103,12 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         if (cudaFuncSetAttribute(k_fz_qp, cudaFuncAttributeMaxDynamicSharedMemorySize, 101 * 1024) != cudaSuccess) return SF_ECUDA;
         qp_attr = true;
     }
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        SF_CUDA_OK(cudaGetDevice(&dev));
+        SF_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
     size_t free_b = 0, total_b = 0;
     if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return SF_ECUDA;
 
@@ -1154,7 +1178,11 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             p.a_lo = a_lo;
             p.a_cnt = (int)(a_lo + na <= n1 ? na : n1 - a_lo);
             fz_ev_begin(0, st);
-            k_fz_qp<<<(unsigned)((long)p.a_cnt * c25 * c35 * c24 * c34), FZ_QP_THREADS, sh.qp_smem, st>>>(p);
+            {
+                const long n_items = (long)p.a_cnt * c25 * c35 * c24 * c34;
+                const long grid = n_items < 2L * n_sm ? n_items : 2L * n_sm;
+                k_fz_qp<<<(unsigned)grid, FZ_QP_THREADS, sh.qp_smem, st>>>(p, n_items);
+            }
             sf_count_launch(1);
             fz_ev_end(st);
             fz_ev_begin(1, st);
