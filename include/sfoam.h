@@ -149,6 +149,11 @@ int sf_last_dmma(double n[3]);
  * The vertex calls return SF_EARG when the selected path cannot hold the problem.  sf_last_path() = path the last
  * vertex call took (1..4). */
 int sf_set_path(int path);
+/* Pure host helper (no device needed): the boxes of shell offsets (o23 o24 o25 o34 o35 o45), o = l - j in units of 1, that
+ * the factorised path splits the range [shell_lo, shell_hi) of the canonical shell order (eq. (9); l45
+ * fastest) into.  boxes[k][0..5] = first offset of each virtual spin, boxes[k][6..11] = number of offsets; at most 11 boxes,
+ * disjoint, in ascending shell order, their union is the range.  SF_EARG on a bad range or an odd / negative two_dl. */
+int sf_shell_boxes(int two_dl, long shell_lo, long shell_hi, int boxes[16][12], int* n_boxes);
 int sf_last_path(void);
 /* Bytes of global scratch the staged path may use for its two ping-pong buffers (default 6 GiB). */
 void sf_set_staged_budget(unsigned long bytes);

@@ -139,6 +139,15 @@ def sf_last_dmma():
     return list(n)
 
 
+def sf_shell_boxes(two_dl, shell_lo, shell_hi):
+    """Boxes (lo[6], cnt[6]) of shell offsets the factorised path splits [shell_lo, shell_hi) into (host only)."""
+    boxes = ((ctypes.c_int * 12) * 16)()
+    n = ctypes.c_int(0)
+    _check(_lib().sf_shell_boxes(int(two_dl), ctypes.c_long(shell_lo), ctypes.c_long(shell_hi), boxes, ctypes.byref(n)),
+           "sf_shell_boxes")
+    return [(list(boxes[k][0:6]), list(boxes[k][6:12])) for k in range(n.value)]
+
+
 def sf_set_path(path):
     """0 = automatic, 1 = staged (general sizes), 2 = first fused on-chip path, 3 = line path (on-chip, register
     accumulation over lines of shells); 2 and 3 raise SF_EARG at call time for shapes they do not hold."""

@@ -940,6 +940,27 @@ static void fz_boxes(int nl, long lo, long hi, int digit, FzBox prefix, FzBox* o
     }
 }
 
+/* Host helper behind the C ABI (include/sfoam.h): the boxes the factorised path splits [shell_lo, shell_hi) into. */
+extern "C" int sf_shell_boxes(int two_dl, long shell_lo, long shell_hi, int boxes[16][12], int* n_boxes)
+{
+    if (!boxes || !n_boxes || two_dl < 0 || (two_dl & 1)) return SF_EARG;
+    const int nl = two_dl / 2 + 1;
+    long n_shells = 1;
+    for (int d = 0; d < 6; ++d) n_shells *= nl;
+    if (shell_lo < 0 || shell_hi > n_shells || shell_lo > shell_hi) return SF_EARG;
+    FzBox b[16], none;
+    memset(&none, 0, sizeof none);
+    int n = 0;
+    fz_boxes(nl, shell_lo, shell_hi, 0, none, b, &n);
+    for (int k = 0; k < n; ++k)
+        for (int d = 0; d < 6; ++d) {
+            boxes[k][d] = b[k].lo[d];
+            boxes[k][6 + d] = b[k].cnt[d];
+        }
+    *n_boxes = n;
+    return SF_OK;
+}
+
 struct FzShape {
     bool ok;
     int V, NP, W3p, W4p, LDQ, LDS3, VG;

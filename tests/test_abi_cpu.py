@@ -114,3 +114,48 @@ def test_no_cpu_fallback():
     with pytest.raises(sf.SfError) as e:
         sf.sf_sixj_get([2, 2, 2, 2, 2, 2])
     assert e.value.status == sf.SF_ENOTINIT
+
+
+def test_shell_boxes_tile_the_range_exactly():
+    """Host logic of the factorised path: a range of the canonical shell order (l45 fastest, eq. (9)) is a
+    disjoint, ordered union of at most 11 boxes of offsets."""
+    import itertools
+    import random
+    rng = random.Random(5)
+    for nl in (1, 2, 3, 4):
+        n = nl ** 6
+        cases = [(0, n), (0, 0), (n, n), (0, 1), (n - 1, n)] + [tuple(sorted((rng.randrange(n + 1), rng.randrange(n + 1))))
+                                                                 for _ in range(40)]
+        for lo, hi in cases:
+            boxes = sf.sf_shell_boxes(2 * (nl - 1), lo, hi)
+            assert len(boxes) <= 11
+            shells = []
+            for blo, cnt in boxes:
+                assert all(c >= 1 for c in cnt) and all(0 <= a and a + c <= nl for a, c in zip(blo, cnt))
+                for o in itertools.product(*[range(a, a + c) for a, c in zip(blo, cnt)]):
+                    s = 0
+                    for d in o:
+                        s = s * nl + d
+                    shells.append(s)
+            # box order = shell order between boxes; inside a box the offsets enumerate a sorted set
+            assert sorted(shells) == list(range(lo, hi)), (nl, lo, hi, boxes)
+            firsts = [min(sh) for sh in _box_shell_sets(boxes, nl)]
+            assert firsts == sorted(firsts)
+    with pytest.raises(sf.SfError):
+        sf.sf_shell_boxes(3, 0, 1)
+    with pytest.raises(sf.SfError):
+        sf.sf_shell_boxes(2, 5, 4)
+
+
+def _box_shell_sets(boxes, nl):
+    import itertools
+    out = []
+    for blo, cnt in boxes:
+        ss = []
+        for o in itertools.product(*[range(a, a + c) for a, c in zip(blo, cnt)]):
+            s = 0
+            for d in o:
+                s = s * nl + d
+            ss.append(s)
+        out.append(ss)
+    return out
