@@ -32,6 +32,9 @@ import workloads as wl  # noqa: E402
 
 METRIC = "eprl_shells_contracted_per_s"
 PATH_NAMES = {1: "staged", 2: "fused", 3: "line", 4: "factorised"}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch (the heaviest of the three passes over i1) from the committed
+# `ncu --set full` captures of config 3, profiles/r1e_factorised.md; null for any other workload
+NCU_TRAFFIC_CONFIG3 = {"k_fz_qp": 15.29e9, "k_fz_gemm<FzMapR>": 24.15e9, "k_fz_gemm<FzMapA>": 8.73e9}
 UNIT = "shells/s"
 
 
@@ -299,7 +302,10 @@ def run_ours(args, cfg, rank, world, local_rank):
         dom = max(names, key=lambda n: per[n]["ms_per_step"])
         tf_all = 512.0 * sum(dmma) / (sum(kms[:3]) / args.steps * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": dom, "achieved": per[dom]["tflops_executed"], "peak": peak,
-                    "unit": "TFLOP/s", "frac": per[dom]["frac"], "traffic": None, "peak_source": peak_source,
+                    "unit": "TFLOP/s", "frac": per[dom]["frac"],
+                    "traffic": NCU_TRAFFIC_CONFIG3.get(dom) if cfg["name"] == wl.CONFIGS[3]["name"] else None,
+                    "traffic_source": "ncu --set full, heaviest of the 3 launches per step, profiles/r1e_factorised.md",
+                    "peak_source": peak_source,
                     "definition": "executed FP64 tensor-pipe flop (512 x issued DMMA.8x8x4, padding included) / event time",
                     "kernels": per, "all_three": {"tflops_executed": tf_all, "frac": tf_all / peak},
                     "precompute_ms_per_step": kms[3] / args.steps,
