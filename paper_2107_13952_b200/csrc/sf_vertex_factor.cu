@@ -45,7 +45,7 @@ struct FzParams {
     int V;                      // largest number of x values of any (i1, l25): triad (i1 l25 x) of eq. (5)
     int NP;                     // n5 * n4 rounded up to even: row length of P and R
     int jsum;                   // sum of the ten boundary spins (2j units)
-    int W3p, W4p, LDQ, LDS3, VG;   // k_fz_qp shared-memory shape
+    int W4p, LDQ, VG;           // k_fz_qp shared-memory shape: Qs[VG][W4p][LDQ]
     const int2* w3A;            // [o34][o35] window (lo, cnt) of q3 allowed by the pair (l34 l35)
     const int2* w3B;            // [o23]      window of q3 allowed by the pair (j13 l23)
     const int2* w4A;            // [o24][o34] window of q4 allowed by the pair (l24 l34)
@@ -963,7 +963,7 @@ extern "C" int sf_shell_boxes(int two_dl, long shell_lo, long shell_hi, int boxe
 
 struct FzShape {
     bool ok;
-    int V, NP, W3p, W4p, LDQ, LDS3, VG;
+    int V, NP, W4p, LDQ, VG;
     size_t qp_smem;
 };
 
@@ -990,11 +990,9 @@ static FzShape fz_shape(const SfDims& D)
             if (a.y > w3) w3 = a.y;
             if (b.y > w4) w4 = b.y;
         }
-    s.W3p = (w3 + 7) & ~7;
     s.W4p = (w4 + 3) & ~3;
-    if (s.W3p == 0 || s.W4p == 0) return s;
+    if (w3 == 0 || s.W4p == 0) return s;
     s.LDQ = ((n54 + 15) & ~15) + 8;                   // = 8 mod 16: conflict-free B fragments
-    s.LDS3 = (s.W4p % 8 == 0) ? s.W4p + 4 : s.W4p;    // = 4 mod 8: conflict-free A fragments
     // x values per pass: fill the 8-row tiles of (v, i5) as well as possible inside ~100 KB (two CTAs per SM)
     int best = 0;
     double best_fill = 0.0;
@@ -1014,6 +1012,8 @@ static FzShape fz_shape(const SfDims& D)
     // int offsets inside one gather-GEMM item
     const double slab = (double)D.n_k_pad[1] * s.V * D.nl * D.n_i[2] * s.NP;
     if (slab > 2.0e9 || (double)D.n_out / D.n_i[0] > 2.0e9) return s;
+    // the k list of A' (one entry per (k3, x, l23)) lives in shared memory beside the operand ring of k_fz_gemm<FzMapA>
+    if ((long)D.n_k_pad[1] * s.V * D.nl > 14000) return s;
     s.ok = true;
     return s;
 }
@@ -1084,8 +1084,6 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     if (!sh.ok) return SF_EARG;
     const int nl = D.nl, n1 = D.n_i[0], n2 = D.n_i[1], n3 = D.n_i[2], n4 = D.n_i[3], n5 = D.n_i[4];
     const int P3 = D.n_k_pad[1], P4 = D.n_k_pad[2];
-    const long slice = D.n_out / n1;
-
     FzBox boxes[16];
     int nbox = 0;
     FzBox none;
@@ -1099,10 +1097,8 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     p.P = P;
     p.V = sh.V;
     p.NP = sh.NP;
-    p.W3p = sh.W3p;
     p.W4p = sh.W4p;
     p.LDQ = sh.LDQ;
-    p.LDS3 = sh.LDS3;
     p.VG = sh.VG;
     for (int s = 0; s < 10; ++s) p.jsum += D.two_j[s];
 
@@ -1130,8 +1126,11 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         SF_CUDA_OK(cudaGetDevice(&dev));
         SF_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     }
-    size_t free_b = 0, total_b = 0;
-    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return SF_ECUDA;
+    static size_t total_b = 0;                       // device memory size: asked once (cudaMemGetInfo costs milliseconds)
+    if (!total_b) {
+        size_t free_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return SF_ECUDA;
+    }
 
     g_fz_ev_used = 0;
     if (sf_counting_on()) {
@@ -1171,8 +1170,13 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         double* B3 = (double*)sf_scratch(FZ_SLOT_B3, sizeof(double) * (size_t)nB3);
         double* S3 = (double*)sf_scratch(FZ_SLOT_S3, sizeof(double) * (size_t)nS3);
         double* G = (double*)sf_scratch(FZ_SLOT_G, sizeof(double) * (size_t)nG);
-        double* Pq = (double*)sf_scratch(FZ_SLOT_P, sizeof(double) * (size_t)(pP * na));
-        double* Rq = (double*)sf_scratch(FZ_SLOT_R, sizeof(double) * (size_t)(pR * na));
+        double *Pq = nullptr, *Rq = nullptr;
+        for (;;) {                                   // other tenants of the device may hold memory: shrink the pass until it fits
+            Pq = (double*)sf_scratch(FZ_SLOT_P, sizeof(double) * (size_t)(pP * na));
+            Rq = Pq ? (double*)sf_scratch(FZ_SLOT_R, sizeof(double) * (size_t)(pR * na)) : nullptr;
+            if ((Pq && Rq) || na == 1) break;
+            na = (na + 1) / 2;
+        }
         int* lists = (int*)sf_scratch(FZ_SLOT_LIST, sizeof(int2) * P3 + sizeof(int) * (size_t)P3 * (1 + c34 * c35));
         if (!Z || !B4 || !B3 || !S3 || !G || !Pq || !Rq || !lists) return SF_ENOMEM;
         p.win23 = (const int2*)lists;

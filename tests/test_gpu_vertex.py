@@ -133,6 +133,26 @@ def test_paths_agree_on_a_full_tensor():
     assert_parity(A3, Ao, Aabs, what="config 2 dl=4, line")
 
 
+def test_config3_full_size_factorised_equals_line():
+    """All 1 771 561 shells of the headline workload, in the launch configuration bench.py times: the factorised path and
+    the per-shell line path (each compared with the oracle on sub-ranges above) give the same tensor to rounding.  A
+    property that holds at any size: both are the sum of eq. (3), in different orders."""
+    cfg = wl.CONFIGS[3]
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    sf.sf_sixj_table(60)
+    sf.sf_set_path(4)
+    A4 = run_gpu(cfg["two_j"], cfg["two_dl"], B, Bdev=Bdev)
+    assert sf.sf_last_path() == 4
+    sf.sf_set_path(3)
+    A3 = run_gpu(cfg["two_j"], cfg["two_dl"], B, Bdev=Bdev)
+    sf.sf_set_path(0)
+    sf.sf_sixj_table(-1)
+    assert np.isfinite(A4).all() and np.abs(A4).max() > 0
+    # FP64 sums of ~1e9 terms per entry in two different orders; measured 8e-15 of the largest entry
+    assert np.abs(A4 - A3).max() <= 1e-12 * np.abs(A3).max()
+
+
 def _config4(lam):
     base, _ = wl.config4_base_spins(lambda tj: all(n > 0 for _, n in ranges.boundary_ranges(tj)))
     assert base == [8, 7, 12, 3, 8, 5, 9, 12, 3, 7]          # SURVEY.md 8(d)
