@@ -993,12 +993,13 @@ static FzShape fz_shape(const SfDims& D)
     s.W4p = (w4 + 3) & ~3;
     if (w3 == 0 || s.W4p == 0) return s;
     s.LDQ = ((n54 + 15) & ~15) + 8;                   // = 8 mod 16: conflict-free B fragments
-    // x values per pass: fill the 8-row tiles of (v, i5) as well as possible inside ~100 KB (two CTAs per SM)
+    // x values per pass: fill the 8-row tiles of (v, i5) as well as possible inside ~100 KB (two CTAs per SM); a single x
+    // may take up to 200 KB (one CTA per SM) before the path gives up
     int best = 0;
     double best_fill = 0.0;
     for (int vg = 1; vg <= s.V; ++vg) {
         const size_t bytes = sizeof(double) * (size_t)vg * s.W4p * s.LDQ;
-        if (bytes > 100 * 1024) break;
+        if (bytes > (vg == 1 ? 200 : 100) * 1024) break;
         const int rows = vg * D.n_i[4];
         const double fill = (double)rows / (((rows + 7) / 8) * 8);
         if (fill > best_fill + 1e-9) {
@@ -1013,7 +1014,7 @@ static FzShape fz_shape(const SfDims& D)
     const double slab = (double)D.n_k_pad[1] * s.V * D.nl * D.n_i[2] * s.NP;
     if (slab > 2.0e9 || (double)D.n_out / D.n_i[0] > 2.0e9) return s;
     // the k list of A' (one entry per (k3, x, l23)) lives in shared memory beside the operand ring of k_fz_gemm<FzMapA>
-    if ((long)D.n_k_pad[1] * s.V * D.nl > 14000) return s;
+    if ((long)D.n_k_pad[1] * s.V * D.nl > 14700) return s;    // 226 KB - 110.6 KB ring - 3.1 KB tables = 8 B x 14 712 entries
     s.ok = true;
     return s;
 }
@@ -1117,7 +1118,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     }
     static bool qp_attr = false;
     if (!qp_attr) {
-        if (cudaFuncSetAttribute(k_fz_qp, cudaFuncAttributeMaxDynamicSharedMemorySize, 101 * 1024) != cudaSuccess) return SF_ECUDA;
+        if (cudaFuncSetAttribute(k_fz_qp, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024) != cudaSuccess) return SF_ECUDA;
         qp_attr = true;
     }
     static int n_sm = 0;

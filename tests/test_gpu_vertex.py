@@ -159,7 +159,7 @@ def _config4(lam):
     return wl.config4(base, lam)
 
 
-@pytest.mark.parametrize("lam,n", [(1, 60), (2, 6), (3, 1)])
+@pytest.mark.parametrize("lam,n", [(1, 60), (2, 6), (3, 1), (4, 1), (6, 1)])
 def test_config4_sub_ranges(path, lam, n):
     if path == 3 and lam > 1:
         pytest.skip("the line path holds intertwiner ranges of at most 16 values")
