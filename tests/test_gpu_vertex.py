@@ -240,6 +240,33 @@ def test_half_integer_nonhomogeneous_full(path):
     assert_parity(Ag, Ao, Aabs, what="half-integer non-homogeneous")
 
 
+def test_random_small_spin_sets_full(path):
+    """Seeded random boundary spins (integer and half-integer mixed, 2j <= 5) with random Delta_l <= 2, full tensors:
+    irregular ranges, empty k-ranges for some triples, one-value intertwiner ranges."""
+    rng = random.Random(2107)
+    done = 0
+    while done < 8:
+        two_j = [rng.randrange(0, 6) for _ in range(10)]
+        two_dl = 2 * rng.randrange(0, 3)
+        if not all(n > 0 for _, n in ranges.boundary_ranges(two_j)):
+            continue
+        cfg = dict(two_j=two_j, two_dl=two_dl, boosters="random", seed=1000 + done)
+        try:
+            B = boosters_for(cfg)
+        except sf.SfError:
+            continue                                  # a booster edge without any valid k: nothing to contract
+        try:
+            Ag = run_gpu(two_j, two_dl, B)
+        except sf.SfError as e:
+            if path == 3 and e.status == sf.SF_EARG:
+                done += 1
+                continue                              # the line path does not hold this shape
+            raise
+        Ao, Aabs = run_oracle(two_j, two_dl, B)
+        assert_parity(Ag, Ao, Aabs, what=f"random spins {two_j} dl {two_dl}")
+        done += 1
+
+
 def test_errors(path):
     two_j = [2] * 10
     B = to_device(boosters_for(wl.CONFIGS[0]))
