@@ -1,6 +1,6 @@
 """bench.py -- throughput of the EPRL vertex-tensor hot path (all rows of SURVEY.md 8(a)) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference] [--path 0..4]
 
 A "step" is one pass of the whole hot path over one workload: one sf_vertex_amplitude call (k-range tables, the five S
 arrays of {6j}, {15j} assembly + four mode products over every shell, fixed-order accumulation, normalisation).  The
@@ -10,6 +10,12 @@ tables) is built before the timed region and reported separately.
 
 N > 1: the path does not shard (north_star: one GPU, no collectives) => N independent replicas, one per rank,
 "scaling": "weak"; value = shells of all replicas / max-over-ranks time.
+
+The library takes the fastest path that holds the problem (`--path 0`): the factorised path (the sum of eq. (3) taken one
+virtual spin at a time, DESIGN.md 5 K-f); `--path 3` times the per-shell line kernel instead.  Timed region: K asynchronous
+calls between two CUDA events on the call's stream.  `roofline` then comes from a second, instrumented pass of K steps
+(per-kernel CUDA events inside the library) and one call with the kernels' DMMA counters on: achieved = executed FP64
+tensor-pipe flop of the kernel that takes the most time / its event time, against the DMMA peak measured in this process.
 
 Prints ONE JSON line (rank 0).  `--impl reference` times the oracle (oracle/, plain CPU loops) on the host cores on a
 bounded sample of the same workload.
