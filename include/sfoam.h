@@ -114,6 +114,14 @@ int sf_vertex_amplitude(const int two_j[10], int two_dl, const sf_boosters *boos
  * Ranges are additive: the sum of the outputs over a partition of the shells equals the full tensor up to rounding. */
 int sf_vertex_amplitude_range(const int two_j[10], int two_dl, const sf_boosters *boosters,
                               long shell_lo, long shell_hi, double *out, sf_stream_t stream);
+/* The vertex tensor for a reduced set of boundary intertwiners ("It is also possible to compute the vertex
+ * tensor for a reduced set of intertwiner indices"; also the paper's way of splitting a tensor that does not
+ * fit into batches over i1): node n = 1..5 keeps the i_count[n-1] values starting at index i_first[n-1] (0-based offset
+ * from the range minimum of sf_vertex_dims, steps of 1 in spin).  boosters: the caller's full arrays, unchanged layout.
+ * out: DEVICE pointer, prod(i_count) doubles, row-major out[i1][i2][i3][i4][i5] over the kept values, overwritten; equal to
+ * the corresponding sub-block of the full tensor.  SF_EARG if a range leaves the node's range or a count is < 1. */
+int sf_vertex_amplitude_intertwiners(const int two_j[10], int two_dl, const sf_boosters *boosters,
+                                     const int i_first[5], const int i_count[5], double *out, sf_stream_t stream);
 /* End-to-end variant with HOST buffers (pinned or pageable): copies the four boosters to the device, computes, copies
  * the tensor back and synchronises `stream`.  host_boosters[e] holds n_triples*n_i*n_k_pad doubles. */
 int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const double *const host_boosters[4],

@@ -58,6 +58,8 @@ def _lib():
                                             ctypes.c_void_p]
         lib.sf_vertex_amplitude_range.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_long,
                                                   ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
+        lib.sf_vertex_amplitude_intertwiners.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_int * 5,
+                                                         ctypes.c_int * 5, ctypes.c_void_p, ctypes.c_void_p]
         lib.sf_vertex_amplitude_host.argtypes = [_I10, ctypes.c_int, ctypes.c_void_p * 4, ctypes.c_void_p,
                                                  ctypes.c_void_p]
         lib.sf_set_staged_budget.argtypes = [ctypes.c_size_t]
@@ -277,6 +279,17 @@ def sf_vertex_amplitude_range(two_j, two_dl, boosters, shell_lo, shell_hi, out, 
     b = _boosters(boosters)
     _check(_lib().sf_vertex_amplitude_range(_spins(two_j), int(two_dl), ctypes.byref(b), int(shell_lo), int(shell_hi),
                                             _ptr(out), _stream(stream)), "sf_vertex_amplitude_range")
+    return out
+
+
+def sf_vertex_amplitude_intertwiners(two_j, two_dl, boosters, i_first, i_count, out, stream=None):
+    """The sub-block out[i1][i2][i3][i4][i5] of the vertex tensor over i_count[n] intertwiner values of node n + 1 starting
+    at index i_first[n]."""
+    b = _boosters(boosters)
+    first = (ctypes.c_int * 5)(*[int(v) for v in i_first])
+    count = (ctypes.c_int * 5)(*[int(v) for v in i_count])
+    _check(_lib().sf_vertex_amplitude_intertwiners(_spins(two_j), int(two_dl), ctypes.byref(b), first, count, _ptr(out),
+                                                   _stream(stream)), "sf_vertex_amplitude_intertwiners")
     return out
 
 

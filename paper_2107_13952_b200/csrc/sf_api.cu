@@ -173,7 +173,8 @@ __global__ void k_kranges(SfProblem P, int nt, SfKRange* __restrict__ out)
 }
 
 // steps 1-2 on the device side: the problem descriptor and the per-triple k-range tables (no host->device copy)
-static int setup_problem(const SfDims& D, const sf_boosters* boosters, SfProblem& P, cudaStream_t st)
+static int setup_problem(const SfDims& D, const sf_boosters* boosters, SfProblem& P, cudaStream_t st,
+                         const int* b_rows = nullptr, const int* b_first = nullptr)
 {
     memset(&P, 0, sizeof P);
     memcpy(P.two_j, D.two_j, sizeof P.two_j);
@@ -185,7 +186,11 @@ static int setup_problem(const SfDims& D, const sf_boosters* boosters, SfProblem
     memcpy(P.k_max, D.k_max, sizeof P.k_max);
     P.two_x_base = D.two_x_base;
     P.n_x_pad = D.n_x_pad;
-    for (int e = 0; e < 4; ++e) P.B[e] = boosters ? boosters->B[e] : nullptr;
+    for (int e = 0; e < 4; ++e) {
+        P.B[e] = boosters ? boosters->B[e] : nullptr;
+        P.b_n[e] = b_rows ? b_rows[e] : D.n_i[e + 1];
+        P.b_i0[e] = b_first ? b_first[e] : 0;
+    }
     const int nt = D.nl * D.nl * D.nl;
     SfKRange* d = (SfKRange*)sf_scratch(SLOT_KR, sizeof(SfKRange) * nt * 4);
     if (!d) return SF_ENOMEM;
@@ -196,7 +201,7 @@ static int setup_problem(const SfDims& D, const sf_boosters* boosters, SfProblem
 }
 
 static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo, long shell_hi,
-                        double* out, cudaStream_t st, bool full)
+                        double* out, cudaStream_t st, bool full, const int* i_first = nullptr, const int* i_count = nullptr)
 {
     if (!g_ctx.init) return SF_ENOTINIT;
     if (!two_j || !boosters || !out) return SF_EARG;
@@ -209,6 +214,26 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
         shell_lo = 0;
         shell_hi = D.n_shells;
     }
+    // a restricted range of boundary intertwiners: the same problem with shifted range minima; only
+    // the rows taken from the caller's boosters keep the full layout
+    int b_rows[4], b_first[4];
+    for (int e = 0; e < 4; ++e) {
+        b_rows[e] = D.n_i[e + 1];
+        b_first[e] = 0;
+    }
+    if (i_first && i_count) {
+        long n_out = 1;
+        for (int n = 0; n < 5; ++n) {
+            if (i_first[n] < 0 || i_count[n] < 1 || i_first[n] + i_count[n] > D.n_i[n]) return SF_EARG;
+            n_out *= i_count[n];
+        }
+        for (int n = 0; n < 5; ++n) {
+            if (n > 0) b_first[n - 1] = i_first[n];
+            D.two_i_min[n] += 2 * i_first[n];
+            D.n_i[n] = i_count[n];
+        }
+        D.n_out = n_out;
+    }
     if (shell_lo < 0 || shell_hi > D.n_shells || shell_lo > shell_hi) return SF_EARG;
     // largest factorial argument of any 6j on the path stays inside the table of sf_sixj.cuh
     {
@@ -218,7 +243,7 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
     }
 
     SfProblem P;
-    rc = setup_problem(D, boosters, P, st);
+    rc = setup_problem(D, boosters, P, st, b_rows, b_first);
     if (rc != SF_OK) return rc;
 
     // step 4: the five S arrays
@@ -271,6 +296,13 @@ extern "C" int sf_vertex_amplitude_range(const int two_j[10], int two_dl, const 
                                          long shell_hi, double* out, sf_stream_t stream)
 {
     return vertex_range(two_j, two_dl, boosters, shell_lo, shell_hi, out, (cudaStream_t)stream, false);
+}
+
+extern "C" int sf_vertex_amplitude_intertwiners(const int two_j[10], int two_dl, const sf_boosters* boosters,
+                                                const int i_first[5], const int i_count[5], double* out, sf_stream_t stream)
+{
+    if (!i_first || !i_count) return SF_EARG;
+    return vertex_range(two_j, two_dl, boosters, 0, 0, out, (cudaStream_t)stream, true, i_first, i_count);
 }
 
 extern "C" int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const double* const host_boosters[4],

@@ -47,7 +47,15 @@ struct SfProblem {
     const SfKRange* kr[4];        // device: per edge, nl^3 entries
     const double* S[5];           // device: S1..S5, layouts in sf_slices.cu
     const double* B[4];           // device: caller's boosters, edges 2..5
+    int b_n[4], b_i0[4];          // rows per triple of the caller's booster, and the row of this problem's first intertwiner
+                                  // (a restricted intertwiner range, keeps the caller's full layout)
 };
+
+// row (i, :) of the booster of edge e + 2 at triple t; ii counts from this problem's first intertwiner
+__host__ __device__ inline const double* sf_brow(const SfProblem& P, int e, long t, int ii)
+{
+    return P.B[e] + (t * P.b_n[e] + P.b_i0[e] + ii) * P.n_k_pad[e];
+}
 
 // shell -> offsets (o23 o24 o25 o34 o35 o45), o45 fastest (eq. (9))
 __host__ __device__ inline void sf_shell_offsets(long shell, int nl, int o[6])

@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(256) k_fz_z(FzParams p, double* __restrict__ Z
         const int i5 = e % n5, r = e / n5, v = r % nxs, q4 = r / nxs;
         const double* s2 = P.S[1] + ((((long)(o35 * nl + o45) * P4 + q4) * P5 + q5b) * NX) + xg0 + v;
         const double* s1 = P.S[0] + (((long)(o25 * n1 + a1) * P5 + q5b) * NX) + xg0 + v;
-        const double* b5 = P.B[3] + ((long)t5 * n5 + i5) * P5 + q5b;
+        const double* b5 = sf_brow(P, 3, t5, i5) + q5b;
         double val = 0.0;
         for (int c = 0; c < r5.n_k; ++c) {
             double term = s2[(long)c * NX] * s1[(long)c * NX] * ((double)(r5.two_k_min + 2 * c + 1) * b5[c]);
@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(256) k_fz_b4t(FzParams p, long n, double* __re
     const SfKRange r4 = P.kr[2][t4];
     const int c = q4 - ((r4.two_k_min - P.two_k_base[2]) >> 1);
     double val = 0.0;
-    if (c >= 0 && c < r4.n_k) val = (double)(r4.two_k_min + 2 * c + 1) * P.B[2][((long)t4 * n4 + i4) * P4 + q4];
+    if (c >= 0 && c < r4.n_k) val = (double)(r4.two_k_min + 2 * c + 1) * sf_brow(P, 2, t4, i4)[q4];
     out[e] = val;
 }
 
@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(256) k_fz_b3t(FzParams p, long n, double* __re
     const SfKRange r3 = P.kr[1][t3];
     const int c = q3 - ((r3.two_k_min - P.two_k_base[1]) >> 1);
     double val = 0.0;
-    if (c >= 0 && c < r3.n_k) val = (double)(r3.two_k_min + 2 * c + 1) * P.B[1][((long)t3 * n3 + i3) * P3 + q3];
+    if (c >= 0 && c < r3.n_k) val = (double)(r3.two_k_min + 2 * c + 1) * sf_brow(P, 1, t3, i3)[q3];
     out[e] = val;
 }
 
@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(256) k_fz_g(FzParams p, long n, double* __rest
         const int h0 = (p.jsum + i1 + P.two_k_base[0] + P.two_k_base[1] + P.two_k_base[2] + P.two_k_base[3]) >> 1;
         const double* s5 = P.S[4] + (((long)o25 * n1 + a1) * P2 + q2b) * NX + xg0 + v;
         const double* s4 = P.S[3] + ((((long)o23 * nl + o24) * P2 + q2b) * P3 + q3) * NX + xg0 + v;
-        const double* b2 = P.B[0] + ((long)blk * n2 + i2) * P2 + q2b;
+        const double* b2 = sf_brow(P, 0, blk, i2) + q2b;
         for (int c = 0; c < r2.n_k; ++c) {
             double term = (double)(r2.two_k_min + 2 * c + 1) * b2[c] * s5[(long)c * NX] * s4[(long)c * P3 * NX];
             if ((q2b + c) & 1) term = -term;

@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 1) k_vertex_fused(const FusedPa
                     if (ii < P.n_i[e + 1] && c < sd.K[e]) {
                         const int kk0 = (sd.kmin[e] - P.two_k_base[e]) >> 1;
                         v = (double)(sd.kmin[e] + 2 * c + 1) *
-                            P.B[e][((long)sd.t[e] * P.n_i[e + 1] + ii) * P.n_k_pad[e] + kk0 + c];
+                            sf_brow(P, e, sd.t[e], ii)[kk0 + c];
                     }
                     Bw[z] = v;
                 }

@@ -124,7 +124,7 @@ __global__ void k_line_prep_z(SfProblem P, int NT8, int NXF, double* __restrict_
         const int q5b = (r5.two_k_min - P.two_k_base[3]) >> 1;
         const double* s2 = P.S[1] + ((((long)(o35 * nl + o45) * P4 + q4) * P5 + q5b) * NX) + xg;
         const double* s1 = P.S[0] + (((long)(o25 * n1 + a1) * P5 + q5b) * NX) + xg;
-        const double* b5 = P.B[3] + ((long)t5 * n5 + n) * P5 + q5b;
+        const double* b5 = sf_brow(P, 3, t5, n) + q5b;
         for (int c = 0; c < r5.n_k; ++c) {
             double term = s2[(long)c * NX] * s1[(long)c * NX] * ((double)(r5.two_k_min + 2 * c + 1) * b5[c]);
             if ((q5b + c) & 1) term = -term;
@@ -144,7 +144,7 @@ __global__ void k_line_prep_b4(SfProblem P, int NT8, int LDK4, double* __restric
     for (int e = threadIdx.x; e < NT8 * LDK4; e += blockDim.x) {
         const int n = e / LDK4, c = e - n * LDK4;
         double val = 0.0;
-        if (n < n4 && c < r4.n_k) val = (double)(r4.two_k_min + 2 * c + 1) * P.B[2][((long)t4 * n4 + n) * P4 + q4b + c];
+        if (n < n4 && c < r4.n_k) val = (double)(r4.two_k_min + 2 * c + 1) * sf_brow(P, 2, t4, n)[q4b + c];
         Bw4[(long)t4 * NT8 * LDK4 + e] = val;
     }
 }
@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(LINE_THREADS, 1) k_vertex_line(const LineParam
             }
             for (int e = tid; e < n2 * SLOTS; e += LINE_CONSUMERS) {
                 const int s = e % SLOTS, i2 = e / SLOTS;
-                Bw2[e] = s < nslots ? (double)(u.k2min + 2 * (u.cb + s) + 1) * P.B[0][((long)u.blk * n2 + i2) * P2 + u.q2b + u.cb + s] : 0.0;
+                Bw2[e] = s < nslots ? (double)(u.k2min + 2 * (u.cb + s) + 1) * sf_brow(P, 0, u.blk, i2)[u.q2b + u.cb + s] : 0.0;
             }
             for (int e = tid; e < SLOTS * R; e += LINE_CONSUMERS) X2[e] = 0.0;
         }
@@ -367,7 +367,7 @@ __global__ void __launch_bounds__(LINE_THREADS, 1) k_vertex_line(const LineParam
                 for (int e = tid; e < NT8 * LDK3; e += LINE_CONSUMERS) {
                     const int ii = e / LDK3, c = e - ii * LDK3;
                     Bw3[e] = (ii < n3 && c < K3)
-                                 ? (double)(r3.two_k_min + 2 * c + 1) * P.B[1][((long)t3 * n3 + ii) * P3 + q3b + c]
+                                 ? (double)(r3.two_k_min + 2 * c + 1) * sf_brow(P, 1, t3, ii)[q3b + c]
                                  : 0.0;
                 }
                 for (int row = tid; row < lp.mt_max * 8; row += LINE_CONSUMERS) {

@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(128) k_stage_mode(SfProblem P, long shell0, in
     const int K = S.K[e], N = P.n_i[e + 1], Kmax = P.k_max[e];
     {
         const int kk0 = (S.kmin[e] - P.two_k_base[e]) >> 1, Pk = P.n_k_pad[e];
-        const double* Bm = P.B[e] + (long)S.t[e] * N * Pk;
+        const double* Bm = sf_brow(P, e, S.t[e], 0);
         for (int q = threadIdx.x; q < N * K; q += blockDim.x) {
             const int ii = q / K, c = q % K;
             Bw[q] = (double)(S.kmin[e] + 2 * c + 1) * Bm[(long)ii * Pk + kk0 + c];

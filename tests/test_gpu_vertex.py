@@ -267,6 +267,46 @@ def test_random_small_spin_sets_full(path):
         done += 1
 
 
+def _run_sub(two_j, two_dl, Bdev, first, count):
+    out = torch.full(tuple(count), float("nan"), dtype=torch.float64, device="cuda")
+    sf.sf_vertex_amplitude_intertwiners(two_j, two_dl, Bdev, first, count, out, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+@pytest.mark.parametrize("which", ["config0", "config2_dl2", "half_integer"])
+def test_reduced_intertwiner_ranges(path, which):
+    """the tensor for a reduced set of boundary intertwiners = the sub-block of the full tensor; batches
+    over i1 joined at the end give the full tensor."""
+    if which == "config0":
+        cfg = wl.CONFIGS[0]
+    elif which == "config2_dl2":
+        cfg = wl.config2(2)
+    else:
+        cfg = dict(two_j=[4, 3, 1, 4, 2, 5, 5, 5, 4, 3], two_dl=4, boosters="random", seed=77)
+    two_j, two_dl = cfg["two_j"], cfg["two_dl"]
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    Ao, Aabs = run_oracle(two_j, two_dl, B)
+    _, n_i = sf.sf_vertex_dims(two_j)
+    rng = random.Random(41)
+    for _ in range(4):
+        first = [rng.randrange(n) for n in n_i]
+        count = [rng.randrange(1, n - f + 1) for n, f in zip(n_i, first)]
+        sl = tuple(slice(f, f + c) for f, c in zip(first, count))
+        assert_parity(_run_sub(two_j, two_dl, Bdev, first, count), Ao[sl], Aabs[sl], what=f"{which} block {first} {count}")
+    # batches over i1, joined (the paper's way of splitting a tensor that does not fit)
+    full = run_gpu(two_j, two_dl, B, Bdev=Bdev)
+    joined = np.concatenate([_run_sub(two_j, two_dl, Bdev, [a, 0, 0, 0, 0], [1] + list(n_i[1:])) for a in range(n_i[0])], axis=0)
+    assert_parity(joined, Ao, Aabs, what=f"{which} joined i1 batches")
+    assert np.abs(joined - full).max() <= 1e-13 * max(Aabs.max(), 1e-300)
+    for bad_first, bad_count in [([0] * 5, [n_i[0] + 1] + list(n_i[1:])), ([0, 0, -1, 0, 0], list(n_i)), ([0] * 5, [1, 1, 0, 1, 1])]:
+        with pytest.raises(sf.SfError) as e:
+            sf.sf_vertex_amplitude_intertwiners(two_j, two_dl, Bdev, bad_first, bad_count,
+                                                torch.zeros(8, dtype=torch.float64, device="cuda"))
+        assert e.value.status == sf.SF_EARG
+
+
 def test_errors(path):
     two_j = [2] * 10
     B = to_device(boosters_for(wl.CONFIGS[0]))
