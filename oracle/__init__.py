@@ -16,6 +16,8 @@ Contents (each function cites the PAPER.md passage it restates):
   vertex.py     eq. (3): level L0 = literal nested sum (tiny inputs),
                 level L1 = per-shell W + naive mode products (C loops)   [pinned]
   vertex_l1.c   the naive C loops behind L1 (steps 5-7)
+  contract.py   downstream contractions vertex x vertex and vertex x five
+                complex vectors, exact sums       [pinned]
 
 Parity status: every function here is pinned by `tests/test_oracle_*.py`
 (closed forms, identities, printed exact values under tests/golden/, brute
