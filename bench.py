@@ -176,6 +176,44 @@ def whole_job_value(units_per_rank, steps, world, seconds):
     return world * units_per_rank * steps / seconds
 
 
+def bench_contractions(torch, sf, stream):
+    """Secondary row (SURVEY.md K-e; Fig. 3): vertex x vertex and vertex x five complex vectors on
+    synthetic tensors of (2J+1)^5 entries, J = 10 and J = 20.  HBM-bound streaming reductions: algorithmic bytes = 8 B per
+    entry read once (16 B for two tensors) / CUDA-event time, against the measured copy bandwidth."""
+    peak = None
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            peak = float(json.load(fh)["hbm_gbs"])
+    except (OSError, KeyError, ValueError):
+        pass
+    peak_src = "MEASURED_PEAKS.json hbm_gbs" if peak else "fallback of B200_PROFILING.md (6550 GB/s copy bandwidth)"
+    peak = peak or 6550.0
+    out = {"unit": "GB/s", "peak": peak, "peak_source": peak_src, "bound": "hbm", "cases": []}
+    for n in (21, 41):
+        A = torch.randn((n,) * 5, dtype=torch.float64, device="cuda")
+        B = torch.randn((n,) * 5, dtype=torch.float64, device="cuda")
+        psi = [torch.randn(n, dtype=torch.complex128, device="cuda") for _ in range(5)]
+        res = torch.zeros(2, dtype=torch.float64, device="cuda")
+        for name, call, nbytes in (("vertex_x_vertex", lambda: sf.sf_contract_vertices(A, B, res, stream), 16 * A.numel()),
+                                   ("vertex_x_5_vectors", lambda: sf.sf_contract_vectors(A, psi, res, stream), 8 * A.numel())):
+            for _ in range(3):
+                call()
+            reps = 20
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                call()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            gbs = nbytes / (ms * 1e-3) / 1e9
+            out["cases"].append({"contraction": name, "entries": A.numel(), "ms": ms, "achieved": gbs, "frac": gbs / peak,
+                                 "note": "back-to-back repeats: the %d MB working set %s the 126 MB L2"
+                                         % (nbytes >> 20, "fits" if nbytes < 126 << 20 else "exceeds")})
+        del A, B
+    return out
+
+
 def run_ours(args, cfg, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -343,6 +381,8 @@ def run_ours(args, cfg, rank, world, local_rank):
                                "accumulate_normalise": stage[2] / args.steps},
         "sixj_table_build_ms": table_ms,
     }
+    if world == 1:
+        line["contractions"] = bench_contractions(torch, sf, stream)
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         n_sample = min(args.ref_shells, n_shells)

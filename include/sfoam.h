@@ -127,6 +127,18 @@ int sf_vertex_amplitude_intertwiners(const int two_j[10], int two_dl, const sf_b
 int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const double *const host_boosters[4],
                              double *host_out, sf_stream_t stream);
 
+/* Downstream contractions of vertex tensors (Fig. 3; the paper's contract(...)).  All
+ * pointers are DEVICE pointers; asynchronous, ordered on `stream`; fixed summation order (bitwise reproducible).
+ *   sf_contract_vertices: result[0] = sum_z a[z] b[z] over the n entries of two vertex tensors of the same shape (all five
+ *     edges glued).
+ *   sf_contract_vectors: result[0] + i result[1] = sum A[i1][i2][i3][i4][i5] psi[0][i1] psi[1][i2] psi[2][i3] psi[3][i4]
+ *     psi[4][i5]; A in the layout of sf_vertex_amplitude with n_i[5] entries per index, psi[e] = n_i[e] complex numbers
+ *     stored (re, im) interleaved, no conjugation (coherent-state coefficients in the paper; their computation is out of
+ *     scope).
+ * SF_EARG on a null pointer, n < 0 or an n_i < 1. */
+int sf_contract_vertices(const double *a, const double *b, long n, double *result, sf_stream_t stream);
+int sf_contract_vectors(const double *A, const int n_i[5], const double *const psi[5], double *result, sf_stream_t stream);
+
 /* Number of kernels the library launched since sf_init / the last reset (bench.py's gpu_launches). */
 long sf_launch_count(int reset);
 /* Milliseconds of device time (CUDA events on the call's stream) spent in each stage of the LAST vertex call,

@@ -60,6 +60,9 @@ def _lib():
                                                   ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
         lib.sf_vertex_amplitude_intertwiners.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_int * 5,
                                                          ctypes.c_int * 5, ctypes.c_void_p, ctypes.c_void_p]
+        lib.sf_contract_vertices.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
+        lib.sf_contract_vectors.argtypes = [ctypes.c_void_p, ctypes.c_int * 5, ctypes.c_void_p * 5, ctypes.c_void_p,
+                                            ctypes.c_void_p]
         lib.sf_vertex_amplitude_host.argtypes = [_I10, ctypes.c_int, ctypes.c_void_p * 4, ctypes.c_void_p,
                                                  ctypes.c_void_p]
         lib.sf_set_staged_budget.argtypes = [ctypes.c_size_t]
@@ -291,6 +294,22 @@ def sf_vertex_amplitude_intertwiners(two_j, two_dl, boosters, i_first, i_count, 
     _check(_lib().sf_vertex_amplitude_intertwiners(_spins(two_j), int(two_dl), ctypes.byref(b), first, count, _ptr(out),
                                                    _stream(stream)), "sf_vertex_amplitude_intertwiners")
     return out
+
+
+def sf_contract_vertices(a, b, result, stream=None):
+    """result[0] = sum a b over two vertex tensors of the same shape (device tensors)."""
+    _check(_lib().sf_contract_vertices(_ptr(a), _ptr(b), ctypes.c_long(a.numel()), _ptr(result), _stream(stream)),
+           "sf_contract_vertices")
+    return result
+
+
+def sf_contract_vectors(A, psi, result, stream=None):
+    """result[0] + i result[1] = sum A[i1..i5] psi[0][i1] ... psi[4][i5]; A a 5-index float64 device tensor, psi five
+    complex128 device tensors."""
+    n = (ctypes.c_int * 5)(*[int(v) for v in A.shape])
+    arr = (ctypes.c_void_p * 5)(*[p.data_ptr() for p in psi])
+    _check(_lib().sf_contract_vectors(_ptr(A), n, arr, _ptr(result), _stream(stream)), "sf_contract_vectors")
+    return result
 
 
 def sf_vertex_amplitude_host(two_j, two_dl, host_boosters, host_out, stream=None):
