@@ -567,7 +567,7 @@ struct FzGemmHdr {
 // rows m = (i5 i4), columns n = (l23 i3) over the l23 whose pair (j13 l23) allows k3; one item = (i1, l24, l25, k3, tile),
 // every x of (i1 l25) in turn
 struct FzMapR {
-    static constexpr bool A16 = true;
+    static constexpr bool A16 = true, B16 = false;
     static constexpr int CNT = 1, KC = 32, ST = 2;    // rows of P start 16-byte aligned (NP even) and m runs contiguously: copy pairs
     static __device__ const double* srcA(const FzParams& p) { return p.Pq; }
     static __device__ const double* srcB(const FzParams& p) { return p.Bw3T; }
@@ -628,13 +628,14 @@ struct FzMapR {
 // A'[l24 l25; i1; i2; (i3 i4 i5)] = sum over (k3, x, l23) with k3 allowed by (j13 l23) of G[..][(k3 x l23)][i2] R[..][(k3 x l23)][(i3, i5 i4)]
 struct FzMapA {
     static constexpr bool A16 = false;
+    static constexpr bool B16 = true;    // columns run over the padded rows of R (i3, NP): contiguous and 16-byte aligned pairs
     static constexpr int CNT = 2, KC = 16, ST = 3;
     static __device__ const double* srcA(const FzParams& p) { return p.G; }
     static __device__ const double* srcB(const FzParams& p) { return p.Rq; }
     static __device__ double* dstC(const FzParams& p) { return p.Apart; }
     static __host__ __device__ long items(const FzParams& p, int BM, int BN)
     {
-        const long ntn = ((long)p.P.n_i[2] * p.P.n_i[3] * p.P.n_i[4] + BN - 1) / BN, ntm = (p.P.n_i[1] + BM - 1) / BM;
+        const long ntn = ((long)p.P.n_i[2] * p.NP + BN - 1) / BN, ntm = (p.P.n_i[1] + BM - 1) / BM;
         return ntn * ntm * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
     }
     static __device__ void setup(const FzParams& p, long item, int BM, int BN, FzGemmHdr* h, int* offAm, int* offCm,
@@ -644,7 +645,8 @@ struct FzMapA {
         const int n1 = P.n_i[0], n2 = P.n_i[1], n3 = P.n_i[2], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5, n345 = n3 * n54;
         const int P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
         const int c23 = p.box.cnt[0], c24 = p.box.cnt[1], c25 = p.box.cnt[2];
-        const int ntn = (n345 + BN - 1) / BN, ntm = (n2 + BM - 1) / BM;
+        const int NN = n3 * NP;                      // columns (i3, r) over the padded rows of R; r >= n5 n4 is padding
+        const int ntn = (NN + BN - 1) / BN, ntm = (n2 + BM - 1) / BM;
         const int nt = (int)(item % ntn); item /= ntn;
         const int mt = (int)(item % ntm); item /= ntm;
         const int b25 = (int)(item % c25); item /= c25;
@@ -653,7 +655,7 @@ struct FzMapA {
         const int a1 = p.a_lo + ac;
         int x0, nxs, xg0;
         fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, p.box.lo[2] + b25, x0, nxs, xg0);
-        const int m0 = mt * BM, n0 = nt * BN, M = min(BM, n2 - m0), N = min(BN, n345 - n0);
+        const int m0 = mt * BM, n0 = nt * BN, M = min(BM, n2 - m0), N = min(BN, NN - n0);
         // k list in the order (k3, x, l23): the x of each k3 (triad (k3 l24 x)), then prefix sums of (x count) * (l23 count)
         const int l24 = P.two_j[J24] + 2 * (p.box.lo[1] + b24);
         for (int q3 = threadIdx.x; q3 < P3; q3 += blockDim.x) {
@@ -683,9 +685,9 @@ struct FzMapA {
             offCm[m] = (m0 + m) * n345;
         }
         for (int n = threadIdx.x; n < BN; n += blockDim.x) {
-            const int ng = n0 + n, i3 = ng / n54, r = ng - i3 * n54, i5 = r / n4, i4 = r - i5 * n4;
-            offBn[n] = i3 * NP + r;
-            offCn[n] = (i3 * n4 + i4) * n5 + i5;
+            const int ng = n0 + n, i3 = ng / NP, r = ng - i3 * NP, i5 = r / n4, i4 = r - i5 * n4;
+            offBn[n] = ng;
+            offCn[n] = r < n54 ? (i3 * n4 + i4) * n5 + i5 : -1;      // -1: a padding column, never stored
         }
         __syncthreads();
         for (int e = threadIdx.x; e < P3 * nxs; e += blockDim.x) {
@@ -793,8 +795,8 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
 #pragma unroll
                 for (int j = 0; j < TN; ++j) {
                     const int n = wn * TN * 8 + 8 * j + 2 * q;
-                    if (n < N) cm[offCn[n]] = acc[i][j][0];
-                    if (n + 1 < N) cm[offCn[n + 1]] = acc[i][j][1];
+                    if (n < N && offCn[n] >= 0) cm[offCn[n]] = acc[i][j][0];
+                    if (n + 1 < N && offCn[n + 1] >= 0) cm[offCn[n + 1]] = acc[i][j][1];
                 }
             }
 #pragma unroll
@@ -808,10 +810,10 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     int l_sub = 0, l_c = 0;                          // next chunk to request: product l_sub, chunk l_c of it
     // every thread copies the same m (pair of m) and n of each k-row it serves: offsets and bounds are fixed per item
     constexpr int AW = Map::A16 ? 2 : 1, ATPR = BM / AW, ARPP = NTH / ATPR, APASS = KC / ARPP;
-    constexpr int BTPR = BN, BRPP = NTH / BTPR, BPASS = KC / BRPP;
+    constexpr int BW = Map::B16 ? 2 : 1, BTPR = BN / BW, BRPP = NTH / BTPR, BPASS = KC / BRPP;
     static_assert(NTH % ATPR == 0 && KC % ARPP == 0 && NTH % BTPR == 0 && KC % BRPP == 0, "loader shape");
-    const int am = (tid % ATPR) * AW, akr = tid / ATPR, bn = tid % BTPR, bkr = tid / BTPR;
-    const int a_bytes = 8 * max(0, min(AW, M - am)), b_bytes = bn < N ? 8 : 0;
+    const int am = (tid % ATPR) * AW, akr = tid / ATPR, bn = (tid % BTPR) * BW, bkr = tid / BTPR;
+    const int a_bytes = 8 * max(0, min(AW, M - am)), b_bytes = 8 * max(0, min(BW, N - bn));
     const int a_off = a_bytes ? offAm[am] : 0, b_off = b_bytes ? offBn[bn] : 0;
     const unsigned a_dst = fz_smem_u32(As + akr * LDA + am), b_dst = fz_smem_u32(Bs + bkr * LDB + bn);
     auto load_chunk = [&](int gc) {
@@ -833,7 +835,11 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
             for (int it = 0; it < BPASS; ++it) {
                 const int kr = bkr + it * BRPP, k = k0 + kr;
                 const bool ok = b_bytes && k < K;
-                fz_cp_async8(b_dst + 8u * (unsigned)((s * KC + it * BRPP) * LDB), ok ? Bq + offBk[k] : B0, ok ? 8 : 0);
+                const unsigned dst = b_dst + 8u * (unsigned)((s * KC + it * BRPP) * LDB);
+                if (Map::B16)
+                    fz_cp_async16(dst, ok ? Bq + offBk[k] : B0, ok ? b_bytes : 0);
+                else
+                    fz_cp_async8(dst, ok ? Bq + offBk[k] : B0, ok ? 8 : 0);
             }
             if (++l_c == nchunks) {
                 l_c = 0;
