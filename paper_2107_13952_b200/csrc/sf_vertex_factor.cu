@@ -275,8 +275,16 @@ __global__ void __launch_bounds__(256) k_fz_g(FzParams p, long n, double* __rest
     const int o23 = p.box.lo[0] + b23, o24 = p.box.lo[1] + b24, o25 = p.box.lo[2] + b25;
     int x0, nxs, xg0;
     fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
+    // only the entries k_fz_gemm<FzMapA> reads: x of this (i1 l25), k3 allowed by (j13 l23) and by the triad (k3 l24 x)
+    if (v >= nxs) return;
+    {
+        const int2 wb = p.w3B[o23];
+        const int k3 = P.two_k_base[1] + 2 * q3, l24 = P.two_j[J24] + 2 * o24, x = x0 + 2 * v;
+        const int d = l24 > x ? l24 - x : x - l24;
+        if (q3 < wb.x || q3 >= wb.x + wb.y || k3 < d || k3 > l24 + x || ((l24 + x + k3) & 1)) return;
+    }
     double val = 0.0;
-    if (v < nxs) {
+    {
         const int blk = (o23 * nl + o24) * nl + o25;
         const SfKRange r2 = P.kr[0][blk];
         const int q2b = (r2.two_k_min - P.two_k_base[0]) >> 1;
@@ -795,8 +803,9 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
 #pragma unroll
                 for (int j = 0; j < TN; ++j) {
                     const int n = wn * TN * 8 + 8 * j + 2 * q;
-                    if (n < N && offCn[n] >= 0) cm[offCn[n]] = acc[i][j][0];
-                    if (n + 1 < N && offCn[n + 1] >= 0) cm[offCn[n + 1]] = acc[i][j][1];
+                    // maps whose columns include padding (B16) mark it with a negative offset
+                    if (n < N && (!Map::B16 || offCn[n] >= 0)) cm[offCn[n]] = acc[i][j][0];
+                    if (n + 1 < N && (!Map::B16 || offCn[n + 1] >= 0)) cm[offCn[n + 1]] = acc[i][j][1];
                 }
             }
 #pragma unroll
