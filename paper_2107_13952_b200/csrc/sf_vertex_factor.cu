@@ -345,9 +345,9 @@ __global__ void __launch_bounds__(32) k_fz_lists(FzParams p, int2* __restrict__ 
 // The triads of eq. (5) that contain x, (k4 l35 x) and (k3 l24 x), bound k4 and k3 for every x: only those k4 are
 // computed and only those rows k3 of P are written (k_fz_gemm reads exactly the same set, fz_vrange).
 #define FZ_QP_THREADS 256
-#define FZ_QKS 3      /* fast Q phase: c45 <= 12, n4 <= 16, (v, i5) rows of a pass <= 32 */
+#define FZ_QKS 3      /* fast Q phase: c45 <= 12, n4 <= 16, (v, i5) rows of a pass <= 40 */
 #define FZ_QNT 2
-#define FZ_QMT 4
+#define FZ_QMT 5
 #define FZ_PKS 6      /* fast P phase: k4 windows of at most 24 values */
 __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, long n_items)
 {
@@ -1008,20 +1008,24 @@ static FzShape fz_shape(const SfDims& D)
     s.W4p = (w4 + 3) & ~3;
     if (w3 == 0 || s.W4p == 0) return s;
     s.LDQ = ((n54 + 15) & ~15) + 8;                   // = 8 mod 16: conflict-free B fragments
-    // x values per pass: fill the 8-row tiles of (v, i5) as well as possible inside ~100 KB (two CTAs per SM); a single x
-    // may take up to 200 KB (one CTA per SM) before the path gives up
-    int best = 0;
+    // x values per pass.  Every pass costs two CTA barriers and a fixed amount of index work, so more x per pass is better
+    // as long as the 8-row tiles of (v, i5) stay well filled, the rows fit the fast Q phase (8 FZ_QMT) and two CTAs keep
+    // ~100 KB of the SM for L1: the largest vg inside 80 KB with fill >= 0.8, else the best-filled one; a single x may take up
+    // to 200 KB (one CTA per SM) before the path gives up.
+    int best = 0, best_any = 0;
     double best_fill = 0.0;
     for (int vg = 1; vg <= s.V; ++vg) {
         const size_t bytes = sizeof(double) * (size_t)vg * s.W4p * s.LDQ;
-        if (bytes > (vg == 1 ? 200 : 100) * 1024) break;
+        if (bytes > (vg == 1 ? 200 : 80) * 1024) break;
         const int rows = vg * D.n_i[4];
         const double fill = (double)rows / (((rows + 7) / 8) * 8);
         if (fill > best_fill + 1e-9) {
             best_fill = fill;
-            best = vg;
+            best_any = vg;
         }
+        if (fill >= 0.8 && (rows <= 8 * FZ_QMT || best == 0)) best = vg;
     }
+    if (best == 0) best = best_any;
     if (best == 0) return s;
     s.VG = best;
     s.qp_smem = sizeof(double) * (size_t)s.VG * s.W4p * s.LDQ;
