@@ -40,7 +40,7 @@ METRIC = "eprl_shells_contracted_per_s"
 PATH_NAMES = {1: "staged", 2: "fused", 3: "line", 4: "factorised"}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch (the heaviest of the three passes over i1) from the committed
 # `ncu --set full` captures of config 3, profiles/r1e_factorised.md; null for any other workload
-NCU_TRAFFIC_CONFIG3 = {"k_fz_qp": 15.29e9, "k_fz_gemm<FzMapR>": 24.15e9, "k_fz_gemm<FzMapA>": 8.73e9}   # r1e, r1g
+NCU_TRAFFIC_CONFIG3 = {"k_fz_qp": 15.13e9, "k_fz_gemm<FzMapR>": 24.15e9, "k_fz_gemm<FzMapA>": 8.73e9}   # r1e, r1g, r1h
 UNIT = "shells/s"
 
 
