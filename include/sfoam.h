@@ -31,6 +31,11 @@
  * (released by sf_finalize).  All functions return SF_OK (0) or a negative sf_status; none throws or aborts; `out` is
  * not written when an error is returned before launch.  There is NO CPU fallback: without a CUDA device every compute
  * entry point returns SF_ECUDA.
+ *
+ * Concurrency: one context per process, bound to the device that was current at sf_init; the library keeps its scratch
+ * buffers and path selection in that context, so calls must not overlap (issue them from one thread, or serialise them).
+ * Calls are asynchronous on the stream they are given; two vertex calls on different streams share the scratch buffers and
+ * must be ordered by the caller.
  */
 #ifndef SFOAM_H
 #define SFOAM_H
