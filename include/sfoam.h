@@ -159,6 +159,9 @@ int sf_last_kernel_ms(double ms[4]);
  * included; sf_last_dmma returns the counts of the last vertex call, same order as ms[0..2] above.  Measurement only: the
  * call becomes synchronous and slightly slower; the result is unchanged. */
 int sf_set_counting(int on);
+/* Debug aid of the factorised path: when on, its intermediate arrays (Z, G, P, R) are filled with NaN bit patterns before
+ * they are produced, so that reading an entry nobody wrote shows up as a NaN in the tensor.  The result must not change. */
+int sf_set_debug_poison(int on);
 int sf_last_dmma(double n[3]);
 
 /* Path selection for steps 5-7.  All paths compute the same sum of eq. (3); they differ in the

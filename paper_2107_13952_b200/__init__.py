@@ -136,6 +136,10 @@ def sf_set_counting(on):
     _check(_lib().sf_set_counting(int(bool(on))), "sf_set_counting")
 
 
+def sf_set_debug_poison(on):
+    _check(_lib().sf_set_debug_poison(int(bool(on))), "sf_set_debug_poison")
+
+
 def sf_last_dmma():
     """Factorised path: DMMA.8x8x4 warp instructions issued by [k_fz_qp, k_fz_gemm<FzMapR>, k_fz_gemm<FzMapA>] in the last
     vertex call made with sf_set_counting(True)."""

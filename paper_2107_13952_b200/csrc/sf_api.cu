@@ -20,6 +20,7 @@ struct SfContext {
     int last_path = 0;
     bool timing = false;
     bool counting = false;
+    bool poison = false;
     cudaEvent_t ev[4] = {};
     double stage_ms[3] = {};
 };
@@ -50,6 +51,7 @@ void* sf_scratch(int slot, size_t bytes)
 
 bool sf_timing_on(void) { return g_ctx.timing; }
 bool sf_counting_on(void) { return g_ctx.counting; }
+bool sf_poison_on(void) { return g_ctx.poison; }
 
 void sf_timing_mark(int idx, cudaStream_t st)
 {
@@ -129,6 +131,11 @@ extern "C" int sf_set_timing(int on)
 extern "C" int sf_set_counting(int on)
 {
     g_ctx.counting = on != 0;
+    return SF_OK;
+}
+extern "C" int sf_set_debug_poison(int on)
+{
+    g_ctx.poison = on != 0;
     return SF_OK;
 }
 extern "C" int sf_last_stage_ms(double ms[3])

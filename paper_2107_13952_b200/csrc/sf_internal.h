@@ -112,6 +112,7 @@ void* sf_scratch(int slot, size_t bytes);
 void sf_count_launch(int n);
 bool sf_timing_on(void);
 bool sf_counting_on(void);
+bool sf_poison_on(void);
 void sf_timing_mark(int idx, cudaStream_t st);   // records event idx of the stage timing when it is enabled
 void sf_launch_finalize(const SfProblem& P, long n_out, const double* acc, double* out, cudaStream_t st);
 

@@ -1210,6 +1210,10 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         p.Rq = Rq;
         p.a_lo = 0;
         p.a_cnt = n1;
+        if (sf_poison_on()) {                        // debug: an entry read without having been written becomes a NaN
+            SF_CUDA_OK(cudaMemsetAsync(Z, 0xFF, sizeof(double) * (size_t)nZ, st));
+            SF_CUDA_OK(cudaMemsetAsync(G, 0xFF, sizeof(double) * (size_t)nG, st));
+        }
         fz_ev_begin(3, st);
         k_fz_z<<<(unsigned)(c25 * n1 * c35 * c45), 256, 0, st>>>(p, Z);
         k_fz_b4t<<<(unsigned)((nB4 + 255) / 256), 256, 0, st>>>(p, nB4, B4);
@@ -1222,6 +1226,10 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         for (int a_lo = 0; a_lo < n1; a_lo += (int)na) {
             p.a_lo = a_lo;
             p.a_cnt = (int)(a_lo + na <= n1 ? na : n1 - a_lo);
+            if (sf_poison_on()) {
+                SF_CUDA_OK(cudaMemsetAsync(Pq, 0xFF, sizeof(double) * (size_t)(pP * na), st));
+                SF_CUDA_OK(cudaMemsetAsync(Rq, 0xFF, sizeof(double) * (size_t)(pR * na), st));
+            }
             fz_ev_begin(0, st);
             {
                 const long n_items = (long)p.a_cnt * c25 * c35 * c24 * c34;

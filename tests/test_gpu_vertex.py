@@ -307,6 +307,38 @@ def test_reduced_intertwiner_ranges(path, which):
         assert e.value.status == sf.SF_EARG
 
 
+def test_factorised_path_reads_only_what_it_wrote():
+    """The intermediates of the factorised path are written and read through the same range predicates; with the arrays
+    pre-filled with NaN patterns (sf_set_debug_poison) the tensor must come out bit for bit the same."""
+    cases = [wl.CONFIGS[0], wl.config2(3), wl.config1(5), dict(two_j=[4, 3, 1, 4, 2, 5, 5, 5, 4, 3], two_dl=4, boosters="random", seed=77),
+             _config4(2)]
+    sf.sf_set_path(4)
+    try:
+        for cfg in cases:
+            B = boosters_for(cfg)
+            Bdev = to_device(B)
+            n = (cfg["two_dl"] // 2 + 1) ** 6
+            for lo, hi in [(None, None), (n // 3, n // 3 + 57 if n > 100 else n)]:
+                clean = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+                sf.sf_set_debug_poison(True)
+                poisoned = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+                sf.sf_set_debug_poison(False)
+                assert np.isfinite(poisoned).all() and np.array_equal(clean, poisoned), cfg.get("name")
+        # the headline workload on one block of shells and on a ragged range
+        cfg = wl.CONFIGS[3]
+        B = boosters_for(cfg)
+        Bdev = to_device(B)
+        for lo, hi in [(11 ** 3 * 40, 11 ** 3 * 41), (11 ** 5 * 7 - 300, 11 ** 5 * 7 + 900)]:
+            clean = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+            sf.sf_set_debug_poison(True)
+            poisoned = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+            sf.sf_set_debug_poison(False)
+            assert np.array_equal(clean, poisoned)
+    finally:
+        sf.sf_set_debug_poison(False)
+        sf.sf_set_path(0)
+
+
 def test_errors(path):
     two_j = [2] * 10
     B = to_device(boosters_for(wl.CONFIGS[0]))
