@@ -362,6 +362,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, lo
     const int NT = (n54 + 7) >> 3, NT4 = (n4 + 7) >> 3, KS45 = (c45 + 3) >> 2, NTQ = (NT + 3) >> 2;
     const int sZ = P4 * V * n5, c2434n4 = c24 * c34 * n4;
     const long prow = (long)c34 * c35 * NP;          // stride of v in P
+    const float inv_ntq = 1.0f / (float)NTQ;
     const bool fastq = KS45 <= FZ_QKS && NT4 <= FZ_QNT && ((VG * n5 + 7) >> 3) <= FZ_QMT;
     const bool fastp = W4p <= 4 * FZ_PKS;
     double* Qs = smem;                               // [VG][W4p][LDQ]
@@ -405,6 +406,7 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, lo
         const int lo4 = max(w4a.x, p.hull4B.x);
         const int w4 = max(0, min(w4a.x + w4a.y, p.hull4B.y) - lo4);
         const int MT3 = (w3.y + 7) >> 3;
+        const float inv_mt3 = 1.0f / (float)MT3;
         const double* Zb = p.Z + ((((long)b25 * n1 + a1) * c35 + b35) * c45) * (long)sZ;
         const double* S3b = p.S3T + ((((long)b24 * c34 + b34) * c35 + b35) * NX + xg0) * (long)(P3 * P4) + (long)w3.x * P4 + lo4;
         const double* B4b = p.Bw4T + ((long)b24 * c34 + b34) * n4;
@@ -512,7 +514,10 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, lo
             }
             // ---- P phase: one A fragment (S3, straight from L1/L2) feeds four column tiles of Q ----
             for (int task = warp; task < nv * MT3 * NTQ; task += NW) {
-                const int ntq = task % NTQ, t2 = task / NTQ, mt3 = t2 % MT3, vv = t2 / MT3;
+                // task = (vv MT3 + mt3) NTQ + ntq; quotients of small integers through one float multiply (exact: the
+                // fractional part of (t + 0.5) / d is at least 0.5 / d, far above the rounding error)
+                const int t2 = __float2int_rz(((float)task + 0.5f) * inv_ntq), ntq = task - t2 * NTQ;
+                const int vv = __float2int_rz(((float)t2 + 0.5f) * inv_mt3), mt3 = t2 - vv * MT3;
                 // rows k3 the triad (k3 l24 x) allows for this x
                 const int2 wx = fz_window(l24, x0 + 2 * (v0 + vv), P.two_k_base[1], P3);
                 const int rlo = max(wx.x, w3.x) - w3.x, rhi = wx.y > 0 ? min(wx.x + wx.y, w3.x + w3.y) - w3.x : 0;
