@@ -307,6 +307,20 @@ def test_reduced_intertwiner_ranges(path, which):
         assert e.value.status == sf.SF_EARG
 
 
+def test_many_shells_small_spins(path):
+    """Delta_l = 13 on j = 1 (14 values per virtual spin, 7.5 M shells; most of them empty): more than 12 offsets per
+    spin takes the general-size branch of the factorised Q phase."""
+    cfg = dict(two_j=[2] * 10, two_dl=26, boosters="random", seed=4242)
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    nl3 = 14 ** 3
+    for lo, hi in [(3, 203), (0, nl3), (nl3 * 15 + 7, nl3 * 16 + 500)]:
+        Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+        Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, hi)
+        assert np.abs(Ao).max() > 0
+        assert_parity(Ag, Ao, Aabs, what=f"j=1 dl=13 shells [{lo},{hi})")
+
+
 def test_factorised_path_reads_only_what_it_wrote():
     """The intermediates of the factorised path are written and read through the same range predicates; with the arrays
     pre-filled with NaN patterns (sf_set_debug_poison) the tensor must come out bit for bit the same."""
