@@ -214,6 +214,53 @@ def bench_contractions(torch, sf, stream):
     return out
 
 
+def bench_other_workloads(torch, sf, stream):
+    """The other four workloads of BASELINE.json in full (north_star: throughput on all five), each a few asynchronous calls
+    between two CUDA events: config 0, config 1 at j = 10 (identity boosters, A = N(i) {15j}), config 2 at Delta_l = 8,
+    config 4 at lambda = 1..6.  Secondary rows: the headline stays config 3."""
+    def valid(two_j):
+        try:
+            sf.sf_vertex_dims(two_j)
+            return True
+        except sf.SfError:
+            return False
+
+    base, _ = wl.config4_base_spins(valid)
+    cases = [wl.CONFIGS[0], wl.config1(20), wl.config2(8)] + [wl.config4(base, lam) for lam in range(1, 7)]
+    rows = []
+    for c in cases:
+        two_j, two_dl = c["two_j"], c["two_dl"]
+        nl = two_dl // 2 + 1
+        edge_dims, k_ranges = {}, {}
+        for edge in (2, 3, 4, 5):
+            _, n_i_e, kbase, pad = sf.sf_booster_dims(two_j, two_dl, edge)
+            edge_dims[edge] = (n_i_e, kbase, pad)
+            k_ranges[edge] = sf.sf_booster_kranges(two_j, two_dl, edge)
+        lo, n_i = sf.sf_vertex_dims(two_j)
+        if c["boosters"] == "identity":
+            B = wl.identity_boosters(edge_dims, lo)
+        else:
+            B = wl.random_boosters(c["seed"], nl, edge_dims, k_ranges)
+        Bdev = [torch.from_numpy(np.ascontiguousarray(B[e])).cuda() for e in (2, 3, 4, 5)]
+        out = torch.zeros(tuple(n_i), dtype=torch.float64, device="cuda")
+        sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)          # warm-up (sizes the scratch buffers)
+        sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)
+        torch.cuda.synchronize()
+        reps = 10 if nl ** 6 * int(np.prod(n_i)) < 10 ** 10 else 2
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        rows.append({"workload": c["name"], "shells": nl ** 6, "out_shape": list(n_i), "ms_per_tensor": ms,
+                     "shells_per_s": nl ** 6 / (ms * 1e-3), "tensors_per_s": 1e3 / ms,
+                     "path": PATH_NAMES.get(sf.sf_last_path(), "?"), "finite": bool(torch.isfinite(out).all())})
+        del Bdev, out
+    return rows
+
+
 def run_ours(args, cfg, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -383,6 +430,8 @@ def run_ours(args, cfg, rank, world, local_rank):
     }
     if world == 1:
         line["contractions"] = bench_contractions(torch, sf, stream)
+        if cfg["name"] == wl.CONFIGS[3]["name"] and args.path == 0:
+            line["other_workloads"] = bench_other_workloads(torch, sf, stream)
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         n_sample = min(args.ref_shells, n_shells)
