@@ -345,10 +345,10 @@ __global__ void __launch_bounds__(32) k_fz_lists(FzParams p, int2* __restrict__ 
 // The triads of eq. (5) that contain x, (k4 l35 x) and (k3 l24 x), bound k4 and k3 for every x: only those k4 are
 // computed and only those rows k3 of P are written (k_fz_gemm reads exactly the same set, fz_vrange).
 #define FZ_QP_THREADS 256
-#define FZ_QKS 3      /* fast Q phase: c45 <= 12, n4 <= 16, (v, i5) rows of a pass <= 40 */
+#define FZ_QKS 3      /* fast Q phase: c45 <= 12, (v, i5) rows of a pass <= 40; i4 in groups of FZ_QNT column tiles */
 #define FZ_QNT 2
 #define FZ_QMT 5
-#define FZ_PKS 6      /* fast P phase: k4 windows of at most 24 values */
+#define FZ_PKS 6      /* P phase: S3 fragments of 6 k-steps (24 values of k4) are loaded together */
 __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, long n_items)
 {
     extern __shared__ __align__(16) double smem[];
@@ -363,21 +363,16 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, lo
     const int sZ = P4 * V * n5, c2434n4 = c24 * c34 * n4;
     const long prow = (long)c34 * c35 * NP;          // stride of v in P
     const float inv_ntq = 1.0f / (float)NTQ;
-    const bool fastq = KS45 <= FZ_QKS && NT4 <= FZ_QNT && ((VG * n5 + 7) >> 3) <= FZ_QMT;
-    const bool fastp = W4p <= 4 * FZ_PKS;
+    const bool fastq = KS45 <= FZ_QKS && ((VG * n5 + 7) >> 3) <= FZ_QMT;
     double* Qs = smem;                               // [VG][W4p][LDQ]
     for (int z = tid; z < VG * W4p * LDQ; z += FZ_QP_THREADS) Qs[z] = 0.0;   // rows never written must stay finite
     // constants of the CTA: this lane's fragment offsets inside one k4 block of Bw4T / of Z, its C rows in Qs (-1: none)
-    int bofs[FZ_QNT][FZ_QKS], zofs[FZ_QMT][FZ_QKS], qrow[FZ_QMT];
+    int bofs[FZ_QKS], zofs[FZ_QMT][FZ_QKS], qrow[FZ_QMT];
 #pragma unroll
     for (int ks = 0; ks < FZ_QKS; ++ks) {
         const int b45 = 4 * ks + q;
         const bool kin = ks < KS45 && b45 < c45;
-#pragma unroll
-        for (int nt = 0; nt < FZ_QNT; ++nt) {
-            const int i4 = nt * 8 + g;
-            bofs[nt][ks] = (kin && nt < NT4 && i4 < n4) ? b45 * c2434n4 + i4 : -1;
-        }
+        bofs[ks] = kin ? b45 * c2434n4 + g : -1;
 #pragma unroll
         for (int mt = 0; mt < FZ_QMT; ++mt) zofs[mt][ks] = kin ? b45 * sZ + mt * 8 + g : -1;
     }
@@ -435,30 +430,35 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, lo
                     const double* zq = Zb + ((long)q4 * V + v0) * n5;
                     const double* bq = B4b + (long)q4 * c45 * c2434n4;
                     ndm += MT * NT4 * KS45;
-                    double a[FZ_QMT][FZ_QKS], b[FZ_QNT][FZ_QKS];
+                    double a[FZ_QMT][FZ_QKS];
 #pragma unroll
-                    for (int ks = 0; ks < FZ_QKS; ++ks) {
-#pragma unroll
-                        for (int nt = 0; nt < FZ_QNT; ++nt) b[nt][ks] = bofs[nt][ks] >= 0 ? __ldg(bq + bofs[nt][ks]) : 0.0;
+                    for (int ks = 0; ks < FZ_QKS; ++ks)
 #pragma unroll
                         for (int mt = 0; mt < FZ_QMT; ++mt)
                             a[mt][ks] = (zofs[mt][ks] >= 0 && mt * 8 + g < rows) ? __ldg(zq + zofs[mt][ks]) : 0.0;
-                    }
+                    for (int ntc = 0; ntc < NT4; ntc += FZ_QNT) {           // FZ_QNT column tiles of i4 at a time
+                        double b[FZ_QNT][FZ_QKS];
 #pragma unroll
-                    for (int mt = 0; mt < FZ_QMT; ++mt) {
-                        if (mt >= MT) break;
-                        double* dst = Qs + qrow[mt] + r4 * LDQ;
-                        const bool okm = mt * 8 + g < rows;
+                        for (int ks = 0; ks < FZ_QKS; ++ks)
 #pragma unroll
-                        for (int nt = 0; nt < FZ_QNT; ++nt) {
-                            if (nt >= NT4) break;
-                            double c0 = 0.0, c1 = 0.0;
+                            for (int nt = 0; nt < FZ_QNT; ++nt)
+                                b[nt][ks] = (bofs[ks] >= 0 && (ntc + nt) * 8 + g < n4) ? __ldg(bq + bofs[ks] + (ntc + nt) * 8) : 0.0;
 #pragma unroll
-                            for (int ks = 0; ks < FZ_QKS; ++ks)
-                                if (ks < KS45) fz_dmma(c0, c1, a[mt][ks], b[nt][ks]);
-                            const int j4 = nt * 8 + 2 * q;
-                            if (okm && j4 < n4) dst[nt * 8] = c0;
-                            if (okm && j4 + 1 < n4) dst[nt * 8 + 1] = c1;
+                        for (int mt = 0; mt < FZ_QMT; ++mt) {
+                            if (mt >= MT) break;
+                            double* dst = Qs + qrow[mt] + r4 * LDQ + ntc * 8;
+                            const bool okm = mt * 8 + g < rows;
+#pragma unroll
+                            for (int nt = 0; nt < FZ_QNT; ++nt) {
+                                if (ntc + nt >= NT4) break;
+                                double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                                for (int ks = 0; ks < FZ_QKS; ++ks)
+                                    if (ks < KS45) fz_dmma(c0, c1, a[mt][ks], b[nt][ks]);
+                                const int j4 = (ntc + nt) * 8 + 2 * q;
+                                if (okm && j4 < n4) dst[nt * 8] = c0;
+                                if (okm && j4 + 1 < n4) dst[nt * 8 + 1] = c1;
+                            }
                         }
                     }
                 }
@@ -531,28 +531,21 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, lo
                 double c[4][2];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) c[j][0] = c[j][1] = 0.0;
-                if (fastp) {
-                    double av[FZ_PKS];
+                for (int kc = k4a; kc < k4b; kc += 4 * FZ_PKS) {          // FZ_PKS k-steps at a time: their S3 fragments are
+                    double av[FZ_PKS];                                     // requested together, before the first MMA
 #pragma unroll
                     for (int i = 0; i < FZ_PKS; ++i) {
-                        const int ks = k4a + 4 * i;
+                        const int ks = kc + 4 * i;
                         av[i] = (ks < k4b && rok && ks + q < w4) ? __ldg(ap + ks) : 0.0;
                     }
 #pragma unroll
                     for (int i = 0; i < FZ_PKS; ++i) {
-                        const int ks = k4a + 4 * i;
+                        const int ks = kc + 4 * i;
                         if (ks < k4b) {
 #pragma unroll
                             for (int j = 0; j < 4; ++j)
                                 if (j < ntl) fz_dmma(c[j][0], c[j][1], av[i], bp[ks * LDQ + 8 * j]);
                         }
-                    }
-                } else {
-                    for (int ks = k4a; ks < k4b; ks += 4) {
-                        const double av = (rok && ks + q < w4) ? __ldg(ap + ks) : 0.0;
-#pragma unroll
-                        for (int j = 0; j < 4; ++j)
-                            if (j < ntl) fz_dmma(c[j][0], c[j][1], av, bp[ks * LDQ + 8 * j]);
                     }
                 }
                 if (r3 >= rlo && r3 < rhi) {
