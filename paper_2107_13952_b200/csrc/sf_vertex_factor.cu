@@ -561,12 +561,13 @@ __global__ void __launch_bounds__(FZ_QP_THREADS, 2) k_fz_qp(const FzParams p, lo
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// k_fz_gemm: gather-GEMM  C[offCm[m] + offCn[n]] = sum_kk A[offAk[kk] + offAm[m]] B[offBk[kk] + offBn[n]]
+// k_fz_gemm: gather-GEMM  C[offCm[m] + offCn[n]] = sum_kk A[kA kix[kk] + offAm[m]] B[kB kix[kk] + offBn[n]]
 // ---------------------------------------------------------------------------------------------------------
 struct FzGemmHdr {
     int M, N, K;
     int nsub;                   // products that share the index tables: A, B and C advance by sA, sB, sC
     long baseA, baseB, baseC, sA, sB, sC;
+    int kA, kB;                 // strides of the k list: entry kk of the list sits at kA * kix[kk] in A, kB * kix[kk] in B
 };
 
 // R[l24 l25 i1; k3 x; l23 i3; (i5 i4)] = sum over the pairs (l34 l35) that allow k3 of P[..][(l34 l35)][(i5 i4)] Bw3T[k3][(l34 l35)][(l23 i3)]
@@ -584,7 +585,7 @@ struct FzMapR {
         return ntn * ntm * p.P.n_k_pad[1] * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
     }
     static __device__ void setup(const FzParams& p, long item, int BM, int BN, FzGemmHdr* h, int* offAm, int* offCm,
-                                 int* offBn, int* offCn, int* offAk, int* offBk, int* tmp)
+                                 int* offBn, int* offCn, int* kix, int* tmp)
     {
         const SfProblem& P = p.P;
         const int n3 = P.n_i[2], n54 = P.n_i[3] * P.n_i[4], P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
@@ -616,6 +617,8 @@ struct FzMapR {
             h->sA = (long)c34 * c35 * NP;
             h->sB = 0;
             h->sC = (long)c23 * n3 * NP;
+            h->kA = NP;
+            h->kB = c23 * n3;
         }
         if (M <= 0) return;
         for (int m = threadIdx.x; m < BM; m += blockDim.x) offAm[m] = offCm[m] = m;
@@ -625,8 +628,7 @@ struct FzMapR {
         }
         for (int kk = threadIdx.x; kk < K; kk += blockDim.x) {
             const int c = list[1 + kk];
-            offAk[kk] = c * NP;
-            offBk[kk] = c * c23 * n3;
+            kix[kk] = c;
         }
     }
 };
@@ -645,7 +647,7 @@ struct FzMapA {
         return ntn * ntm * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
     }
     static __device__ void setup(const FzParams& p, long item, int BM, int BN, FzGemmHdr* h, int* offAm, int* offCm,
-                                 int* offBn, int* offCn, int* offAk, int* offBk, int* tmp)
+                                 int* offBn, int* offCn, int* kix, int* tmp)
     {
         const SfProblem& P = p.P;
         const int n1 = P.n_i[0], n2 = P.n_i[1], n3 = P.n_i[2], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5, n345 = n3 * n54;
@@ -685,6 +687,8 @@ struct FzMapA {
             h->baseB = (((long)ac * c24 + b24) * c25 + b25) * ((long)P3 * V * c23 * n3 * NP);
             h->baseC = ((p.part0 + (long)b24 * c25 + b25) * n1 + a1) * ((long)n2 * n345);
             h->sA = h->sB = h->sC = 0;
+            h->kA = n2;
+            h->kB = n3 * NP;
         }
         for (int m = threadIdx.x; m < BM; m += blockDim.x) {
             offAm[m] = m0 + m;
@@ -704,8 +708,7 @@ struct FzMapA {
             const int at = tmp[q3] + vi * win.y;
             for (int b = 0; b < win.y; ++b) {
                 const int row = (q3 * V + v) * c23 + win.x + b;
-                offAk[at + b] = row * n2;
-                offBk[at + b] = row * n3 * NP;
+                kix[at + b] = row;
             }
         }
     }
@@ -763,11 +766,10 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     int* offBn = offCm + BM;
     int* offCn = offBn + BN;
     int* tmp = offCn + BN;                           // 240 ints of scratch for the setup
-    int* offAk = tmp + 240;
-    int* offBk = offAk + kcap;
+    int* kix = tmp + 240;                            // the k list (kcap entries)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
     const int wm = warp / WGN, wn = warp % WGN;
-    Map::setup(p, blockIdx.x, BM, BN, &hdr, offAm, offCm, offBn, offCn, offAk, offBk, tmp);
+    Map::setup(p, blockIdx.x, BM, BN, &hdr, offAm, offCm, offBn, offCn, kix, tmp);
     __syncthreads();
     const int M = hdr.M, N = hdr.N, K = hdr.K, nsub = hdr.nsub;
     if (M <= 0) return;
@@ -777,6 +779,7 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     const double* B = B0 + hdr.baseB;
     double* C = Map::dstC(p) + hdr.baseC;
     const long sA = hdr.sA, sB = hdr.sB, sC = hdr.sC;
+    const long kA = hdr.kA, kB = hdr.kB;
     const int nchunks = (K + KC - 1) / KC, total = nsub * nchunks;
     int tma = 0, tna = 0;                            // live 8-row / 8-column tiles of this warp
 #pragma unroll
@@ -834,9 +837,9 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
                 const bool ok = a_bytes && k < K;
                 const unsigned dst = a_dst + 8u * (unsigned)((s * KC + it * ARPP) * LDA);
                 if (Map::A16)
-                    fz_cp_async16(dst, ok ? Aq + offAk[k] : A0, ok ? a_bytes : 0);
+                    fz_cp_async16(dst, ok ? Aq + kA * kix[k] : A0, ok ? a_bytes : 0);
                 else
-                    fz_cp_async8(dst, ok ? Aq + offAk[k] : A0, ok ? 8 : 0);
+                    fz_cp_async8(dst, ok ? Aq + kA * kix[k] : A0, ok ? 8 : 0);
             }
 #pragma unroll
             for (int it = 0; it < BPASS; ++it) {
@@ -844,9 +847,9 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
                 const bool ok = b_bytes && k < K;
                 const unsigned dst = b_dst + 8u * (unsigned)((s * KC + it * BRPP) * LDB);
                 if (Map::B16)
-                    fz_cp_async16(dst, ok ? Bq + offBk[k] : B0, ok ? b_bytes : 0);
+                    fz_cp_async16(dst, ok ? Bq + kB * kix[k] : B0, ok ? b_bytes : 0);
                 else
-                    fz_cp_async8(dst, ok ? Bq + offBk[k] : B0, ok ? 8 : 0);
+                    fz_cp_async8(dst, ok ? Bq + kB * kix[k] : B0, ok ? 8 : 0);
             }
             if (++l_c == nchunks) {
                 l_c = 0;
@@ -1031,7 +1034,7 @@ static FzShape fz_shape(const SfDims& D)
     const double slab = (double)D.n_k_pad[1] * s.V * D.nl * D.n_i[2] * s.NP;
     if (slab > 2.0e9 || (double)D.n_out / D.n_i[0] > 2.0e9) return s;
     // the k list of A' (one entry per (k3, x, l23)) lives in shared memory beside the operand ring of k_fz_gemm<FzMapA>
-    if ((long)D.n_k_pad[1] * s.V * D.nl > 14700) return s;    // 226 KB - 110.6 KB ring - 3.1 KB tables = 8 B x 14 712 entries
+    if ((long)D.n_k_pad[1] * s.V * D.nl > 26000) return s;    // 226 KB - 116.7 KB ring - 3.4 KB tables = 4 B x 27 100 entries
     s.ok = true;
     return s;
 }
@@ -1042,7 +1045,7 @@ template <class Map, int WGM, int WGN, int TM, int TN>
 static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
 {
     constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8;
-    const size_t smem = sizeof(double) * Map::ST * Map::KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 240 + 2 * (size_t)kcap);
+    const size_t smem = sizeof(double) * Map::ST * Map::KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 240 + (size_t)kcap);
     if (smem > 226 * 1024) return SF_EARG;
     static size_t attr = 0;
     if (smem > attr) {
@@ -1241,7 +1244,8 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             fz_ev_end(st);
             if (rc != SF_OK) return rc;
             fz_ev_begin(2, st);
-            rc = fz_launch_gemm<FzMapA, 1, 8, 2, 4>(p, (int)(P3 * sh.V * c23), st);
+            rc = n2 <= 16 ? fz_launch_gemm<FzMapA, 1, 8, 2, 4>(p, (int)(P3 * sh.V * c23), st)      // rows i2: one tile of 16
+                          : fz_launch_gemm<FzMapA, 1, 8, 4, 4>(p, (int)(P3 * sh.V * c23), st);     // or of 32: R is read once
             fz_ev_end(st);
             if (rc != SF_OK) return rc;
         }
