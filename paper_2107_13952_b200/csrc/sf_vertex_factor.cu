@@ -134,6 +134,35 @@ __device__ __forceinline__ void fz_cp_wait()
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
+// mbarrier / bulk-copy primitives (PTX ISA: mbarrier, cp.async.bulk; SASS UBLKCP)
+__device__ __forceinline__ void fz_mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void fz_mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void fz_mbar_wait(unsigned bar, unsigned parity)
+{
+    unsigned done = 0;
+    for (unsigned spin = 0; !done; ++spin) {
+        asm volatile(
+            "{\n.reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(done)
+            : "r"(bar), "r"(parity)
+            : "memory");
+        if (spin > (1u << 28)) __trap();   // a lost signal must fail the launch, never hang the device
+    }
+}
+__device__ __forceinline__ void fz_bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
 __device__ __forceinline__ void fz_prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -575,6 +604,7 @@ struct FzGemmHdr {
 // every x of (i1 l25) in turn
 struct FzMapR {
     static constexpr bool A16 = true, B16 = false;
+    static constexpr bool ABULK = true;  // the m-tile of a row of P is one contiguous, 16-byte aligned run: one bulk copy per k row
     static constexpr int CNT = 1, KC = 32, ST = 2;    // rows of P start 16-byte aligned (NP even) and m runs contiguously: copy pairs
     static __device__ const double* srcA(const FzParams& p) { return p.Pq; }
     static __device__ const double* srcB(const FzParams& p) { return p.Bw3T; }
@@ -635,7 +665,7 @@ struct FzMapR {
 
 // A'[l24 l25; i1; i2; (i3 i4 i5)] = sum over (k3, x, l23) with k3 allowed by (j13 l23) of G[..][(k3 x l23)][i2] R[..][(k3 x l23)][(i3, i5 i4)]
 struct FzMapA {
-    static constexpr bool A16 = false;
+    static constexpr bool A16 = false, ABULK = false;
     static constexpr bool B16 = true;    // columns run over the padded rows of R (i3, NP): contiguous and 16-byte aligned pairs
     static constexpr int CNT = 2, KC = 16, ST = 3;
     static __device__ const double* srcA(const FzParams& p) { return p.G; }
@@ -759,6 +789,7 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     constexpr int KC = Map::KC, ST = Map::ST;        // k-chunk depth and ring stages
     extern __shared__ __align__(16) double smem[];
     __shared__ FzGemmHdr hdr;
+    __shared__ __align__(8) unsigned long long abar[4];      // ABULK: one mbarrier per stage (ST <= 4)
     double* As = smem;                               // [ST][KC][LDA], [k][m]
     double* Bs = As + ST * KC * LDA;       // [ST][KC][LDB], [k][n]
     int* offAm = (int*)(Bs + ST * KC * LDB);
@@ -769,6 +800,10 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     int* kix = tmp + 240;                            // the k list (kcap entries)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
     const int wm = warp / WGN, wn = warp % WGN;
+    if (Map::ABULK && tid == 0) {
+        for (int s = 0; s < ST; ++s) fz_mbar_init(fz_smem_u32(&abar[s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     Map::setup(p, blockIdx.x, BM, BN, &hdr, offAm, offCm, offBn, offCn, kix, tmp);
     __syncthreads();
     const int M = hdr.M, N = hdr.N, K = hdr.K, nsub = hdr.nsub;
@@ -831,15 +866,30 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
             const int s = gc % ST, k0 = l_c * KC;
             const double* Aq = A + l_sub * sA + a_off;
             const double* Bq = B + l_sub * sB + b_off;
+            if (Map::ABULK) {
+                // warp 0: one bulk copy per k row (the row's M entries, rounded up to 16 bytes), completion on the stage's
+                // mbarrier; rows past K of the last chunk are zeroed by hand (they are summed over)
+                const int kv = min(KC, K - k0);
+                const unsigned rowb = (unsigned)(((M + 1) & ~1) * 8);
+                if (warp == 0) {
+                    const unsigned bar = fz_smem_u32(&abar[s]);
+                    if (lane == 0) fz_mbar_expect_tx(bar, rowb * (unsigned)kv);
+                    __syncwarp();
+                    for (int kr = lane; kr < kv; kr += 32)
+                        fz_bulk_g2s(fz_smem_u32(As + (s * KC + kr) * LDA), A + l_sub * sA + kA * kix[k0 + kr], rowb, bar);
+                }
+                for (int e = tid; e < (KC - kv) * BM; e += NTH) As[(s * KC + kv + e / BM) * LDA + e % BM] = 0.0;
+            } else {
 #pragma unroll
-            for (int it = 0; it < APASS; ++it) {
-                const int kr = akr + it * ARPP, k = k0 + kr;
-                const bool ok = a_bytes && k < K;
-                const unsigned dst = a_dst + 8u * (unsigned)((s * KC + it * ARPP) * LDA);
-                if (Map::A16)
-                    fz_cp_async16(dst, ok ? Aq + kA * kix[k] : A0, ok ? a_bytes : 0);
-                else
-                    fz_cp_async8(dst, ok ? Aq + kA * kix[k] : A0, ok ? 8 : 0);
+                for (int it = 0; it < APASS; ++it) {
+                    const int kr = akr + it * ARPP, k = k0 + kr;
+                    const bool ok = a_bytes && k < K;
+                    const unsigned dst = a_dst + 8u * (unsigned)((s * KC + it * ARPP) * LDA);
+                    if (Map::A16)
+                        fz_cp_async16(dst, ok ? Aq + kA * kix[k] : A0, ok ? a_bytes : 0);
+                    else
+                        fz_cp_async8(dst, ok ? Aq + kA * kix[k] : A0, ok ? 8 : 0);
+                }
             }
 #pragma unroll
             for (int it = 0; it < BPASS; ++it) {
@@ -864,6 +914,7 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
     unsigned ndm = 0;                                // DMMA instructions of this warp (reported when p.cnt is set)
     for (int gc = 0; gc < total; ++gc) {
         fz_cp_wait<ST - 2>();
+        if (Map::ABULK) fz_mbar_wait(fz_smem_u32(&abar[gc % ST]), (unsigned)((gc / ST) & 1));
         __syncthreads();                             // chunk gc has landed; every warp is done with chunk gc - 1
         load_chunk(gc + ST - 1);              // refills the stage chunk gc - 1 used
         if (active) {
