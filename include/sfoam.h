@@ -27,6 +27,9 @@
  *     paper's column-major A^{i5 i4 i3 i2 i1}.
  *   - The result is bitwise reproducible run to run for identical inputs (fixed-order accumulation, no float atomics).
  *
+ * Measurement and debugging entry points (timers, counters, peak probes, memory-budget hooks) are NOT part of this
+ * contract: they live in include/sfoam_debug.h.
+ *
  * Ownership: the caller owns booster and output buffers; the library owns the {6j} table and its scratch memory
  * (released by sf_finalize).  All functions return SF_OK (0) or a negative sf_status; none throws or aborts; `out` is
  * not written when an error is returned before launch.  There is NO CPU fallback: without a CUDA device every compute
@@ -81,7 +84,9 @@ int sf_sixj_table_two_jmax(void);
 
 /* Test hooks for {6j} parity.  two_j6 = (a b c d e f) for {a b c; d e f}; HOST pointers.
  * sf_sixj_get evaluates one symbol on the device (direct Racah sum).  sf_sixj_batch evaluates n symbols;
- * mode 0 = direct evaluation, mode 1 = gather from the resident table (SF_ETABLE if absent or an argument exceeds it). */
+ * mode 0 = direct evaluation, mode 1 = gather from the resident table (SF_ETABLE if absent or an argument exceeds it).
+ * Accuracy of the direct evaluation: relative 1e-12 for every 2j <= 150, ~1e-9 at 2j = 200; arguments above 2j = 256 are
+ * refused (SF_EARG), and so is a vertex call whose largest {6j} label 2 * (max two_j + two_dl) exceeds 256. */
 int sf_sixj_get(const int two_j6[6], double *host_out);
 int sf_sixj_batch(const int *two_j6, long n, int mode, double *host_out);
 
@@ -100,17 +105,6 @@ int sf_booster_kranges(const int two_j[10], int two_dl, int edge, int *two_k_min
  * Host integer function. */
 int sf_vertex_work(const int two_j[10], int two_dl, long shell_lo, long shell_hi,
                    double *f_con, long *n_nonempty, double *n_w);
-
-/* Number of (entry, x) summands of eq. (5) over shells [shell_lo, shell_hi): the sum over the entries
- * (i1 k2 k3 k4 k5) of every non-empty shell of the size of the intersection of the five triads that contain x.  The
- * algorithmic assembly work is F_asm = 6 * n_terms (five multiplications by a {6j} or by (2x+1), one addition).
- * Counted by a device kernel (integer work, exact); synchronises the default stream.  Requires sf_init. */
-int sf_vertex_terms(const int two_j[10], int two_dl, long shell_lo, long shell_hi, double *n_terms);
-
-/* FP64 roofline denominators measured in this process: TFLOP/s of dependent-chain microbenchmarks,
- * kind 0 = DFMA (vector FP64 fused multiply-add), kind 1 = DMMA (mma.sync m8n8k4 f64 on the tensor cores).
- * Best of 5 launches of a few ms each; synchronises the default stream.  Requires sf_init. */
-int sf_fp64_peak(int kind, double *tflops);
 
 /* The vertex tensor (steps 4-7).  boosters / out: DEVICE pointers; out holds prod(n_i) doubles and
  * is overwritten.  Asynchronous w.r.t. the host, ordered on `stream`.  Requires sf_init. */
@@ -146,36 +140,19 @@ int sf_contract_vectors(const double *A, const int n_i[5], const double *const p
 
 /* Number of kernels the library launched since sf_init / the last reset (bench.py's gpu_launches). */
 long sf_launch_count(int reset);
-/* Milliseconds of device time (CUDA events on the call's stream) spent in each stage of the LAST vertex call,
- * recorded when sf_set_timing(1) is on: [0] S arrays (step 4), [1] assembly + contraction (steps 5-6(iii)),
- * [2] accumulation (step 6(iv) + normalisation).  Enabling timing makes the vertex calls synchronous. */
-int sf_set_timing(int on);
-int sf_last_stage_ms(double ms[3]);
-/* Factorised path only (sf_set_path): CUDA-event times of its kernels, summed over the launches of the last vertex call made
- * with sf_set_timing(1): ms[0] k_fz_qp (sums over l45 and k4), ms[1] k_fz_gemm<FzMapR> (sum over l34 l35, edge-3 product),
- * ms[2] k_fz_gemm<FzMapA> (sum over x, k3, l23, edge-2 product), ms[3] the precomputations (Z, weighted boosters, G). */
-int sf_last_kernel_ms(double ms[4]);
-/* sf_set_counting(1): the factorised kernels count the FP64 MMA instructions (DMMA.8x8x4, 512 flop each) they issue, padding
- * included; sf_last_dmma returns the counts of the last vertex call, same order as ms[0..2] above.  Measurement only: the
- * call becomes synchronous and slightly slower; the result is unchanged. */
-int sf_set_counting(int on);
-/* Debug aid of the factorised path: when on, its intermediate arrays (Z, G, P, R) are filled with NaN bit patterns before
- * they are produced, so that reading an entry nobody wrote shows up as a NaN in the tensor.  The result must not change. */
-int sf_set_debug_poison(int on);
-int sf_last_dmma(double n[3]);
-
 /* Path selection for steps 5-7.  All paths compute the same sum of eq. (3); they differ in the
  * order of the additions only.
- *   0 = automatic: the fastest path that supports the problem's sizes (4, else 3, else 2, else 1)
+ *   0 = automatic: the fastest path that supports the problem's sizes (4, else 3, else 1); when the chosen path runs out of
+ *       device memory the next one is tried
  *   1 = staged: per batch of shells, {15j} assembly and the four mode products as separate kernels with intermediates
  *       in global memory, split along i1 when needed; any size
- *   2 = fused: one kernel per chunk of shells, accumulators in registers, intermediates in shared memory
  *   3 = line: persistent per-shell kernel (x-sum of eq. (5) and the k4 product per shell, k3 / k2 products per line /
- *       block of shells by linearity); every intertwiner range <= 16 values
+ *       block of shells by linearity); every intertwiner range <= 16 values.  This is the implementation of the method as
+ *       the paper states it (one {15j} assembly and four mode products per shell)
  *   4 = factorised: the sums over the virtual spins are taken one spin at a time with x kept open (Q = sum_l45,
  *       R = sum_{l34 l35}, A' = sum_l23, A = sum_{l24 l25}); same terms, far fewer operations
- * The vertex calls return SF_EARG when the selected path cannot hold the problem.  sf_last_path() = path the last
- * vertex call took (1..4). */
+ * (2 was an earlier on-chip kernel, removed: SF_EARG.)  The vertex calls return SF_EARG when the selected path cannot hold
+ * the problem.  sf_last_path() = path the last vertex call took (1, 3 or 4). */
 int sf_set_path(int path);
 /* Pure host helper (no device needed): the boxes of shell offsets (o23 o24 o25 o34 o35 o45), o = l - j in units of 1, that
  * the factorised path splits the range [shell_lo, shell_hi) of the canonical shell order (eq. (9); l45
@@ -183,8 +160,6 @@ int sf_set_path(int path);
  * disjoint, in ascending shell order, their union is the range.  SF_EARG on a bad range or an odd / negative two_dl. */
 int sf_shell_boxes(int two_dl, long shell_lo, long shell_hi, int boxes[16][12], int* n_boxes);
 int sf_last_path(void);
-/* Bytes of global scratch the staged path may use for its two ping-pong buffers (default 6 GiB). */
-void sf_set_staged_budget(unsigned long bytes);
 
 #ifdef __cplusplus
 }

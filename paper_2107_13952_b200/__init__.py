@@ -53,6 +53,8 @@ def _lib():
                                        ctypes.POINTER(ctypes.c_double)]
         lib.sf_vertex_terms.argtypes = [_I10, ctypes.c_int, ctypes.c_long, ctypes.c_long,
                                         ctypes.POINTER(ctypes.c_double)]
+        lib.sf_factor_work.argtypes = [_I10, ctypes.c_int, ctypes.c_double * 6, ctypes.c_double * 4]
+        lib.sf_set_factor_budget.argtypes = [ctypes.c_size_t]
         lib.sf_fp64_peak.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
         lib.sf_vertex_amplitude.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_void_p,
                                             ctypes.c_void_p]
@@ -158,8 +160,9 @@ def sf_shell_boxes(two_dl, shell_lo, shell_hi):
 
 
 def sf_set_path(path):
-    """0 = automatic, 1 = staged (general sizes), 2 = first fused on-chip path, 3 = line path (on-chip, register
-    accumulation over lines of shells); 2 and 3 raise SF_EARG at call time for shapes they do not hold."""
+    """0 = automatic (factorised, else line, else staged), 1 = staged (any size), 3 = line (the per-shell method of the paper
+    on chip; intertwiner ranges <= 16 values), 4 = factorised; 3 and 4 raise SF_EARG at call time for shapes they do not
+    hold, 2 (a removed kernel) always."""
     _check(_lib().sf_set_path(int(path)), "sf_set_path")
 
 
@@ -169,6 +172,11 @@ def sf_last_path():
 
 def sf_set_staged_budget(nbytes):
     _lib().sf_set_staged_budget(int(nbytes))
+
+
+def sf_set_factor_budget(nbytes):
+    """Device bytes the factorised path may use for P and R of one pass over i1 (0 = default, a third of the device)."""
+    _lib().sf_set_factor_budget(int(nbytes))
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -250,6 +258,14 @@ def sf_vertex_terms(two_j, two_dl, shell_lo=0, shell_hi=None):
     _check(_lib().sf_vertex_terms(_spins(two_j), int(two_dl), int(shell_lo), int(shell_hi), ctypes.byref(n)),
            "sf_vertex_terms")
     return n.value
+
+
+def sf_factor_work(two_j, two_dl):
+    """Useful multiply-adds of the six contractions of the factorised path (Z, Q, P, R, G, A') and the structurally non-zero
+    entries of its intermediates (Z, Q, P, R), from the triangle inequalities only (host integer function)."""
+    mac, elems = (ctypes.c_double * 6)(), (ctypes.c_double * 4)()
+    _check(_lib().sf_factor_work(_spins(two_j), int(two_dl), mac, elems), "sf_factor_work")
+    return dict(zip(("Z", "Q", "P", "R", "G", "A"), mac)), dict(zip(("Z", "Q", "P", "R"), elems))
 
 
 def sf_fp64_peak(kind):

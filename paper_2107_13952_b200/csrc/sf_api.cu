@@ -16,7 +16,7 @@ struct SfContext {
     void* scratch[SF_NSCRATCH] = {};
     size_t scratch_bytes[SF_NSCRATCH] = {};
     long launches = 0;
-    int path = 0;          // 0 auto, 1 staged, 2 fused
+    int path = 0;          // sf_set_path: 0 automatic, 1 staged, 3 line, 4 factorised
     int last_path = 0;
     bool timing = false;
     bool counting = false;
@@ -144,10 +144,10 @@ extern "C" int sf_last_stage_ms(double ms[3])
     memcpy(ms, g_ctx.stage_ms, sizeof g_ctx.stage_ms);
     return SF_OK;
 }
-// 0 = automatic (fused on-chip path when the tensor fits, staged path otherwise), 1 = staged, 2 = fused
+// 0 = automatic (factorised, else line, else staged), 1 = staged, 3 = line, 4 = factorised (include/sfoam.h)
 extern "C" int sf_set_path(int path)
 {
-    if (path < 0 || path > 4) return SF_EARG;
+    if (path < 0 || path > 4 || path == 2) return SF_EARG;
     g_ctx.path = path;
     return SF_OK;
 }
@@ -242,11 +242,12 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
         D.n_out = n_out;
     }
     if (shell_lo < 0 || shell_hi > D.n_shells || shell_lo > shell_hi) return SF_EARG;
-    // largest factorial argument of any 6j on the path stays inside the table of sf_sixj.cuh
+    // every label of the {6j} of eq. (5) is a spin l <= j + Delta_l or a recoupling of two of them (k, x <= 2 (j + Delta_l)):
+    // the largest one must stay inside the validated accuracy envelope of the {6j} evaluation
     {
         int m = 0;
         for (int s = 0; s < 10; ++s) m = two_j[s] > m ? two_j[s] : m;
-        if (2 * (m + two_dl) + 2 >= 1000) return SF_EARG;
+        if (2 * (m + two_dl) > SF_SIXJ_MAX_TWO_J) return SF_EARG;
     }
 
     SfProblem P;
@@ -268,16 +269,18 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
     sf_timing_mark(1, st);
 
     // steps 5-7
-    const bool line_ok = sf_vertex_line_supported(D), fused_ok = sf_vertex_fused_supported(D);
-    const bool factor_ok = sf_vertex_factor_supported(D);
-    if ((g_ctx.path == 2 && !fused_ok) || (g_ctx.path == 3 && !line_ok) || (g_ctx.path == 4 && !factor_ok)) return SF_EARG;
-    int path = g_ctx.path;
-    if (path == 0) path = factor_ok ? 4 : line_ok ? 3 : fused_ok ? 2 : 1;
-    g_ctx.last_path = path;
-    rc = path == 4   ? sf_vertex_factor(D, P, shell_lo, shell_hi, out, st)
-         : path == 3 ? sf_vertex_line(D, P, shell_lo, shell_hi, out, st)
-         : path == 2 ? sf_vertex_fused(D, P, shell_lo, shell_hi, out, st)
-                     : sf_vertex_staged(D, P, shell_lo, shell_hi, out, st);
+    const bool line_ok = sf_vertex_line_supported(D), factor_ok = sf_vertex_factor_supported(D);
+    if ((g_ctx.path == 3 && !line_ok) || (g_ctx.path == 4 && !factor_ok)) return SF_EARG;
+    // automatic: the fastest path that holds the problem; a path that runs out of device memory hands over to the next
+    int path = g_ctx.path ? g_ctx.path : factor_ok ? 4 : line_ok ? 3 : 1;
+    for (;;) {
+        g_ctx.last_path = path;
+        rc = path == 4   ? sf_vertex_factor(D, P, shell_lo, shell_hi, out, st)
+             : path == 3 ? sf_vertex_line(D, P, shell_lo, shell_hi, out, st)
+                         : sf_vertex_staged(D, P, shell_lo, shell_hi, out, st);
+        if (rc != SF_ENOMEM || g_ctx.path != 0 || path == 1) break;
+        path = (path == 4 && line_ok) ? 3 : 1;
+    }
     if (rc != SF_OK) return rc;
     sf_timing_mark(3, st);
     if (g_ctx.timing) {

@@ -7,6 +7,7 @@
 #include <stdint.h>
 
 #include "../../include/sfoam.h"
+#include "../../include/sfoam_debug.h"
 
 // spin order of two_j[10] (Listing 8)
 enum { J12 = 0, J13, J14, J15, J23, J24, J25, J34, J35, J45 };
@@ -77,6 +78,11 @@ __host__ __device__ inline void sf_triples(const int o[6], int nl, int t[4])
 // -------------------------------------------------------------------------------------------------------------
 // {6j} machinery (sf_sixj.cu)
 // -------------------------------------------------------------------------------------------------------------
+// Accuracy envelope of the double-double Racah sum (sf_sixj.cuh): relative 1e-12 for every argument 2j <= 150, degrading
+// to ~1e-9 at 2j = 200 (tests/test_gpu_sixj.py); beyond this bound the alternating sum cancels more than 106 bits resolve,
+// so larger arguments are refused (SF_EARG) instead of returning cancelled digits.
+#define SF_SIXJ_MAX_TWO_J 256
+
 struct SfSixjTable {
     int two_jmax;            // -1 if absent
     long n_slots;
@@ -100,8 +106,6 @@ int sf_build_slices(const SfDims& D, double* const S[5], const SfSixjTable& tab,
 
 struct SfScratch;   // owned by the context (sf_api.cu)
 int sf_vertex_staged(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
-int sf_vertex_fused(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
-bool sf_vertex_fused_supported(const SfDims& D);
 int sf_vertex_line(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
 bool sf_vertex_line_supported(const SfDims& D);
 int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);

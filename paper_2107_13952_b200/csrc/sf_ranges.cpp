@@ -205,3 +205,165 @@ extern "C" int sf_vertex_work(const int two_j[10], int two_dl, long shell_lo, lo
     if (n_w) *n_w = w;
     return SF_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// useful work of the factorised path (include/sfoam_debug.h: sf_factor_work)
+// ---------------------------------------------------------------------------------------------------------
+// A term of a contraction counts when the triangle inequalities among the labels of BOTH operands hold (the {6j} of
+// eq. (5) vanish otherwise, and a booster entry outside its triple's k-range is zero by reading G9) and, for an
+// intermediate, when at least one term reaches the entry.  Sets of k values are bit masks (n_k_pad <= 128).
+namespace {
+struct Bits {
+    unsigned long long w[2];
+    Bits() { w[0] = w[1] = 0; }
+    void set(int b) { w[b >> 6] |= 1ull << (b & 63); }
+    bool test(int b) const { return (w[b >> 6] >> (b & 63)) & 1ull; }
+    bool meets(const Bits& o) const { return (w[0] & o.w[0]) || (w[1] & o.w[1]); }
+    void join(const Bits& o) { w[0] |= o.w[0]; w[1] |= o.w[1]; }
+    int count() const { return __builtin_popcountll(w[0]) + __builtin_popcountll(w[1]); }
+};
+inline bool tri(int a, int b, int c)
+{
+    const int d = a > b ? a - b : b - a;
+    return !((a + b + c) & 1) && c >= d && c <= a + b;
+}
+}   // namespace
+
+extern "C" int sf_factor_work(const int two_j[10], int two_dl, double mac[6], double elems[4])
+{
+    if (!mac || !elems) return SF_EARG;
+    SfDims D;
+    int rc = sf_host_dims(two_j, two_dl, &D);
+    if (rc != SF_OK) return rc;
+    for (int e = 0; e < 4; ++e)
+        if (D.n_k_pad[e] > 128) return SF_EARG;
+    const int nl = D.nl, n1 = D.n_i[0], NX = D.n_x_pad;
+    const double n2 = D.n_i[1], n3 = D.n_i[2], n4 = D.n_i[3], n5 = D.n_i[4];
+    const int* j = D.two_j;
+    const int P2 = D.n_k_pad[0], P3 = D.n_k_pad[1], P4 = D.n_k_pad[2], P5 = D.n_k_pad[3];
+    auto L = [&](int s, int o) { return j[s] + 2 * o; };
+    auto K = [&](int e, int q) { return D.two_k_base[e] + 2 * q; };
+    auto I1 = [&](int a) { return D.two_i_min[0] + 2 * a; };
+    auto X = [&](int xx) { return D.two_x_base + 2 * xx; };
+    for (int q = 0; q < 6; ++q) mac[q] = 0.0;
+    for (int q = 0; q < 4; ++q) elems[q] = 0.0;
+
+    // ---- Z = sum_k5 S2 S1 Bw5:  S1 {i1 l25 x; k5 j14 j15}, S2 {j14 k5 x; l35 k4 l45}, B5 range (j15 l25 | l35 l45)
+    // nk5[o25][xx][o35][o45] = number of k5 with (k5 l25 j15), (k5 j14 x), (l35 k5 l45)
+    std::vector<int> nk5((size_t)nl * NX * nl * nl, 0);
+    for (int o25 = 0; o25 < nl; ++o25)
+        for (int xx = 0; xx < NX; ++xx)
+            for (int o35 = 0; o35 < nl; ++o35)
+                for (int o45 = 0; o45 < nl; ++o45) {
+                    int n = 0;
+                    for (int q = 0; q < P5; ++q)
+                        n += tri(K(3, q), L(J25, o25), j[J15]) && tri(K(3, q), j[J14], X(xx)) &&
+                             tri(L(J35, o35), K(3, q), L(J45, o45));
+                    nk5[((size_t)(o25 * NX + xx) * nl + o35) * nl + o45] = n;
+                }
+    // k4 sets: (j14 k4 l45) per o45, (l35 k4 x) per (o35, xx), (l24 l34 k4) per (o24, o34)
+    std::vector<Bits> k4_45(nl), k4_35x((size_t)nl * NX), k4_2434((size_t)nl * nl);
+    for (int q = 0; q < P4; ++q) {
+        for (int o = 0; o < nl; ++o)
+            if (tri(j[J14], K(2, q), L(J45, o))) k4_45[o].set(q);
+        for (int o = 0; o < nl; ++o)
+            for (int xx = 0; xx < NX; ++xx)
+                if (tri(L(J35, o), K(2, q), X(xx))) k4_35x[(size_t)o * NX + xx].set(q);
+        for (int a = 0; a < nl; ++a)
+            for (int b = 0; b < nl; ++b)
+                if (tri(L(J24, a), L(J34, b), K(2, q))) k4_2434[(size_t)a * nl + b].set(q);
+    }
+    std::vector<double> npair4(P4, 0.0);             // number of (l24 l34) pairs that allow k4
+    for (int q = 0; q < P4; ++q)
+        for (int a = 0; a < nl * nl; ++a) npair4[q] += k4_2434[a].test(q);
+    // k3 sets: (k3 l35 l34) per (o34, o35), (k3 l24 x) per (o24, xx); l23 counts per k3: (j13 k3 l23)
+    std::vector<Bits> k3_3435((size_t)nl * nl), k3_24x((size_t)nl * NX);
+    std::vector<double> nl23(P3, 0.0);
+    for (int q = 0; q < P3; ++q) {
+        for (int a = 0; a < nl; ++a)
+            for (int b = 0; b < nl; ++b)
+                if (tri(K(1, q), L(J35, b), L(J34, a))) k3_3435[(size_t)a * nl + b].set(q);
+        for (int a = 0; a < nl; ++a)
+            for (int xx = 0; xx < NX; ++xx)
+                if (tri(K(1, q), L(J24, a), X(xx))) k3_24x[(size_t)a * NX + xx].set(q);
+        for (int o = 0; o < nl; ++o) nl23[q] += tri(j[J13], K(1, q), L(J23, o));
+    }
+    // G operands: k2 with (l23 l24 k2), (l25 j12 k2), (k2 j13 x)
+    std::vector<int> nk2((size_t)nl * nl * nl * NX, 0);
+    for (int o23 = 0; o23 < nl; ++o23)
+        for (int o24 = 0; o24 < nl; ++o24)
+            for (int o25 = 0; o25 < nl; ++o25)
+                for (int xx = 0; xx < NX; ++xx) {
+                    int n = 0;
+                    for (int q = 0; q < P2; ++q)
+                        n += tri(L(J23, o23), L(J24, o24), K(0, q)) && tri(L(J25, o25), j[J12], K(0, q)) &&
+                             tri(K(0, q), j[J13], X(xx));
+                    nk2[((size_t)(o23 * nl + o24) * nl + o25) * NX + xx] = n;
+                }
+
+    std::vector<Bits> zk4((size_t)nl);               // per o35: the k4 for which Z[l25 i1 l35 . k4 x] has an entry
+    std::vector<Bits> k3set((size_t)nl);             // per o24: the k3 for which R[l24 l25 i1 k3 x .] has an entry
+    for (int o25 = 0; o25 < nl; ++o25)
+        for (int a1 = 0; a1 < n1; ++a1)
+            for (int xx = 0; xx < NX; ++xx) {
+                if (!tri(I1(a1), L(J25, o25), X(xx))) continue;
+                // Z and Q
+                for (int o35 = 0; o35 < nl; ++o35) {
+                    zk4[o35] = Bits();
+                    const Bits& kx = k4_35x[(size_t)o35 * NX + xx];
+                    for (int o45 = 0; o45 < nl; ++o45) {
+                        const int n5k = nk5[((size_t)(o25 * NX + xx) * nl + o35) * nl + o45];
+                        if (!n5k) continue;
+                        Bits k4;
+                        k4.w[0] = kx.w[0] & k4_45[o45].w[0];
+                        k4.w[1] = kx.w[1] & k4_45[o45].w[1];
+                        const int c = k4.count();
+                        mac[0] += (double)n5k * c * n5;
+                        elems[0] += (double)c * n5;
+                        zk4[o35].join(k4);
+                        for (int q = 0; q < P4; ++q)
+                            if (k4.test(q)) mac[1] += npair4[q] * n5 * n4;          // Q: one term per l45, all (l24 l34) of k4
+                    }
+                    for (int q = 0; q < P4; ++q)
+                        if (zk4[o35].test(q)) elems[1] += npair4[q] * n5 * n4;
+                }
+                // P, R, A' per l24
+                for (int o24 = 0; o24 < nl; ++o24) {
+                    k3set[o24] = Bits();
+                    const Bits& k3x = k3_24x[(size_t)o24 * NX + xx];
+                    for (int o34 = 0; o34 < nl; ++o34) {
+                        const Bits& k4a = k4_2434[(size_t)o24 * nl + o34];
+                        for (int o35 = 0; o35 < nl; ++o35) {
+                            Bits k4;
+                            k4.w[0] = zk4[o35].w[0] & k4a.w[0];
+                            k4.w[1] = zk4[o35].w[1] & k4a.w[1];
+                            const int c4 = k4.count();
+                            if (!c4) continue;
+                            Bits k3;
+                            k3.w[0] = k3x.w[0] & k3_3435[(size_t)o34 * nl + o35].w[0];
+                            k3.w[1] = k3x.w[1] & k3_3435[(size_t)o34 * nl + o35].w[1];
+                            const int c3 = k3.count();
+                            if (!c3) continue;
+                            mac[2] += (double)c3 * c4 * n5 * n4;
+                            elems[2] += (double)c3 * n5 * n4;
+                            k3set[o24].join(k3);
+                            for (int q = 0; q < P3; ++q)
+                                if (k3.test(q)) mac[3] += nl23[q] * n3 * n4 * n5;   // R: one term per (l34 l35), all l23 of k3
+                        }
+                    }
+                    for (int q = 0; q < P3; ++q) {
+                        if (!k3x.test(q)) continue;
+                        for (int o23 = 0; o23 < nl; ++o23) {
+                            if (!tri(j[J13], K(1, q), L(J23, o23))) continue;
+                            const int n2k = nk2[((size_t)(o23 * nl + o24) * nl + o25) * NX + xx];
+                            mac[4] += (double)n2k * n2;                                 // G
+                            if (k3set[o24].test(q)) {
+                                elems[3] += n3 * n4 * n5;
+                                if (n2k) mac[5] += n2 * n3 * n4 * n5;                   // A'
+                            }
+                        }
+                    }
+                }
+            }
+    return SF_OK;
+}

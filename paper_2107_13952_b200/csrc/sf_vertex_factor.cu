@@ -1092,6 +1092,9 @@ static FzShape fz_shape(const SfDims& D)
 
 bool sf_vertex_factor_supported(const SfDims& D) { return fz_shape(D).ok; }
 
+static size_t g_fz_budget = 0;                       // sf_set_factor_budget: bytes for P and R of one pass (0 = a third of the device)
+extern "C" void sf_set_factor_budget(unsigned long bytes) { g_fz_budget = bytes; }
+
 template <class Map, int WGM, int WGN, int TM, int TN>
 static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
 {
@@ -1233,9 +1236,12 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         const long pP = c24 * c25 * P3 * sh.V * c34 * c35 * sh.NP;     // per i1
         const long pR = c24 * c25 * P3 * sh.V * c23 * n3 * sh.NP;
         // i1 values per pass: P and R of a pass inside ~1/3 of the device memory
-        const double budget = (double)total_b / 3.0;
+        const double budget = g_fz_budget ? (double)g_fz_budget : (double)total_b / 3.0;
         long na = (long)(budget / (8.0 * (double)(pP + pR)));
-        if (na < 1) return SF_ENOMEM;
+        if (na < 1) {
+            if (!g_fz_budget) return SF_ENOMEM;
+            na = 1;                                  // a test budget below one i1 still runs, one i1 per pass
+        }
         if (na > n1) na = n1;
         double* Z = (double*)sf_scratch(FZ_SLOT_Z, sizeof(double) * (size_t)nZ);
         double* B4 = (double*)sf_scratch(FZ_SLOT_B4, sizeof(double) * (size_t)nB4);

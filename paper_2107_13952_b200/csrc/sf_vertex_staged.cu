@@ -182,6 +182,19 @@ int sf_vertex_staged(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     double* acc = (double*)sf_scratch(0, sizeof(double) * D.n_out);
     if (!acc) return SF_ENOMEM;
     SF_CUDA_OK(cudaMemsetAsync(acc, 0, sizeof(double) * D.n_out, st));
+    {   // k_stage_mode keeps one booster sub-matrix (n_i x k_max doubles) in dynamic shared memory: opt in above 48 KB
+        size_t need = 0;
+        for (int e = 0; e < 4; ++e) {
+            const size_t b = sizeof(double) * (size_t)D.n_i[e + 1] * D.k_max[e];
+            if (b > need) need = b;
+        }
+        static size_t attr = 48 * 1024;
+        if (need > 226 * 1024) return SF_EARG;       // a booster sub-matrix beyond one SM's shared memory: not held
+        if (need > attr) {
+            SF_CUDA_OK(cudaFuncSetAttribute(k_stage_mode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));
+            attr = need;
+        }
+    }
     if (M2 && M3 && M4 && M5 && shell_hi > shell_lo) {
         // per-i1 size of the largest intermediate
         long per1 = M2 * M3 * M4 * M5;

@@ -1,6 +1,6 @@
 """CPU-side checks of the C-ABI library (no compute calls: there is no GPU here).
 
-  * libsfoam.so loads and exports every function include/sfoam.h declares
+  * libsfoam.so loads and exports every function include/sfoam.h and include/sfoam_debug.h declare
   * the pure host integer helpers (step 2 of the algorithm) agree with the oracle's range code
     and with the counts of SURVEY.md 8(a)/8(c) P2
   * without a CUDA device the compute entry points fail loudly (no CPU fallback)
@@ -24,14 +24,14 @@ def built():
 
 
 def test_every_declared_symbol_is_exported():
-    header = open(os.path.join(ROOT, "include", "sfoam.h")).read()
+    header = open(os.path.join(ROOT, "include", "sfoam.h")).read() + open(os.path.join(ROOT, "include", "sfoam_debug.h")).read()
     header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
     names = set(re.findall(r"\b(sf_[a-z0-9_]+)\s*\(", header))
     assert {"sf_init", "sf_sixj_table", "sf_vertex_amplitude", "sf_vertex_amplitude_range",
             "sf_vertex_amplitude_host", "sf_sixj_get", "sf_vertex_dims", "sf_booster_dims"} <= names
     lib = ctypes.CDLL(sf.LIB_PATH)
     for n in sorted(names):
-        assert hasattr(lib, n), f"{n} declared in sfoam.h but not exported"
+        assert hasattr(lib, n), f"{n} declared in include/*.h but not exported"
 
 
 SPIN_SETS = [([2] * 10, 4), ([1] * 10, 2), ([6] * 10, 6), ([10] * 10, 4),
@@ -159,3 +159,80 @@ def _box_shell_sets(boxes, nl):
             ss.append(s)
         out.append(ss)
     return out
+
+
+def _tri(a, b, c):
+    return ((a + b + c) % 2 == 0) & (c >= abs(a - b)) & (c <= a + b)
+
+
+def _factor_work_bruteforce(two_j, two_dl):
+    """The counts sf_factor_work returns, by dense boolean masks over every index of every contraction of the factorised
+    chain (K-f): a term counts when the triads among the labels of both operands hold."""
+    import numpy as np
+    from oracle.ranges import J12, J13, J14, J15, J23, J24, J25, J34, J35, J45
+    nl, j = two_dl // 2 + 1, two_j
+    br = ranges.boundary_ranges(two_j)
+    n1, n2, n3, n4, n5 = [b[1] for b in br]
+    lv = {s: j[s] + 2 * np.arange(nl) for s in (J23, J24, J25, J34, J35, J45)}
+    i1 = br[0][0] + 2 * np.arange(n1)
+    ks = []
+    for e in (2, 3, 4, 5):
+        _, _, _, base, pad = ranges.booster_dims(two_j, two_dl, e)
+        ks.append(base + 2 * np.arange(pad))
+    k2, k3, k4, k5 = ks
+    x = np.arange(min(abs(a - b) for a in i1 for b in lv[J25]), max(a + b for a in i1 for b in lv[J25]) + 1, 2)
+
+    def m(spec, *vals):
+        """boolean triad mask with one axis per array argument (scalars broadcast)"""
+        arrs = [v for v in vals if not np.isscalar(v)]
+        nd, out, pos = len(arrs), [], 0
+        for v in vals:
+            if np.isscalar(v):
+                out.append(v)
+            else:
+                sh = [1] * nd
+                sh[pos] = len(v)
+                out.append(v.reshape(sh))
+                pos += 1
+        return _tri(*out).astype(np.int64)
+
+    I = np.einsum
+    t_i1_l25_x = m("", i1, lv[J25], x)
+    t_k5_l25 = m("", k5, lv[J25], j[J15])
+    t_k5_x = m("", k5, j[J14], x)
+    t_k4_l45 = m("", j[J14], k4, lv[J45])
+    t_l35_k5_l45 = m("", lv[J35], k5, lv[J45])
+    t_l35_k4_x = m("", lv[J35], k4, x)
+    t_l24_l34_k4 = m("", lv[J24], lv[J34], k4)
+    t_k3_l35_l34 = m("", k3, lv[J35], lv[J34])
+    t_k3_l24_x = m("", k3, lv[J24], x)
+    t_k3_l23 = m("", j[J13], k3, lv[J23])
+    t_k2_l23_l24 = _tri(lv[J23].reshape(1, -1, 1), lv[J24].reshape(1, 1, -1), k2.reshape(-1, 1, 1)).astype(np.int64)
+    t_k2_l25 = m("", k2, lv[J25], j[J12])
+    t_k2_x = m("", k2, j[J13], x)
+    zc = I("abx,ub,ux,kd,cud,ckx->bacdkx", t_i1_l25_x, t_k5_l25, t_k5_x, t_k4_l45, t_l35_k5_l45, t_l35_k4_x)
+    zmask = (zc > 0).astype(np.int64)
+    qc = I("bacdkx,kd,efk->bacefkx", zmask, t_k4_l45, t_l24_l34_k4)
+    qmask = (qc > 0).astype(np.int64)
+    pc = I("bacefkx,ckx,efk,gcf,gex->ebagxfc", qmask, t_l35_k4_x, t_l24_l34_k4, t_k3_l35_l34, t_k3_l24_x)
+    pmask = (pc > 0).astype(np.int64)
+    rc = I("ebagxfc,gcf,gh->ebagxh", pmask, t_k3_l35_l34, t_k3_l23)
+    rmask = (rc > 0).astype(np.int64)
+    gc = I("whe,wb,wx,abx,gex,gh->ebagxh", t_k2_l23_l24, t_k2_l25, t_k2_x, t_i1_l25_x, t_k3_l24_x, t_k3_l23)
+    mac = {"Z": zc.sum() * n5, "Q": qc.sum() * n5 * n4, "P": pc.sum() * n5 * n4, "R": rc.sum() * n3 * n4 * n5,
+           "G": gc.sum() * n2, "A": ((gc > 0) * rmask).sum() * n2 * n3 * n4 * n5}
+    elems = {"Z": zmask.sum() * n5, "Q": qmask.sum() * n4 * n5, "P": pmask.sum() * n4 * n5, "R": rmask.sum() * n3 * n4 * n5}
+    return mac, elems
+
+
+@pytest.mark.parametrize("two_j,two_dl", [([2] * 10, 4), ([1] * 10, 2), ([6] * 10, 4), ([4, 3, 1, 4, 2, 5, 5, 5, 4, 3], 4),
+                                          ([8, 7, 12, 3, 8, 5, 9, 12, 3, 7], 2)])
+def test_factor_work_matches_dense_mask_count(two_j, two_dl):
+    """The roofline numerator of the factorised path (bench.py) = useful multiply-adds on valid index ranges: the host
+    counter of the library against a dense brute-force count."""
+    mac, elems = sf.sf_factor_work(two_j, two_dl)
+    bmac, belems = _factor_work_bruteforce(two_j, two_dl)
+    for k in mac:
+        assert mac[k] == bmac[k], (k, mac[k], bmac[k])
+    for k in elems:
+        assert elems[k] == belems[k], (k, elems[k], belems[k])

@@ -70,6 +70,9 @@ def test_large_spins_direct():
     # beyond that the alternating sum cancels faster than double-double resolves: the accuracy degrades gracefully
     args = [(200,) * 6, (200, 180, 100, 160, 150, 150)]
     _check(args, sf.sf_sixj_batch(args, mode=0), rel=1e-9)
+    with pytest.raises(sf.SfError) as err:           # beyond the validated envelope: refused, not returned with cancelled digits
+        sf.sf_sixj_batch([(258,) * 6], mode=0)
+    assert err.value.status == sf.SF_EARG
 
 
 def test_table_gather_equals_exact_and_uses_symmetry():
@@ -113,3 +116,56 @@ def test_table_two_jmax_60_sampled():
     got_d = sf.sf_sixj_batch(args, mode=0)
     _check(args, got_t)
     assert np.allclose(got_t, got_d, rtol=1e-14, atol=1e-18)   # table slot = direct value of the canonical image
+
+
+def _exact_many(args, processes=8):
+    from multiprocessing import Pool
+    with Pool(processes) as pool:
+        return pool.starmap(wigner.sixj, args, chunksize=512)
+
+
+def _valid(t):
+    a, b, c, d, e, f = t
+    return (wigner.is_triad(a, b, c) and wigner.is_triad(a, e, f) and wigner.is_triad(d, b, f)
+            and wigner.is_triad(d, e, c))
+
+
+def test_stratified_sweep_two_j_le_60_direct_and_table():
+    """>= 1e5 symbols with every 2j <= 60 against the exact big-integer oracle, direct evaluation and table gather, at the
+    bar of north_star (relative 1e-12; |gpu| <= 1e-18 where the exact value is 0).  Strata: uniform random valid symbols; the
+    whole corner band 56 <= 2j <= 60 (where the Racah sum cancels most: sum|t| / |sum t| ~ 2e5); stretched
+    triads (c = a + b or |a - b|, f likewise); near-equal spins in 30..60."""
+    rng = random.Random(606060)
+    strata = {}
+    strata["uniform"] = [_random_valid(rng, 60) for _ in range(40000)]
+    strata["corner_band"] = [t for t in itertools.product(range(56, 61), repeat=6) if _valid(t)]
+    stretched = []
+    while len(stretched) < 25000:
+        a, b, d, e = (rng.randint(0, 60) for _ in range(4))
+        c = rng.choice([a + b, abs(a - b)])
+        f = rng.choice([a + e, abs(a - e), d + b, abs(d - b)])
+        t = (a, b, c, d, e, f)
+        if max(t) <= 60 and _valid(t):
+            stretched.append(t)
+    strata["stretched"] = stretched
+    near = []
+    while len(near) < 30000:
+        base = rng.randint(30, 60)
+        t = tuple(min(60, max(0, base + rng.randint(-3, 3))) for _ in range(6))
+        if _valid(t):
+            near.append(t)
+    strata["near_equal"] = near
+    args = [t for s in strata.values() for t in s]
+    assert len(args) >= 100000, len(args)
+    exact = np.array(_exact_many(args))
+    sf.sf_sixj_table(60)
+    try:
+        for mode in (0, 1):
+            got = sf.sf_sixj_batch(args, mode=mode)
+            zero = exact == 0.0
+            assert (np.abs(got[zero]) <= 1e-18).all(), f"mode {mode}: a vanishing symbol came out non-zero"
+            rel = np.abs(got[~zero] - exact[~zero]) / np.abs(exact[~zero])
+            worst = int(np.argmax(rel))
+            assert rel.max() <= 1e-12, (mode, rel.max(), np.array(args)[~zero][worst])
+    finally:
+        sf.sf_sixj_table(-1)

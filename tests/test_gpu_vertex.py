@@ -50,7 +50,7 @@ def test_config0_full(path):
     assert sf.sf_last_path() == TAKEN[path]
 
 
-@pytest.mark.parametrize("two_j", [1, 2, 3, 4, 6, 9, 12])
+@pytest.mark.parametrize("two_j", list(range(1, 15)))
 def test_config1_bf_sweep(path, two_j):
     """Identity boosters, Delta_l = 0  =>  A = N(i) {15j}  (reading G8)."""
     cfg = wl.config1(two_j)
@@ -60,11 +60,24 @@ def test_config1_bf_sweep(path, two_j):
         assert Ag[1, 1, 1, 1, 1] == pytest.approx(3 ** 2.5 * 3 ** 4 * (-7 / 432), rel=1e-13)
 
 
-def test_config1_bf_j10_full_tensor():
-    """The largest BF tensor, 21^5 entries (staged path: it does not fit on chip)."""
-    cfg = wl.config1(20)
+@pytest.mark.parametrize("two_j", list(range(15, 21)))
+def test_config1_bf_large_spins_full_tensor(two_j):
+    """The upper end of BASELINE.json's config 1 (j = 15/2 .. 10; up to 21^5 entries), automatic path, full tensors: with
+    test_config1_bf_sweep every 2j = 1 .. 20 of the sweep is compared entrywise with the oracle."""
+    cfg = wl.config1(two_j)
     worst, Ag, Ao = _full(cfg, cfg["name"])
-    assert Ag.shape == (21,) * 5
+    assert Ag.shape == (two_j + 1,) * 5
+    assert sf.sf_last_path() == 4
+
+
+def test_config1_bf_j10_staged_path():
+    """The largest BF tensor on the staged path (the fallback for shapes the other paths do not hold)."""
+    cfg = wl.config1(20)
+    sf.sf_set_path(1)
+    try:
+        _full(cfg, cfg["name"])
+    finally:
+        sf.sf_set_path(0)
 
 
 @pytest.mark.parametrize("dl", [0, 1, 2])
@@ -169,6 +182,101 @@ def test_config4_sub_ranges(path, lam, n):
     Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, lo + n)
     Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, lo + n)
     assert_parity(Ag, Ao, Aabs, what=f"{cfg['name']} shells [{lo},{lo + n})")
+
+
+# (lambda, first shell, number of shells): whole (l34 l35 l45) blocks of 7^3 shells, whole (l35 l45) planes and whole l45
+# lines followed by a ragged tail, so that the boxes the factorised path runs have 7 offsets per virtual spin (c34 = c35 =
+# c45 = 7, two k-steps over l45) as in the full tensors bench.py times; the oracle cost grows like lambda^5, so the larger
+# spins get planes instead of blocks
+CONFIG4_RANGES = [(2, 343 * 170, 343 + 60), (3, 343 * 171, 343 + 60), (4, 343 * 5, 343 + 23), (5, 343 * 200 + 49, 49 * 2 + 17),
+                  (6, 343 * 342 + 49 * 3, 49 + 7 + 3)]
+
+
+@pytest.mark.parametrize("lam,lo,n", CONFIG4_RANGES)
+def test_config4_blocks_planes_and_ragged_tails(lam, lo, n):
+    """BASELINE.json config 4 (js * lambda) for every lambda = 2 .. 6 on the automatic (factorised) path."""
+    cfg = _config4(lam)
+    B = boosters_for(cfg)
+    Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, lo + n)
+    assert sf.sf_last_path() == 4
+    boxes = sf.sf_shell_boxes(cfg["two_dl"], lo, lo + n)
+    assert any(cnt[5] == 7 and cnt[4] == 7 for _, cnt in boxes)
+    Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, lo + n, processes=16)
+    assert np.abs(Ao).max() > 0
+    assert_parity(Ag, Ao, Aabs, what=f"{cfg['name']} shells [{lo},{lo + n})")
+
+
+@pytest.mark.parametrize("lam", [2, 3])
+def test_config4_full_tensor_factorised_equals_staged(lam):
+    """All 117 649 shells of config 4 at lambda = 2, 3: the factorised path (the one bench.py times) and the staged per-shell
+    path (compared with the oracle on sub-ranges above) give the same tensor to rounding."""
+    cfg = _config4(lam)
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    sf.sf_set_path(4)
+    A4 = run_gpu(cfg["two_j"], cfg["two_dl"], B, Bdev=Bdev)
+    sf.sf_set_path(1)
+    A1 = run_gpu(cfg["two_j"], cfg["two_dl"], B, Bdev=Bdev)
+    sf.sf_set_path(0)
+    assert np.isfinite(A4).all() and np.abs(A4).max() > 0
+    assert np.abs(A4 - A1).max() <= 1e-12 * np.abs(A1).max()
+
+
+def test_factorised_path_small_memory_budget_takes_the_multi_pass_branches():
+    """With a P/R budget of a few hundred KB (sf_set_factor_budget) small problems run one i1 per pass, several passes: the
+    branch the full-size workloads take (config 3: 5 + 5 + 1 values of i1), here on tensors the oracle computes in full."""
+    cases = [wl.config2(2), wl.config2(3), dict(two_j=[4, 3, 1, 4, 2, 5, 5, 5, 4, 3], two_dl=4, boosters="random", seed=77),
+             _config4(1)]
+    sf.sf_set_path(4)
+    try:
+        for cfg in cases:
+            B = boosters_for(cfg)
+            Bdev = to_device(B)
+            n = (cfg["two_dl"] // 2 + 1) ** 6
+            lo, hi = (0, n) if n <= 4096 else (n // 2, n // 2 + 343 + 20)
+            Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, hi)
+            ref = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+            for budget in (1, 300 * 1024, 3 * 1024 * 1024):
+                sf.sf_set_factor_budget(budget)
+                Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+                sf.sf_set_factor_budget(0)
+                assert_parity(Ag, Ao, Aabs, what=f"{cfg.get('name')} budget {budget}")
+                assert np.abs(Ag - ref).max() <= 1e-13 * max(Aabs.max(), 1e-300)
+    finally:
+        sf.sf_set_factor_budget(0)
+        sf.sf_set_path(0)
+
+
+def test_config3_full_tensor_against_the_cached_oracle_tensor(golden_dir):
+    """ALL 1 771 561 shells of the headline workload (BASELINE.json config 3), the tensor bench.py times, entry by entry
+    against the oracle's full tensor: tests/golden/config3_full.npz, written by tests/golden/make_config3_full.py from
+    `oracle/` alone (long double, ~2 h of CPU) and keyed by the hash of the inputs.  Both the automatic (factorised) path and
+    the per-shell line path, at the tolerance of north_star."""
+    import hashlib
+    import os
+    f = os.path.join(golden_dir, "config3_full.npz")
+    assert os.path.exists(f), "tests/golden/config3_full.npz is missing: run tests/golden/make_config3_full.py"
+    z = np.load(f)
+    cfg = wl.CONFIGS[3]
+    B = boosters_for(cfg)
+    h = hashlib.sha256()
+    h.update(np.asarray(list(cfg["two_j"]) + [cfg["two_dl"]], dtype=np.int64).tobytes())
+    for edge in (2, 3, 4, 5):
+        h.update(np.ascontiguousarray(B[edge], dtype=np.float64).tobytes())
+    assert h.hexdigest() == str(z["input_sha256"]), "the cached oracle tensor was computed from different inputs"
+    assert int(z["nonempty"]) == 11 ** 6
+    Ao, Aabs = z["A"], z["Aabs"]
+    Bdev = to_device(B)
+    sf.sf_sixj_table(60)
+    try:
+        for path in (0, 3):
+            sf.sf_set_path(path)
+            Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, Bdev=Bdev)
+            assert sf.sf_last_path() == TAKEN[path]
+            assert_parity(Ag, Ao, Aabs, what=f"config 3, all shells, path {TAKEN[path]}")
+    finally:
+        sf.sf_set_path(0)
+        sf.sf_sixj_table(-1)
 
 
 def test_table_and_direct_slices_agree(path):
@@ -357,7 +465,9 @@ def test_errors(path):
     two_j = [2] * 10
     B = to_device(boosters_for(wl.CONFIGS[0]))
     out = torch.zeros(3 ** 5, dtype=torch.float64, device="cuda")
-    for bad_j, bad_dl, status in [([2] * 9 + [3], 4, sf.SF_ESPIN), (two_j, 3, sf.SF_EARG), (two_j, -2, sf.SF_EARG)]:
+    # the last: the largest {6j} label 2 (j + Delta_l) = 260 is beyond the validated envelope of the {6j} evaluation
+    for bad_j, bad_dl, status in [([2] * 9 + [3], 4, sf.SF_ESPIN), (two_j, 3, sf.SF_EARG), (two_j, -2, sf.SF_EARG),
+                                  ([130] * 10, 0, sf.SF_EARG)]:
         with pytest.raises(sf.SfError) as e:
             sf.sf_vertex_amplitude(bad_j, bad_dl, B, out)
         assert e.value.status == status
