@@ -137,7 +137,7 @@ def test_stratified_sweep_two_j_le_60_direct_and_table():
     triads (c = a + b or |a - b|, f likewise); near-equal spins in 30..60."""
     rng = random.Random(606060)
     strata = {}
-    strata["uniform"] = [_random_valid(rng, 60) for _ in range(40000)]
+    strata["uniform"] = [_random_valid(rng, 60) for _ in range(45000)]
     strata["corner_band"] = [t for t in itertools.product(range(56, 61), repeat=6) if _valid(t)]
     stretched = []
     while len(stretched) < 25000:
