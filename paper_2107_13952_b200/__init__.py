@@ -174,6 +174,11 @@ def sf_set_staged_budget(nbytes):
     _lib().sf_set_staged_budget(int(nbytes))
 
 
+def sf_set_factor_variant(bits):
+    """Kernel variants of the factorised path (include/sfoam_debug.h): 0 = default."""
+    _lib().sf_set_factor_variant(int(bits))
+
+
 def sf_set_factor_budget(nbytes):
     """Device bytes the factorised path may use for P and R of one pass over i1 (0 = default, a third of the device)."""
     _lib().sf_set_factor_budget(int(nbytes))
