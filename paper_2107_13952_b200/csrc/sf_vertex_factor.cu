@@ -653,7 +653,7 @@ struct FzChunk<TM, TN, 0, KC> {
 template <class Map, int WGM, int WGN, int TM, int TN>
 __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int kcap)
 {
-    constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8, NTH = WGM * WGN * 32, LDA = BM + 8, LDB = BN + 8;
+    constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8, NTH = WGM * WGN * 32, LDA = BM + 4, LDB = BN + 4;   // = 4 mod 16: half-warp fragment loads hit 16 different banks
     constexpr int KC = Map::KC, ST = Map::ST;        // k-chunk depth and ring stages
     extern __shared__ __align__(16) double smem[];
     __shared__ FzGemmHdr hdr;
@@ -927,7 +927,7 @@ static FzShape fz_shape(const SfDims& D)
         }
     s.W4p = (w4 + 3) & ~3;
     if (w3 == 0 || s.W4p == 0) return s;
-    s.LDQ = ((n54 + 15) & ~15) + 8;                   // = 8 mod 16: conflict-free B fragments
+    s.LDQ = ((n54 + 15) & ~15) + 4;                   // = 4 mod 16: conflict-free B fragments (lanes q * LDQ + g of a half warp)
     // x values per pass.  Every pass costs two CTA barriers and a fixed amount of index work, so more x per pass is better
     // as long as the 8-row tiles of (v, i5) stay well filled, the rows fit the fast Q phase (8 FZ_QMT) and two CTAs keep
     // ~100 KB of the SM for L1: the largest vg inside 80 KB with fill >= 0.8, else the best-filled one; a single x may take up
@@ -969,7 +969,7 @@ template <class Map, int WGM, int WGN, int TM, int TN>
 static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
 {
     constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8;
-    const size_t smem = sizeof(double) * Map::ST * Map::KC * (BM + 8 + BN + 8) + sizeof(int) * (2 * BM + 2 * BN + 240 + (size_t)kcap);
+    const size_t smem = sizeof(double) * Map::ST * Map::KC * (BM + 4 + BN + 4) + sizeof(int) * (2 * BM + 2 * BN + 240 + (size_t)kcap);
     if (smem > 226 * 1024) return SF_EARG;
     static size_t attr = 0;
     if (smem > attr) {
@@ -1022,6 +1022,10 @@ extern "C" int sf_last_dmma(double n[3])
 }
 
 int fz_launch_r2(const FzParams& p, const SfDims& D, int* sched, int n_sm, cudaStream_t st);   // sf_factor_r.cu
+bool fz_qp2_supported(const FzParams& p, const SfDims& D);                                     // sf_factor_qp.cu
+long fz_qp2_b4p_elems(const FzParams& p, const SfDims& D);
+void fz_launch_b4p(const FzParams& p, long n, double* out, cudaStream_t st);
+int fz_launch_qp2(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st);
 
 enum { FZ_SLOT_SCHED = 22, FZ_SLOT_CNT = 23, FZ_SLOT_WIN = 24, FZ_SLOT_LIST, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART };
 
@@ -1104,7 +1108,8 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         p.hull4B = make_int2(lo < hi ? lo : 0, lo < hi ? hi : 0);
 
         const long nZ = c25 * n1 * c35 * c45 * ((long)P4 * sh.V * n5);
-        const long nB4 = (long)P4 * c45 * c24 * c34 * n4, nB3 = (long)P3 * c34 * c35 * c23 * n3;
+        const bool qp2 = !(g_fz_variant & 2) && fz_qp2_supported(p, D);      // second-generation Q/P kernel and its booster layout
+        const long nB4 = qp2 ? fz_qp2_b4p_elems(p, D) : (long)P4 * c45 * c24 * c34 * n4, nB3 = (long)P3 * c34 * c35 * c23 * n3;
         const long nS3 = c24 * c34 * c35 * D.n_x_pad * P3 * P4;
         const long nG = c24 * c25 * n1 * P3 * sh.V * c23 * n2;
         const long pP = c24 * c25 * P3 * sh.V * c34 * c35 * sh.NP;     // per i1
@@ -1120,7 +1125,8 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         double* Z = (double*)sf_scratch(FZ_SLOT_Z, sizeof(double) * (size_t)nZ);
         double* B4 = (double*)sf_scratch(FZ_SLOT_B4, sizeof(double) * (size_t)nB4);
         double* B3 = (double*)sf_scratch(FZ_SLOT_B3, sizeof(double) * (size_t)nB3);
-        double* S3 = (double*)sf_scratch(FZ_SLOT_S3, sizeof(double) * (size_t)nS3);
+        const long padS3 = 24L * P4 + 8;             // k_fz_qp2 reads fragment rows / columns just past a block: keep them finite
+        double* S3 = (double*)sf_scratch(FZ_SLOT_S3, sizeof(double) * (size_t)(nS3 + padS3));
         double* G = (double*)sf_scratch(FZ_SLOT_G, sizeof(double) * (size_t)nG);
         double *Pq = nullptr, *Rq = nullptr;
         for (;;) {                                   // other tenants of the device may hold memory: shrink the pass until it fits
@@ -1148,7 +1154,12 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         }
         fz_ev_begin(3, st);
         k_fz_z<<<(unsigned)(c25 * n1 * c35 * c45), 256, 0, st>>>(p, Z);
-        k_fz_b4t<<<(unsigned)((nB4 + 255) / 256), 256, 0, st>>>(p, nB4, B4);
+        if (qp2) {
+            fz_launch_b4p(p, nB4, B4, st);
+            SF_CUDA_OK(cudaMemsetAsync(S3 + nS3, 0, sizeof(double) * (size_t)padS3, st));
+        } else {
+            k_fz_b4t<<<(unsigned)((nB4 + 255) / 256), 256, 0, st>>>(p, nB4, B4);
+        }
         k_fz_b3t<<<(unsigned)((nB3 + 255) / 256), 256, 0, st>>>(p, nB3, B3);
         k_fz_s3t<<<(unsigned)((nS3 + 255) / 256), 256, 0, st>>>(p, nS3, S3);
         k_fz_g<<<(unsigned)((nG + 255) / 256), 256, 0, st>>>(p, nG, G);
@@ -1163,12 +1174,15 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
                 SF_CUDA_OK(cudaMemsetAsync(Rq, 0xFF, sizeof(double) * (size_t)(pR * na), st));
             }
             fz_ev_begin(0, st);
-            {
+            if (qp2) {
+                const int rcq = fz_launch_qp2(p, D, B4, sched + 1, n_sm, st);
+                if (rcq != SF_OK) return rcq;
+            } else {                                  // shapes the second-generation kernel does not hold
                 const long n_items = (long)p.a_cnt * c25 * c35 * c24 * c34;
                 const long grid = n_items < 2L * n_sm ? n_items : 2L * n_sm;
                 k_fz_qp<<<(unsigned)grid, FZ_QP_THREADS, sh.qp_smem, st>>>(p, n_items);
+                sf_count_launch(1);
             }
-            sf_count_launch(1);
             fz_ev_end(st);
             fz_ev_begin(1, st);
             int rc = g_fz_variant & 1 ? fz_launch_r2(p, D, sched, n_sm, st) : SF_EARG;         // booster block stationary, P streamed once
