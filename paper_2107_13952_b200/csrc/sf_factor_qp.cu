@@ -27,7 +27,10 @@
 
 #define FQ_THREADS 512
 #define FQ_XC 4                   // x values per item
-#define FQ_LDQ 260                // row stride of the Q tiles: 16 x 16 entries (i5, i4) per k4, = 4 mod 16
+#define FQ_QI5 24                 // stride of i5 inside a Q tile row: 16 i4 + 8 pad, so that the 16-byte stores of a quarter warp
+                                  // (two i5, four column pairs) fall into different banks
+#define FQ_LDQ 388                // row stride of the Q tiles: 16 x FQ_QI5 entries (i5, i4) per k4, + 4 (= 4 mod 16)
+#define FQ_GRP (2 * 4 * FQ_LDQ + 2 * 3 * 32)   // doubles of shared memory per group: two Q tiles, two S3 fragment tiles
 #define FQ_L45 12                 // l45 rows per k4 in the Z slab and in Bw4P (3 k-steps)
 
 struct FzQp2Args {
@@ -35,7 +38,9 @@ struct FzQp2Args {
     int vc;                       // chunks of FQ_XC x per (i1 l25)
     int n_items;
     int* sched;
-    const double* Bw4P;           // [b24][b34][q4][FQ_L45][16], zero outside the triple's k-range and beyond (c45, n4)
+    const double* Bw4P;           // [b24][b34][q4][k-step 3][lane 32][column tile 2]: the B fragments of Q in the order the lanes
+                                  // read them (l45 = 4 ks + lane % 4, i4 = 8 j + lane / 4), zero outside the triple's k-range
+                                  // and beyond (c45, n4)
 };
 
 __device__ __forceinline__ void fq_group_sync(int grp)
@@ -53,7 +58,8 @@ __device__ __forceinline__ void fq_sts2(unsigned addr, double a, double b)
     asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(a), "d"(b) : "memory");
 }
 
-// Bw4P[b24][b34][q4][l45 (12)][i4 (16)] = (2k4+1) B4[(o45 o24 o34)][i4][q4] inside the triple's k-range, 0 elsewhere
+// Bw4P[b24][b34][q4][ks][lane][j] = (2k4+1) B4[(o45 o24 o34)][i4][q4], l45 = 4 ks + lane % 4, i4 = 8 j + lane / 4, inside the triple's
+// k-range, 0 elsewhere: one 16-byte load per lane and k-step, 512 contiguous bytes per warp
 __global__ void __launch_bounds__(256) k_fz_b4p(FzParams p, long n, double* __restrict__ out)
 {
     const SfProblem& P = p.P;
@@ -62,8 +68,10 @@ __global__ void __launch_bounds__(256) k_fz_b4p(FzParams p, long n, double* __re
     const int nl = P.nl, n4 = P.n_i[3], P4 = P.n_k_pad[2];
     const int c34 = p.box.cnt[3], c45 = p.box.cnt[5];
     long r = e;
-    const int i4 = (int)(r % 16); r /= 16;
-    const int b45 = (int)(r % FQ_L45); r /= FQ_L45;
+    const int jj = (int)(r % 2); r /= 2;
+    const int ln = (int)(r % 32); r /= 32;
+    const int ks = (int)(r % 3); r /= 3;
+    const int i4 = 8 * jj + (ln >> 2), b45 = 4 * ks + (ln & 3);
     const int q4 = (int)(r % P4); r /= P4;
     const int b34 = (int)(r % c34);
     const int b24 = (int)(r / c34);
@@ -94,21 +102,22 @@ __global__ void __launch_bounds__(FQ_THREADS, 1) k_fz_qp2(const __grid_constant_
     const long prow = (long)c34 * c35 * NP;                   // stride of v in P
     const int nzs = P4 * FQ_L45 * ldz;
     double* Zs = smem;                                        // [P4][FQ_L45][ldz]
-    for (int z = tid; z < nzs + 4 * 2 * 4 * FQ_LDQ; z += FQ_THREADS) smem[z] = 0.0;   // pad rows stay finite
+    for (int z = tid; z < nzs + 4 * FQ_GRP; z += FQ_THREADS) smem[z] = 0.0;   // pad rows stay finite
     const unsigned zs_u32 = fz_smem_u32(Zs);
-    const unsigned qs_u32 = zs_u32 + 8u * (unsigned)(nzs + grp * 2 * 4 * FQ_LDQ);       // this group's [2][4][FQ_LDQ]
+    const unsigned qs_u32 = zs_u32 + 8u * (unsigned)(nzs + grp * FQ_GRP);                 // this group's Q tiles [2][4][FQ_LDQ]
+    const unsigned s3s_u32 = qs_u32 + 8u * (unsigned)(2 * 4 * FQ_LDQ + lane);             // and S3 fragment tiles [2][3][32], this lane's entry
     // per-lane constants of the fragment addresses (bytes)
     const unsigned z_lane = 8u * (unsigned)(q * ldz + g);                             // A of Q: row l45 = 4 ks + q, column + g
     const unsigned z_ks = 8u * (unsigned)(4 * ldz), z_k4 = 8u * (unsigned)(FQ_L45 * ldz);
-    const unsigned qst_lane = 8u * (unsigned)(wq * FQ_LDQ + g * 16 + 2 * q);          // C of Q: row i5 = 8 i + g, columns 8 j + 2 q, + 1
+    const unsigned qst_lane = 8u * (unsigned)(wq * FQ_LDQ + g * FQ_QI5 + 2 * q);          // C of Q: row i5 = 8 i + g, columns 8 j + 2 q, + 1
     unsigned qld_lane[4];                                                             // B of P: k4 row q, column (i5 i4) = 8 (4 wq + j) + g
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         const int col = min(8 * (4 * wq + j) + g, n54 - 1), i5 = col / n4, i4 = col - i5 * n4;
-        qld_lane[j] = 8u * (unsigned)(q * FQ_LDQ + i5 * 16 + i4);
+        qld_lane[j] = 8u * (unsigned)(q * FQ_LDQ + i5 * FQ_QI5 + i4);
     }
     const int njt = min(4, max(0, NT - 4 * wq));              // live column tiles of this warp
-    const int b4_lane = q * 16 + g;                           // B of Q: row l45 = 4 ks + q, column i4 = 8 j + g
+    const int b4_lane = 2 * lane;                             // B of Q: fragment-major, (column tile 0, 1) adjacent
     unsigned ndm = 0;
 
     for (;;) {
@@ -186,7 +195,7 @@ __global__ void __launch_bounds__(FQ_THREADS, 1) k_fz_qp2(const __grid_constant_
             const int MT3 = (q3hi - q3lo + 7) >> 3;           // <= 3
             // this lane's operand pointers at the first k-step
             const double* s3p = p.S3T + ((((long)b24 * c34 + b34) * c35 + b35) * NX + xg0 + v0 + xl) * (long)(P3 * P4) +
-                                (long)(q3lo + g) * P4 + k4lo + q;                       // A of P: row k3 = q3lo + 8 i + g, column k4
+                                (long)(q3lo + 8 * wq + g) * P4 + k4lo + q;              // A of P, row tile wq: row k3 = q3lo + 8 wq + g, column k4
             const double* b4p = a.Bw4P + (((long)b24 * c34 + b34) * P4 + k4lo + wq) * (FQ_L45 * 16) + b4_lane;
             unsigned zq = zs_u32 + z_lane + 8u * (unsigned)(xl * n5) + (unsigned)(k4lo + wq - h4lo) * z_k4;
 
@@ -196,7 +205,19 @@ __global__ void __launch_bounds__(FQ_THREADS, 1) k_fz_qp2(const __grid_constant_
 #pragma unroll
                 for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-            // Q of one k-step: this warp's k4 = k4lo + 4 gi + wq, into buffer gi & 1 (a zero row beyond the window)
+            // Q of one k-step: this warp's k4 = k4lo + 4 gi + wq, into buffer gi & 1 (a zero row beyond the window); its booster
+            // fragments bq are requested before the barrier that precedes it (b4_fetch)
+            double bq[3][2];
+            auto b4_fetch = [&](int gi) {
+                const bool ok = k4lo + 4 * gi + wq < k4hi;
+#pragma unroll
+                for (int ks = 0; ks < 3; ++ks) {
+                    const double2 v = (ok && ks < KS45) ? __ldg(reinterpret_cast<const double2*>(b4p + ks * 64)) : make_double2(0.0, 0.0);
+                    bq[ks][0] = v.x;
+                    bq[ks][1] = v.y;
+                }
+                b4p += 4 * FQ_L45 * 16;
+            };
             auto q_phase = [&](int gi) {
                 const unsigned dst = qs_u32 + qst_lane + 8u * (unsigned)((gi & 1) * 4 * FQ_LDQ);
                 double c[2][2][2];
@@ -205,44 +226,59 @@ __global__ void __launch_bounds__(FQ_THREADS, 1) k_fz_qp2(const __grid_constant_
 #pragma unroll
                     for (int j = 0; j < 2; ++j) c[i][j][0] = c[i][j][1] = 0.0;
                 if (k4lo + 4 * gi + wq < k4hi) {
-                    double bv[3][2];
-#pragma unroll
-                    for (int ks = 0; ks < 3; ++ks)
-#pragma unroll
-                        for (int j = 0; j < 2; ++j) bv[ks][j] = ks < KS45 ? __ldg(b4p + ks * 64 + j * 8) : 0.0;
 #pragma unroll
                     for (int ks = 0; ks < 3; ++ks) {
                         if (ks < KS45) {
                             const double a0 = fq_lds(zq + ks * z_ks), a1v = fq_lds(zq + ks * z_ks + 64);
-                            fz_dmma(c[0][0][0], c[0][0][1], a0, bv[ks][0]);
-                            fz_dmma(c[0][1][0], c[0][1][1], a0, bv[ks][1]);
-                            fz_dmma(c[1][0][0], c[1][0][1], a1v, bv[ks][0]);
-                            fz_dmma(c[1][1][0], c[1][1][1], a1v, bv[ks][1]);
+                            fz_dmma(c[0][0][0], c[0][0][1], a0, bq[ks][0]);
+                            fz_dmma(c[0][1][0], c[0][1][1], a0, bq[ks][1]);
+                            fz_dmma(c[1][0][0], c[1][0][1], a1v, bq[ks][0]);
+                            fz_dmma(c[1][1][0], c[1][1][1], a1v, bq[ks][1]);
                         }
                     }
                     ndm += 4 * KS45;
                 }
-                b4p += 4 * FQ_L45 * 16;
                 zq += 4 * z_k4;
 #pragma unroll
                 for (int i = 0; i < 2; ++i)
 #pragma unroll
-                    for (int j = 0; j < 2; ++j) fq_sts2(dst + 8u * (unsigned)(i * 128 + j * 8), c[i][j][0], c[i][j][1]);
+                    for (int j = 0; j < 2; ++j) fq_sts2(dst + 8u * (unsigned)(i * 8 * FQ_QI5 + j * 8), c[i][j][0], c[i][j][1]);
+            };
+            // S3 fragments of a k-step: warp i < MT3 of the group fetches the fragment of row tile i (straight from L1/L2; the
+            // {6j} array is zero wherever a triad fails, so rows and columns beyond the unit's windows need no predicate: their
+            // k4 meet zero rows of Q, their k3 are not stored) and leaves it in the group's fragment tile for the other three
+            double s3v = 0.0;                                 // this lane's S3 entry of the next k-step to be staged, fetched one k-step ahead
+            auto s3_fetch = [&]() {
+                if (wq < MT3) s3v = __ldg(s3p);
+                s3p += 4;
+            };
+            auto s3_stage = [&](int gi) {
+                if (wq < MT3)
+                    asm volatile("st.shared.f64 [%0], %1;" ::"r"(s3s_u32 + 8u * (unsigned)(((gi & 1) * 3 + wq) * 32)), "d"(s3v) : "memory");
             };
 
-            fq_group_sync(grp);                               // the group is done with the previous unit's Q tiles
-            if (ng > 0) q_phase(0);
+            if (ng > 0) {
+                b4_fetch(0);
+                s3_fetch();
+            }
+            fq_group_sync(grp);                               // the group is done with the previous unit's tiles
+            if (ng > 0) {
+                s3_stage(0);
+                if (ng > 1) s3_fetch();
+                q_phase(0);
+            }
             for (int gi = 0; gi < ng; ++gi) {
-                // S3 fragments of this k-step straight from L1/L2: zero wherever a triad of the {6j} fails, so rows and
-                // columns beyond the unit's windows need no predicate (their k4 meet zero rows of Q, their k3 are not stored)
-                double av[3];
-#pragma unroll
-                for (int i = 0; i < 3; ++i) av[i] = i < MT3 ? __ldg(s3p + (long)(8 * i) * P4) : 0.0;
-                s3p += 4;
-                fq_group_sync(grp);                           // Q of k-step gi is complete; everybody finished P of gi - 1
-                if (gi + 1 < ng) q_phase(gi + 1);
+                if (gi + 1 < ng) b4_fetch(gi + 1);
+                fq_group_sync(grp);                           // Q and S3 of k-step gi are complete; everybody finished P of gi - 1
+                if (gi + 1 < ng) {
+                    s3_stage(gi + 1);
+                    if (gi + 2 < ng) s3_fetch();
+                    q_phase(gi + 1);
+                }
                 const unsigned bs = qs_u32 + 8u * (unsigned)((gi & 1) * 4 * FQ_LDQ);
-                double bv[4];
+                double av[3], bv[4];
+#pragma unroll
+                for (int i = 0; i < 3; ++i) av[i] = i < MT3 ? fq_lds(s3s_u32 + 8u * (unsigned)(((gi & 1) * 3 + i) * 32)) : 0.0;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) bv[j] = fq_lds(bs + qld_lane[j]);
 #pragma unroll
@@ -289,7 +325,7 @@ bool fz_qp2_supported(const FzParams& p, const SfDims& D)
     const int need = (FQ_XC - 1) * n5 + 16;
     int ldz = ((need + 11) & ~15) + 4;
     if (ldz < need) ldz += 16;
-    return sizeof(double) * ((size_t)P4 * FQ_L45 * ldz + 4 * 2 * 4 * FQ_LDQ) <= 225 * 1024;
+    return sizeof(double) * ((size_t)P4 * FQ_L45 * ldz + 4 * FQ_GRP) <= 225 * 1024;
 }
 
 long fz_qp2_b4p_elems(const FzParams& p, const SfDims& D)
@@ -311,7 +347,7 @@ int fz_launch_qp2(const FzParams& p, const SfDims& D, const double* Bw4P, int* s
     const int need = (FQ_XC - 1) * n5 + 16;                   // last x of a chunk reads 16 rows from its first i5
     a.ldz = ((need + 11) & ~15) + 4;
     if (a.ldz < need) a.ldz += 16;
-    const size_t smem = sizeof(double) * ((size_t)P4 * FQ_L45 * a.ldz + 4 * 2 * 4 * FQ_LDQ);
+    const size_t smem = sizeof(double) * ((size_t)P4 * FQ_L45 * a.ldz + 4 * FQ_GRP);
     a.vc = (p.V + FQ_XC - 1) / FQ_XC;
     const long n_items = (long)a.vc * p.a_cnt * p.box.cnt[2] * p.box.cnt[4];
     if (n_items > 2000000000L) return SF_EARG;
