@@ -14,8 +14,13 @@ N > 1: the path does not shard (north_star: one GPU, no collectives) => N indepe
 The library takes the fastest path that holds the problem (`--path 0`): the factorised path (the sum of eq. (3) taken one
 virtual spin at a time, DESIGN.md 5 K-f); `--path 3` times the per-shell line kernel instead.  Timed region: K asynchronous
 calls between two CUDA events on the call's stream.  `roofline` then comes from a second, instrumented pass of K steps
-(per-kernel CUDA events inside the library) and one call with the kernels' DMMA counters on: achieved = executed FP64
-tensor-pipe flop of the kernel that takes the most time / its event time, against the DMMA peak measured in this process.
+(per-kernel CUDA events inside the library): achieved = USEFUL FP64 flop of the kernel that takes the most time (multiply-
+adds on the index combinations the triangle inequalities allow, counted on the host by sf_factor_work: no tile padding, no
+window rounding) / its event time, against the DMMA peak measured in this process.  The executed DMMA count (padding
+included, from the kernels' own counters) is reported beside it as `executed_over_useful`, never as the fraction.  Because
+the factorised sum is not the per-shell method of the paper, `value` on that path is a shells-EQUIVALENT rate (nominal
+shells of the tensor / time); the per-shell method itself (`--path 3`, SURVEY.md 8(d)'s F_asm + F_con) is timed in the same
+run and reported as `per_shell_path`.
 
 Prints ONE JSON line (rank 0).  `--impl reference` times the oracle (oracle/, plain CPU loops) on the host cores on a
 bounded sample of the same workload.
@@ -37,10 +42,11 @@ if ROOT not in sys.path:
 import workloads as wl  # noqa: E402
 
 METRIC = "eprl_shells_contracted_per_s"
-PATH_NAMES = {1: "staged", 2: "fused", 3: "line", 4: "factorised"}
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch (the heaviest of the three passes over i1) from the committed
-# `ncu --set full` captures of config 3, profiles/r1e_factorised.md; null for any other workload
-NCU_TRAFFIC_CONFIG3 = {"k_fz_qp": 15.13e9, "k_fz_gemm<FzMapR>": 24.15e9, "k_fz_gemm<FzMapA>": 8.73e9}   # r1e, r1g, r1h
+PATH_NAMES = {1: "staged", 3: "line", 4: "factorised"}
+# DRAM traffic per launch comes from the committed ncu launch list of one config-3 step (every kernel of one
+# sf_vertex_amplitude call with dram__bytes_read.sum, dram__bytes_write.sum, gpu__time_duration.sum); null for other workloads
+NCU_LAUNCHES_CONFIG3 = os.path.join("profiles", "r2_config3_step_launches.csv")
+FZ_KERNELS = {"qp": "k_fz_qp", "R": "k_fz_gemm<FzMapR", "A": "k_fz_gemm<FzMapA", "R2": "k_fz_r2"}
 UNIT = "shells/s"
 
 
@@ -214,7 +220,7 @@ def bench_contractions(torch, sf, stream):
     return out
 
 
-def bench_other_workloads(torch, sf, stream):
+def bench_other_workloads(torch, sf, stream, peak):
     """The other four workloads of BASELINE.json in full (north_star: throughput on all five), each a few asynchronous calls
     between two CUDA events: config 0, config 1 at j = 10 (identity boosters, A = N(i) {15j}), config 2 at Delta_l = 8,
     config 4 at lambda = 1..6.  Secondary rows: the headline stays config 3."""
@@ -254,11 +260,69 @@ def bench_other_workloads(torch, sf, stream):
         e1.record(stream)
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / reps
-        rows.append({"workload": c["name"], "shells": nl ** 6, "out_shape": list(n_i), "ms_per_tensor": ms,
-                     "shells_per_s": nl ** 6 / (ms * 1e-3), "tensors_per_s": 1e3 / ms,
-                     "path": PATH_NAMES.get(sf.sf_last_path(), "?"), "finite": bool(torch.isfinite(out).all())})
+        row = {"workload": c["name"], "shells": nl ** 6, "out_shape": list(n_i), "ms_per_tensor": ms,
+               "shells_equivalent_per_s": nl ** 6 / (ms * 1e-3), "tensors_per_s": 1e3 / ms,
+               "path": PATH_NAMES.get(sf.sf_last_path(), "?"), "finite": bool(torch.isfinite(out).all())}
+        if sf.sf_last_path() == 4:      # roofline fraction of the whole call on the useful flop of the factorised chain
+            flop, _, _ = factor_work(sf, two_j, two_dl)
+            useful = sum(flop.values())
+            row["useful_flop"] = useful
+            row["useful_tflops"] = useful / (ms * 1e-3) / 1e12
+            row["frac"] = row["useful_tflops"] / peak
+            row["limiter"] = ("launch latency (about 17 launches per call)" if ms < 0.3 else
+                              "FP64 tensor pipe (alu) with operand latency, see roofline.kernels")
+        rows.append(row)
         del Bdev, out
     return rows
+
+
+
+def hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except (OSError, KeyError, ValueError):
+        return 6550.0, "fallback of B200_PROFILING.md (6550 GB/s copy bandwidth)"
+
+
+def ncu_dram_per_step():
+    """{kernel class: (launches, bytes)} and the total, summed over all launches of one config-3 step, from the committed ncu
+    launch list (profiles/r2_config3_step_launches.csv: one row per launch and metric).  None if the file is absent."""
+    import csv
+    path = os.path.join(ROOT, NCU_LAUNCHES_CONFIG3)
+    if not os.path.exists(path):
+        return None
+    per, total = {}, 0.0
+    with open(path) as fh:
+        rows = [r for r in csv.reader(fh) if len(r) > 5]
+    head = next((r for r in rows if "Kernel Name" in r), None)
+    if head is None:
+        return None
+    k_name, k_metric, k_unit, k_val, k_id = (head.index(c) for c in ("Kernel Name", "Metric Name", "Metric Unit", "Metric Value", "ID"))
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    seen = {}
+    for r in rows:
+        if r is head or not r[k_metric].startswith("dram__bytes_"):
+            continue
+        b = float(r[k_val].replace(",", "")) * scale.get(r[k_unit], 1.0)
+        name = r[k_name].split("(")[0].replace("void ", "")
+        if not name.startswith(("k_fz_", "k_slices", "k_kranges")):
+            continue                                  # the one-off {6j} table build is not part of a step
+        cls = next((c for c, pat in FZ_KERNELS.items() if name.startswith(pat)), "other")
+        n, tot = per.get(cls, (0, 0.0))
+        seen.setdefault(cls, set()).add(r[k_id])
+        per[cls] = (len(seen[cls]), tot + b)
+        total += b
+    return {"per_kernel": {c: {"launches": n, "bytes": b} for c, (n, b) in per.items()}, "total": total,
+            "source": NCU_LAUNCHES_CONFIG3}
+
+
+def factor_work(sf, two_j, two_dl):
+    """Useful flop of the factorised chain per kernel (host integer count, include/sfoam_debug.h) and the algorithmic bytes
+    of its intermediates (every structurally non-zero entry of P and R written once and read once, 8 B each)."""
+    mac, elems = sf.sf_factor_work(two_j, two_dl)
+    flop = {"qp": 2.0 * (mac["Q"] + mac["P"]), "R": 2.0 * mac["R"], "A": 2.0 * mac["A"], "pre": 2.0 * (mac["Z"] + mac["G"])}
+    return flop, mac, elems
 
 
 def run_ours(args, cfg, rank, world, local_rank):
@@ -308,6 +372,13 @@ def run_ours(args, cfg, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if args.one_step_only:      # profiling aid: the {6j} table build and exactly one vertex call, nothing else (ncu launch lists)
+        sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)
+        torch.cuda.synchronize()
+        if rank == 0:
+            print(json.dumps({"one_step_only": True, "workload": cfg["name"], "path": PATH_NAMES.get(sf.sf_last_path(), "?"),
+                              "gpu_launches": sf.sf_launch_count(), "max_abs": float(out.abs().max())}))
+        return
     for _ in range(args.warmup):
         flush.zero_()
         sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)
@@ -379,36 +450,89 @@ def run_ours(args, cfg, rank, world, local_rank):
     peak_dfma, peak_dmma = sf.sf_fp64_peak(0), sf.sf_fp64_peak(1)
     peak = max(peak_dfma, peak_dmma)
     peak_source = ("measured in this process: FP64 DFMA %.2f, DMMA(mma.sync m8n8k4) %.2f TFLOP/s" % (peak_dfma, peak_dmma))
+    hbm, hbm_src = hbm_peak()
+    # {6j} gathers (step 4): the S arrays, 8 B read from the table + 8 B written per element, over the event time of the stage
+    n_s_elems = sf.sf_slice_elems(two_j, two_dl)
+    s_ms = stage[0] / args.steps
+    sixj_gather = {"elements": n_s_elems, "algorithmic_bytes": 16.0 * n_s_elems, "ms_per_step": s_ms,
+                   "achieved": 16.0 * n_s_elems / (s_ms * 1e-3) / 1e9 if s_ms > 0 else None, "peak": hbm, "unit": "GB/s",
+                   "bound": "hbm", "peak_source": hbm_src,
+                   "note": "random 8-byte reads of the canonical table (32-byte sectors) + dense writes"}
+    if sixj_gather["achieved"]:
+        sixj_gather["frac"] = sixj_gather["achieved"] / hbm
     if last_path == 4:
-        # Factorised path.  `achieved` of the dominant kernel = FP64 flop it executes on the tensor pipe (512 per issued
-        # DMMA.8x8x4, counted by the kernel itself) / its CUDA-event time: a pipe-utilisation figure that cannot exceed
-        # the peak.  The path as a whole needs far fewer operations than SURVEY.md 8(d)'s per-shell count, so the
-        # per-shell ("algorithmic") rate is reported beside it and may exceed the peak.
-        names = ["k_fz_qp", "k_fz_gemm<FzMapR>", "k_fz_gemm<FzMapA>"]
+        # Factorised path.  Numerator = USEFUL flop per kernel: 2 x the multiply-adds on the index combinations the triangle
+        # inequalities allow (host count, no padding).  The executed work (512 flop per issued DMMA.8x8x4, counted by the
+        # kernels themselves, padding included) is reported as executed_over_useful, the padding tax.
+        flop, mac, elems = factor_work(sf, two_j, two_dl)
+        names = {"qp": "k_fz_qp2 (Q = sum_l45, P = sum_k4)", "R": "k_fz_gemm<FzMapR> (R = sum_{l34 l35})",
+                 "A": "k_fz_gemm<FzMapA> (A' = sum_{k3 x l23})"}
         per = {}
-        for k, name in enumerate(names):
+        for k, key in enumerate(("qp", "R", "A")):
             ms_k = kms[k] / args.steps
-            tf = 512.0 * dmma[k] / (ms_k * 1e-3) / 1e12 if ms_k > 0 else 0.0
-            per[name] = {"ms_per_step": ms_k, "dmma_per_step": dmma[k], "tflops_executed": tf, "frac": tf / peak}
-        dom = max(names, key=lambda n: per[n]["ms_per_step"])
-        tf_all = 512.0 * sum(dmma) / (sum(kms[:3]) / args.steps * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": dom, "achieved": per[dom]["tflops_executed"], "peak": peak,
+            tf = flop[key] / (ms_k * 1e-3) / 1e12 if ms_k > 0 else 0.0
+            per[key] = {"kernel": names[key], "ms_per_step": ms_k, "useful_flop_per_step": flop[key], "useful_tflops": tf,
+                        "frac": tf / peak, "executed_dmma_per_step": dmma[k],
+                        "executed_over_useful": 512.0 * dmma[k] / flop[key] if flop[key] > 0 else None,
+                        "pipe_busy_frac": 512.0 * dmma[k] / (ms_k * 1e-3) / 1e12 / peak if ms_k > 0 else None}
+        dom = max(per, key=lambda n: per[n]["ms_per_step"])
+        useful_all = sum(flop.values())
+        t_all = sum(kms) / args.steps
+        dram = ncu_dram_per_step() if cfg["name"] == wl.CONFIGS[3]["name"] else None
+        alg_bytes = 8.0 * 2.0 * (elems["P"] + elems["R"])
+        roofline = {"bound": "alu", "kernel": per[dom]["kernel"], "achieved": per[dom]["useful_tflops"], "peak": peak,
                     "unit": "TFLOP/s", "frac": per[dom]["frac"],
-                    "traffic": NCU_TRAFFIC_CONFIG3.get(dom) if cfg["name"] == wl.CONFIGS[3]["name"] else None,
-                    "traffic_source": "ncu --set full, heaviest of the 3 launches per step, profiles/r1e_factorised.md",
+                    "traffic": (dram["per_kernel"].get(dom, {}).get("bytes", 0.0) / max(1, dram["per_kernel"].get(dom, {}).get("launches", 1))
+                                if dram else None),
+                    "traffic_note": "DRAM bytes per launch of the dominant kernel (mean over its launches of one step)",
+                    "traffic_source": dram["source"] if dram else None,
                     "peak_source": peak_source,
-                    "definition": "executed FP64 tensor-pipe flop (512 x issued DMMA.8x8x4, padding included) / event time",
-                    "kernels": per, "all_three": {"tflops_executed": tf_all, "frac": tf_all / peak},
+                    "definition": "useful FP64 flop (2 x multiply-adds on valid index ranges, sf_factor_work) / CUDA-event time",
+                    "kernels": per,
+                    "whole_chain": {"useful_flop_per_step": useful_all, "ms_per_step": t_all,
+                                    "useful_tflops": useful_all / (t_all * 1e-3) / 1e12,
+                                    "frac": useful_all / (t_all * 1e-3) / 1e12 / peak},
                     "precompute_ms_per_step": kms[3] / args.steps,
-                    "per_shell_algorithmic": {"flop_per_step": {"contraction": f_con, "assembly": f_asm},
-                                              "tflops": achieved, "frac": achieved / peak,
-                                              "note": "SURVEY.md 8(d) flop of the per-shell method / time of steps 5-6; "
-                                                      "the factorised sum needs fewer operations, so this exceeds the peak"}}
+                    "hbm": {"algorithmic_bytes_per_step": alg_bytes,
+                            "algorithmic_note": "intermediates P and R written once and read once (8 B per structurally non-zero entry); "
+                                                "inputs and output are < 0.2 GB",
+                            "dram_bytes_per_step": dram["total"] if dram else None,
+                            "dram_per_kernel": dram["per_kernel"] if dram else None,
+                            "hbm_frac": dram["total"] / (ms_step * 1e-3) / 1e9 / hbm if dram else None,
+                            "peak": hbm, "peak_source": hbm_src, "source": dram["source"] if dram else None}}
     else:
-        roofline = {"bound": "alu", "kernel": {2: "k_vertex_fused", 3: "k_vertex_line"}.get(last_path, "k_stage_*"),
+        roofline = {"bound": "alu", "kernel": {3: "k_vertex_line"}.get(last_path, "k_stage_*"),
                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
                     "peak_source": peak_source, "flop_per_step": {"contraction": f_con, "assembly": f_asm},
+                    "definition": "SURVEY.md 8(d): F_con + F_asm on valid ranges / CUDA-event time of steps 5-6(iii)",
                     "kernel_ms": kern_ms}
+    # the per-shell method of the paper (sf_set_path 3: one {15j} assembly and four mode products per shell) on SURVEY.md 8(d)'s
+    # own flop count, timed in this run: 1 warm-up + 2 steps
+    per_shell = None
+    if last_path == 4 and args.path == 0 and cfg["name"] == wl.CONFIGS[3]["name"] and world == 1 and not args.no_extras:
+        try:
+            sf.sf_set_path(3)
+            sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)
+            torch.cuda.synchronize()
+            sf.sf_set_timing(True)
+            st3 = np.zeros(3)
+            for _ in range(2):
+                flush.zero_()
+                sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, stream)
+                st3 += np.array(sf.sf_last_stage_ms())
+            sf.sf_set_timing(False)
+            k3 = st3[1] / 2
+            tf3 = (f_con + f_asm) / (k3 * 1e-3) / 1e12
+            per_shell = {"kernel": "k_vertex_line", "ms_per_step": float(st3.sum() / 2), "kernel_ms": k3,
+                         "flop_per_step": {"contraction": f_con, "assembly": f_asm}, "achieved": tf3, "unit": "TFLOP/s",
+                         "peak": peak, "frac": tf3 / peak, "shells_per_s": n_shells / (st3.sum() / 2 * 1e-3),
+                         "max_abs_diff_vs_factorised_over_max": float(np.abs(out.cpu().numpy() - A_dev).max() / np.abs(A_dev).max()),
+                         "definition": "SURVEY.md 8(d): F_con + F_asm on valid ranges / CUDA-event time of steps 5-6(iii)"}
+        except sf.SfError as e:
+            per_shell = {"unavailable": str(e)}
+        finally:
+            sf.sf_set_timing(False)
+            sf.sf_set_path(args.path)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -423,15 +547,19 @@ def run_ours(args, cfg, rank, world, local_rank):
         "e2e": {"value": whole_job_value(n_shells, args.steps, world, e2e_s), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s / args.steps},
         "gpu_launches": launches,
+        "value_note": ("shells-equivalent: nominal shells of the tensor / time; the factorised path sums eq. (3) spin by spin and "
+                       "never iterates shells (per_shell_path has the per-shell method)" if last_path == 4 else "shells iterated"),
         "roofline": roofline,
+        "per_shell_path": per_shell,
+        "sixj_gather": sixj_gather,
         "stages_ms_per_step": {"s_arrays": stage[0] / args.steps, "assembly_contraction": kern_ms,
                                "accumulate_normalise": stage[2] / args.steps},
         "sixj_table_build_ms": table_ms,
     }
-    if world == 1:
+    if world == 1 and not args.no_extras:
         line["contractions"] = bench_contractions(torch, sf, stream)
         if cfg["name"] == wl.CONFIGS[3]["name"] and args.path == 0:
-            line["other_workloads"] = bench_other_workloads(torch, sf, stream)
+            line["other_workloads"] = bench_other_workloads(torch, sf, stream, peak)
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         n_sample = min(args.ref_shells, n_shells)
@@ -462,7 +590,9 @@ def main():
     ap.add_argument("--table", type=int, default=60, help="two_jmax of the resident {6j} table (-1: none)")
     ap.add_argument("--ref-shells", type=int, default=8000, help="shells in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--path", type=int, default=0, help="0 automatic (fastest that fits), 1 staged, 2 fused, 3 line, 4 factorised")
+    ap.add_argument("--no-extras", action="store_true", help="skip the secondary rows (other workloads, contractions, per-shell path)")
+    ap.add_argument("--one-step-only", action="store_true", help="profiling aid: table build + one vertex call, then exit")
+    ap.add_argument("--path", type=int, default=0, help="0 automatic (fastest that fits), 1 staged, 3 line, 4 factorised")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -26,6 +26,11 @@ int sf_vertex_terms(const int two_j[10], int two_dl, long shell_lo, long shell_h
  * flop = 2 * mac.  SF_EARG / SF_ESPIN as sf_vertex_dims. */
 int sf_factor_work(const int two_j[10], int two_dl, double mac[6], double elems[4]);
 
+/* Entries of the five S arrays of step 4 in the library's dense layout = {6j} symbols gathered (or
+ * evaluated) per vertex call: the unit count of the {6j}-gather bandwidth figure (16 B each: 8 read, 8 written).  -1 on bad
+ * arguments.  Host integer function. */
+long sf_slice_elems(const int two_j[10], int two_dl);
+
 /* FP64 roofline denominators measured in this process: TFLOP/s of dependent-chain microbenchmarks,
  * kind 0 = DFMA (vector FP64 fused multiply-add), kind 1 = DMMA (mma.sync m8n8k4 f64 on the tensor cores).
  * Best of 5 launches of a few ms each; synchronises the default stream.  Requires sf_init. */

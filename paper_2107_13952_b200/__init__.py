@@ -55,6 +55,8 @@ def _lib():
                                         ctypes.POINTER(ctypes.c_double)]
         lib.sf_factor_work.argtypes = [_I10, ctypes.c_int, ctypes.c_double * 6, ctypes.c_double * 4]
         lib.sf_set_factor_budget.argtypes = [ctypes.c_size_t]
+        lib.sf_slice_elems.argtypes = [_I10, ctypes.c_int]
+        lib.sf_slice_elems.restype = ctypes.c_long
         lib.sf_fp64_peak.argtypes = [ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
         lib.sf_vertex_amplitude.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_void_p,
                                             ctypes.c_void_p]
@@ -271,6 +273,11 @@ def sf_factor_work(two_j, two_dl):
     mac, elems = (ctypes.c_double * 6)(), (ctypes.c_double * 4)()
     _check(_lib().sf_factor_work(_spins(two_j), int(two_dl), mac, elems), "sf_factor_work")
     return dict(zip(("Z", "Q", "P", "R", "G", "A"), mac)), dict(zip(("Z", "Q", "P", "R"), elems))
+
+
+def sf_slice_elems(two_j, two_dl):
+    """Entries of the five S arrays of step 4 = {6j} symbols gathered per vertex call (host integer function)."""
+    return int(_lib().sf_slice_elems(_spins(two_j), int(two_dl)))
 
 
 def sf_fp64_peak(kind):

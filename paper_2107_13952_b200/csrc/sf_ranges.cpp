@@ -367,3 +367,14 @@ extern "C" int sf_factor_work(const int two_j[10], int two_dl, double mac[6], do
             }
     return SF_OK;
 }
+
+/* Number of entries of the five S arrays of step 4 in the library's dense layout: the {6j} symbols one
+ * vertex call gathers or evaluates.  Host integer function (include/sfoam_debug.h). */
+extern "C" long sf_slice_elems(const int two_j[10], int two_dl)
+{
+    SfDims D;
+    if (sf_host_dims(two_j, two_dl, &D) != SF_OK) return -1;
+    const long nl = D.nl, n1 = D.n_i[0], NX = D.n_x_pad;
+    const long P2 = D.n_k_pad[0], P3 = D.n_k_pad[1], P4 = D.n_k_pad[2], P5 = D.n_k_pad[3];
+    return nl * n1 * P5 * NX + nl * nl * P4 * P5 * NX + nl * nl * nl * P3 * P4 * NX + nl * nl * P2 * P3 * NX + nl * n1 * P2 * NX;
+}
