@@ -325,6 +325,59 @@ def factor_work(sf, two_j, two_dl):
     return flop, mac, elems
 
 
+def bench_many_vertices(torch, sf, stream, n=1024):
+    """SURVEY.md 8(f) item 1 ("many vertex tensors with few shells"): n config-0 vertex tensors (all spins 1,
+    Delta_l = 2, 729 shells each) through sf_vertex_amplitude_batch -- one kernel launch, one CTA per tensor -- against n
+    single calls; CUDA events on the stream, the {6j} table of the bench resident."""
+    cfg = wl.CONFIGS[0]
+    two_j, two_dl = cfg["two_j"], cfg["two_dl"]
+    nl = two_dl // 2 + 1
+    edge_dims, k_ranges = {}, {}
+    for edge in (2, 3, 4, 5):
+        _, n_i_e, kbase, pad = sf.sf_booster_dims(two_j, two_dl, edge)
+        edge_dims[edge] = (n_i_e, kbase, pad)
+        k_ranges[edge] = sf.sf_booster_kranges(two_j, two_dl, edge)
+    _, n_i = sf.sf_vertex_dims(two_j)
+    Bs, outs = [], []
+    for q in range(n):                                # every tensor has its own boosters (seeded) and its own output
+        B = wl.random_boosters(cfg["seed"] + q, nl, edge_dims, k_ranges)
+        Bs.append([torch.from_numpy(np.ascontiguousarray(B[e])).cuda() for e in (2, 3, 4, 5)])
+        outs.append(torch.zeros(tuple(n_i), dtype=torch.float64, device="cuda"))
+    spins = [two_j] * n
+    for _ in range(3):
+        sf.sf_vertex_amplitude_batch(spins, two_dl, Bs, outs, stream)
+    torch.cuda.synchronize()
+    sf.sf_launch_count(reset=True)
+    reps = 5
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(reps):
+        sf.sf_vertex_amplitude_batch(spins, two_dl, Bs, outs, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    launches = sf.sf_launch_count() // reps
+    ref = torch.zeros(tuple(n_i), dtype=torch.float64, device="cuda")
+    sf.sf_vertex_amplitude(two_j, two_dl, Bs[7], ref, stream)
+    torch.cuda.synchronize()
+    m = 64
+    e0.record(stream)
+    for q in range(m):
+        sf.sf_vertex_amplitude(two_j, two_dl, Bs[q], outs[q], stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    single_ms = e0.elapsed_time(e1) / m
+    sf.sf_vertex_amplitude_batch(spins, two_dl, Bs, outs, stream)
+    torch.cuda.synchronize()
+    return {"workload": f"{n} x {cfg['name']}", "tensors": n, "ms_per_batch": ms, "tensors_per_s": n / (ms * 1e-3),
+            "launches_per_batch": launches, "single_call_ms_per_tensor": single_ms,
+            "single_call_tensors_per_s": 1e3 / single_ms, "speedup_over_single_calls": single_ms * n / ms,
+            "max_abs_diff_vs_single_over_max": float((outs[7] - ref).abs().max() / ref.abs().max()),
+            "kernel": "k_vertex_batch (one CTA per tensor; FP64 FMA, S arrays and all intermediates in shared memory)",
+            "limiter": "instruction issue / shared-memory latency: index arithmetic of the irregular ranges dominates the "
+                       "3.4e6 flop per tensor"}
+
+
 def run_ours(args, cfg, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -560,6 +613,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         line["contractions"] = bench_contractions(torch, sf, stream)
         if cfg["name"] == wl.CONFIGS[3]["name"] and args.path == 0:
             line["other_workloads"] = bench_other_workloads(torch, sf, stream, peak)
+            line["many_vertices"] = bench_many_vertices(torch, sf, stream)
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         n_sample = min(args.ref_shells, n_shells)

@@ -121,6 +121,17 @@ int sf_vertex_amplitude_range(const int two_j[10], int two_dl, const sf_boosters
  * the corresponding sub-block of the full tensor.  SF_EARG if a range leaves the node's range or a count is < 1. */
 int sf_vertex_amplitude_intertwiners(const int two_j[10], int two_dl, const sf_boosters *boosters,
                                      const int i_first[5], const int i_count[5], double *out, sf_stream_t stream);
+/* Many vertex tensors in one call (the paper's stated next step, "many vertex tensors with few shells"; graphs
+ * with internal faces need one small tensor per value of the bulk spins).  Problem q = 0..n-1 has the boundary
+ * spins two_j[10 q .. 10 q + 9], the shell count two_dl[q], the boosters boosters[q] and the output out[q], each exactly as in
+ * sf_vertex_amplitude.  two_j, two_dl, boosters and out are HOST arrays (of spins, of device-pointer quadruples and of device
+ * pointers); they may be freed when the call returns.  Every tensor whose {6j} arrays and per-shell intermediates fit one SM's
+ * shared memory (small spins, few shells) is computed by ONE kernel launch, one CTA per tensor, everything on chip; larger ones
+ * are computed afterwards by the single-tensor path.  Asynchronous on `stream`; bitwise reproducible; uses no library scratch
+ * for the small tensors, so batches on different streams may overlap.  All arguments are validated before anything is
+ * launched: on SF_EARG / SF_ESPIN no output is written. */
+int sf_vertex_amplitude_batch(int n, const int *two_j, const int *two_dl, const sf_boosters *boosters,
+                              double *const *out, sf_stream_t stream);
 /* End-to-end variant with HOST buffers (pinned or pageable): copies the four boosters to the device, computes, copies
  * the tensor back and synchronises `stream`.  host_boosters[e] holds n_triples*n_i*n_k_pad doubles. */
 int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const double *const host_boosters[4],

@@ -64,6 +64,8 @@ def _lib():
                                                   ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
         lib.sf_vertex_amplitude_intertwiners.argtypes = [_I10, ctypes.c_int, ctypes.POINTER(_Boosters), ctypes.c_int * 5,
                                                          ctypes.c_int * 5, ctypes.c_void_p, ctypes.c_void_p]
+        lib.sf_vertex_amplitude_batch.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                                  ctypes.c_void_p]
         lib.sf_contract_vertices.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
         lib.sf_contract_vectors.argtypes = [ctypes.c_void_p, ctypes.c_int * 5, ctypes.c_void_p * 5, ctypes.c_void_p,
                                             ctypes.c_void_p]
@@ -326,6 +328,28 @@ def sf_vertex_amplitude_intertwiners(two_j, two_dl, boosters, i_first, i_count, 
     _check(_lib().sf_vertex_amplitude_intertwiners(_spins(two_j), int(two_dl), ctypes.byref(b), first, count, _ptr(out),
                                                    _stream(stream)), "sf_vertex_amplitude_intertwiners")
     return out
+
+
+def sf_vertex_amplitude_batch(two_j, two_dl, boosters, outs, stream=None):
+    """Many vertex tensors in one call (PAPER.md:581).  two_j: n lists of ten spins; two_dl: n ints (or one int for all);
+    boosters: n quadruples of DEVICE tensors (edges 2..5); outs: n DEVICE float64 tensors, overwritten.  Small tensors are
+    computed by one kernel launch (one CTA each), larger ones by the single-tensor path afterwards."""
+    n = len(two_j)
+    if isinstance(two_dl, int):
+        two_dl = [two_dl] * n
+    if not (len(two_dl) == len(boosters) == len(outs) == n):
+        raise ValueError("two_j, two_dl, boosters and outs must have the same length")
+    spins = (ctypes.c_int * (10 * n))(*[int(s) for tj in two_j for s in tj])
+    dls = (ctypes.c_int * n)(*[int(d) for d in two_dl])
+    barr = (_Boosters * n)()
+    for q, b4 in enumerate(boosters):
+        if isinstance(b4, dict):
+            b4 = [b4[e] for e in (2, 3, 4, 5)]
+        for e, t in enumerate(b4):
+            barr[q].B[e] = t.data_ptr() if hasattr(t, "data_ptr") else int(t)
+    optr = (ctypes.c_void_p * n)(*[o.data_ptr() if hasattr(o, "data_ptr") else int(o) for o in outs])
+    _check(_lib().sf_vertex_amplitude_batch(n, spins, dls, barr, optr, _stream(stream)), "sf_vertex_amplitude_batch")
+    return outs
 
 
 def sf_contract_vertices(a, b, result, stream=None):

@@ -315,6 +315,23 @@ extern "C" int sf_vertex_amplitude_intertwiners(const int two_j[10], int two_dl,
     return vertex_range(two_j, two_dl, boosters, 0, 0, out, (cudaStream_t)stream, true, i_first, i_count);
 }
 
+int sf_vertex_single(const int two_j[10], int two_dl, const sf_boosters* boosters, double* out, cudaStream_t st)
+{
+    return vertex_range(two_j, two_dl, boosters, 0, 0, out, st, true);
+}
+
+int sf_vertex_batch_run(int n, const int* two_j, const int* two_dl, const sf_boosters* boosters, double* const* out,
+                        cudaStream_t st);   // sf_vertex_batch.cu
+
+extern "C" int sf_vertex_amplitude_batch(int n, const int* two_j, const int* two_dl, const sf_boosters* boosters,
+                                         double* const* out, sf_stream_t stream)
+{
+    if (!g_ctx.init) return SF_ENOTINIT;
+    if (n < 0 || (n > 0 && (!two_j || !two_dl || !boosters || !out))) return SF_EARG;
+    if (n == 0) return SF_OK;
+    return sf_vertex_batch_run(n, two_j, two_dl, boosters, out, (cudaStream_t)stream);
+}
+
 extern "C" int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const double* const host_boosters[4],
                                         double* host_out, sf_stream_t stream)
 {

@@ -11,6 +11,7 @@
 // layout, xx = (x - x_base) over the union range of x.  Entries whose triads fail are 0.  Values are gathered from
 // the resident canonical table when every argument fits in it, and evaluated directly otherwise.
 #include "sf_sixj.cuh"
+#include "sf_slices.cuh"
 
 void sf_slice_sizes(const SfDims& D, SfSliceSizes* sz)
 {
@@ -21,68 +22,6 @@ void sf_slice_sizes(const SfDims& D, SfSliceSizes* sz)
     sz->n[2] = nl * nl * nl * P3 * P4 * NX;
     sz->n[3] = nl * nl * P2 * P3 * NX;
     sz->n[4] = nl * n1 * P2 * NX;
-}
-
-struct SliceArgs {
-    int two_j[10];
-    int nl, n1, two_i1_min;
-    int two_k_base[4], n_k_pad[4];
-    int two_x_base, n_x_pad;
-    long n[5];
-    double* S[5];
-};
-
-template <int WHICH>
-__device__ __forceinline__ void slice_args(const SliceArgs& A, long q, int& a, int& b, int& c, int& d, int& e, int& f)
-{
-    const int NX = A.n_x_pad, nl = A.nl;
-    const int x = A.two_x_base + 2 * (int)(q % NX);
-    q /= NX;
-    const int* j = A.two_j;
-    if (WHICH == 0) {          // S1[o25][a1][q5][xx] = {i1 l25 x; k5 j14 j15}
-        const int k5 = A.two_k_base[3] + 2 * (int)(q % A.n_k_pad[3]);
-        q /= A.n_k_pad[3];
-        const int i1 = A.two_i1_min + 2 * (int)(q % A.n1);
-        q /= A.n1;
-        const int l25 = j[J25] + 2 * (int)q;
-        a = i1; b = l25; c = x; d = k5; e = j[J14]; f = j[J15];
-    } else if (WHICH == 1) {   // S2[o35][o45][q4][q5][xx] = {j14 k5 x; l35 k4 l45}
-        const int k5 = A.two_k_base[3] + 2 * (int)(q % A.n_k_pad[3]);
-        q /= A.n_k_pad[3];
-        const int k4 = A.two_k_base[2] + 2 * (int)(q % A.n_k_pad[2]);
-        q /= A.n_k_pad[2];
-        const int l45 = j[J45] + 2 * (int)(q % nl);
-        q /= nl;
-        const int l35 = j[J35] + 2 * (int)q;
-        a = j[J14]; b = k5; c = x; d = l35; e = k4; f = l45;
-    } else if (WHICH == 2) {   // S3[o24][o34][o35][q3][q4][xx] = {k4 l35 x; k3 l24 l34}
-        const int k4 = A.two_k_base[2] + 2 * (int)(q % A.n_k_pad[2]);
-        q /= A.n_k_pad[2];
-        const int k3 = A.two_k_base[1] + 2 * (int)(q % A.n_k_pad[1]);
-        q /= A.n_k_pad[1];
-        const int l35 = j[J35] + 2 * (int)(q % nl);
-        q /= nl;
-        const int l34 = j[J34] + 2 * (int)(q % nl);
-        q /= nl;
-        const int l24 = j[J24] + 2 * (int)q;
-        a = k4; b = l35; c = x; d = k3; e = l24; f = l34;
-    } else if (WHICH == 3) {   // S4[o23][o24][q2][q3][xx] = {l24 k3 x; j13 k2 l23}
-        const int k3 = A.two_k_base[1] + 2 * (int)(q % A.n_k_pad[1]);
-        q /= A.n_k_pad[1];
-        const int k2 = A.two_k_base[0] + 2 * (int)(q % A.n_k_pad[0]);
-        q /= A.n_k_pad[0];
-        const int l24 = j[J24] + 2 * (int)(q % nl);
-        q /= nl;
-        const int l23 = j[J23] + 2 * (int)q;
-        a = l24; b = k3; c = x; d = j[J13]; e = k2; f = l23;
-    } else {                   // S5[o25][a1][q2][xx] = {k2 j13 x; i1 l25 j12}
-        const int k2 = A.two_k_base[0] + 2 * (int)(q % A.n_k_pad[0]);
-        q /= A.n_k_pad[0];
-        const int i1 = A.two_i1_min + 2 * (int)(q % A.n1);
-        q /= A.n1;
-        const int l25 = j[J25] + 2 * (int)q;
-        a = k2; b = j[J13]; c = x; d = i1; e = l25; f = j[J12];
-    }
 }
 
 template <int WHICH>
