@@ -741,6 +741,9 @@ __global__ void __launch_bounds__(WGM* WGN * 32) k_fz_gemm(const FzParams p, int
                 const unsigned rowb = (unsigned)(((M + 1) & ~1) * 8);
                 if (warp == 0) {
                     const unsigned bar = fz_smem_u32(&abar[s]);
+                    // rows of this stage were zero-filled with generic stores two chunks ago (ordered by the CTA barrier):
+                    // make them visible to the asynchronous proxy before the bulk copies overwrite the stage
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                     if (lane == 0) fz_mbar_expect_tx(bar, rowb * (unsigned)kv);
                     __syncwarp();
                     for (int kr = lane; kr < kv; kr += 32)
