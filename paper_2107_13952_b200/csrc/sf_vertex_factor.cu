@@ -52,7 +52,7 @@ __global__ void k_fz_windows(SfProblem P, int2* w3A, int2* w3B, int2* w4A, int2*
 }
 
 // Z[b25][a1][b35][b45][q4][v][i5] = (-1)^(o25+o35+o45+q4) sum_{k5 valid} (-1)^q5 {j14 k5 x; l35 k4 l45} {i1 l25 x; k5 j14 j15} (2k5+1) B5[t5][i5][q5]
-// one CTA per (b25, a1, b35, b45)
+// one CTA per (b25, a1, b35, b45) and k4 (grid.y): single-shell problems (Delta_l = 0, large spins) have few (l25 l35 l45)
 __global__ void __launch_bounds__(256) k_fz_z(FzParams p, double* __restrict__ Z)
 {
     const SfProblem& P = p.P;
@@ -70,10 +70,12 @@ __global__ void __launch_bounds__(256) k_fz_z(FzParams p, double* __restrict__ Z
     const SfKRange r5 = P.kr[3][t5];
     const int q5b = (r5.two_k_min - P.two_k_base[3]) >> 1;
     double* z = Z + (long)blockIdx.x * P4 * V * n5;
-    for (int e = threadIdx.x; e < P4 * nxs * n5; e += blockDim.x) {
-        const int i5 = e % n5, r = e / n5, v = r % nxs, q4 = r / nxs;
+    const int nq4 = (P4 - (int)blockIdx.y + (int)gridDim.y - 1) / (int)gridDim.y;      // the k4 of this CTA: blockIdx.y + gridDim.y * n
+    const double* s1b = P.S[0] + (((long)(o25 * n1 + a1) * P5 + q5b) * NX) + xg0;
+    for (int e = threadIdx.x; e < nq4 * nxs * n5; e += blockDim.x) {
+        const int i5 = e % n5, r = e / n5, v = r % nxs, q4 = blockIdx.y + gridDim.y * (r / nxs);
         const double* s2 = P.S[1] + ((((long)(o35 * nl + o45) * P4 + q4) * P5 + q5b) * NX) + xg0 + v;
-        const double* s1 = P.S[0] + (((long)(o25 * n1 + a1) * P5 + q5b) * NX) + xg0 + v;
+        const double* s1 = s1b + v;
         const double* b5 = sf_brow(P, 3, t5, i5) + q5b;
         double val = 0.0;
         for (int c = 0; c < r5.n_k; ++c) {
@@ -1156,7 +1158,11 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             SF_CUDA_OK(cudaMemsetAsync(G, 0xFF, sizeof(double) * (size_t)nG, st));
         }
         fz_ev_begin(3, st);
-        k_fz_z<<<(unsigned)(c25 * n1 * c35 * c45), 256, 0, st>>>(p, Z);
+        {   // few (l25 i1 l35 l45): spread the k4 over grid.y as well
+            const long nz = c25 * n1 * c35 * c45;
+            const int gy = nz >= 592 ? 1 : (int)((592 + nz - 1) / nz < P4 ? (592 + nz - 1) / nz : P4);
+            k_fz_z<<<dim3((unsigned)nz, (unsigned)gy), 256, 0, st>>>(p, Z);
+        }
         if (qp2) {
             fz_launch_b4p(p, nB4, B4, st);
             SF_CUDA_OK(cudaMemsetAsync(S3 + nS3, 0, sizeof(double) * (size_t)padS3, st));
