@@ -62,7 +62,8 @@ void sf_set_staged_budget(unsigned long bytes);
 void sf_set_factor_budget(unsigned long bytes);
 
 /* Kernel variants of the factorised path, for cross-checks and A/B timing: bit 0 = take the edge-3 contraction (R) through
- * the booster-stationary kernel (sf_factor_r.cu) instead of the general gather-GEMM; bit 1 = take Q/P through the first-generation kernel.
+ * the booster-stationary kernel (sf_factor_r.cu) instead of the general gather-GEMM; bit 1 = take Q/P through the first-generation kernel
+ * (k_fz_qp); bit 2 = take Q/P through the second-generation kernel (k_fz_qp2) instead of the warp-autonomous one (k_fz_qp4).
  * 0 = default (the fastest kernels that hold the shape).  All variants compute the same sums. */
 void sf_set_factor_variant(int bits);
 

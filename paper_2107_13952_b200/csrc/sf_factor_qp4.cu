@@ -1,0 +1,383 @@
+// sf_factor_qp4.cu -- the edge-4 contraction of the factorised path (sf_vertex_factor.cu, DESIGN.md 5 K-f), warp-autonomous kernel:
+//
+//   Q[k4; i5 i4]            = sum_l45 Z[l25 i1 l35 l45; k4 x i5] Bw4P[l24 l34; k4; l45; i4]      (the shells of a line l45)
+//   P[k3; (i5 i4)]          = sum_k4  S3T[l24 l34 l35; x; k3 k4] Q[k4; i5 i4]                    (third {6j} of eq. (5), edge-4 product)
+//
+// for every (i1 l25 l35 | l24 l34 | x): steps 6(i)-(iii) of the algorithm for the factors of eq. (3) that
+// carry l45 and k4.  Q never leaves the chip; the rows of P the triads allow go to HBM for the edge-3 contraction.
+//
+// k_fz_qp2 (sf_factor_qp.cu) shares a unit (l24 l34 x) among four warps: ~60 MMA per warp between two named barriers, 15
+// issued instructions per MMA, the FP64 tensor pipe 40 % busy.  Here ONE warp owns a unit from its first k4 to its rows of P:
+//   * a CTA (8 warps, one per SM) takes items (i1, l25, l35, chunk of <= 4 x) from an atomic counter (execution order only:
+//     every row of P has one writer) and keeps the item's slab of Z in shared memory, as k_fz_qp2 does;
+//   * the windows of every unit of the item are computed once, cooperatively, into a descriptor table in shared memory (units
+//     with more than 16 rows k3 are split in two, so that a warp holds two row tiles x 16 column tiles = 128 accumulator
+//     registers); the warps draw units from a shared-memory counter;
+//   * per k-step of 4 k4 the warp computes Q for the four k4 (2 x 2 tiles each, only over the k-steps of l45 that the triad
+//     (k4 l45 j14) allows: both operands are exactly zero elsewhere) into its PRIVATE tile [4][n5 n4] (compact, row stride = 4
+//     mod 16: conflict-free B fragments), __syncwarp, then accumulates all 16 column tiles of P from that tile: 50-64
+//     independent MMA per k-step and no barrier other than the warp's own;
+//   * the booster fragments of a k-step (4 k4 x 1536 contiguous bytes of Bw4P) arrive by ONE bulk asynchronous copy
+//     (cp.async.bulk = SASS UBLKCP, completion on the warp's own mbarrier) into the warp's slot, issued as soon as the Q phase
+//     has read the slot, so that the copy runs under the P phase; S3 fragments come straight from L1/L2 into registers, one
+//     k-step ahead, their lines sent for into L1 a whole unit earlier.
+//
+// Shapes it holds: those of k_fz_qp2 with c24 c34 <= 256.  sf_vertex_factor falls back to k_fz_qp2 / k_fz_qp otherwise.
+#include "sf_factor.cuh"
+
+#define F4_THREADS 256
+#define F4_WARPS 8
+#define F4_XC 4                   // x values per item
+#define F4_L45 12                 // l45 rows per k4 in the Z slab and in Bw4P (3 k-steps)
+#define F4_LDQ 132                // row stride of a Q tile: >= 128 columns, = 4 mod 16
+#define F4_BSLOT (4 * F4_L45 * 16) // doubles of booster fragments per k-step
+#define F4_MAXU 1024              // units (l24 l34 x) per item; as many overflow units (rows k3 beyond the first 16)
+
+struct FzQp4Args {
+    int ldz;                      // row stride of the Z slab (= 4 mod 16)
+    int vc;                       // chunks of F4_XC x per (i1 l25)
+    int n_items;
+    int* sched;
+    const double* Bw4P;           // [b24][b34][q4][k-step 3][lane 32][column tile 2], see k_fz_b4p (sf_factor_qp.cu)
+};
+
+__device__ __forceinline__ double f4_lds(unsigned addr)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void f4_sts(unsigned addr, double a)
+{
+    asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(a) : "memory");
+}
+
+// LDZ = row stride of the Z slab: 52 for n5 <= 12, else 68 (= 4 mod 16, >= 3 n5 + 16)
+template <int LDZ>
+__global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant__ FzParams p, const __grid_constant__ FzQp4Args a)
+{
+    extern __shared__ __align__(16) double smem[];
+    __shared__ int s_item, s_next;
+    __shared__ int2 s_unit[2 * F4_MAXU];                      // per (b24, b34, x) and its overflow: packed windows, see below
+    __shared__ __align__(8) unsigned long long s_bar[F4_WARPS];   // per warp: completion of the bulk copy into its booster slot
+    __shared__ int s_ksr[32];                                 // per q4: k-steps [lo, hi) of the l45 the triad (k4 l45 j14) allows
+    const SfProblem& P = p.P;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
+    const int nl = P.nl, n1 = P.n_i[0], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5;
+    const int P3 = P.n_k_pad[1], P4 = P.n_k_pad[2], NX = P.n_x_pad, V = p.V, NP = p.NP;
+    const int c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4], c45 = p.box.cnt[5];
+    constexpr int ldz = LDZ, ldq = F4_LDQ;
+    const int NT = (n54 + 7) >> 3;
+    const bool two4 = n4 > 8, two5 = n5 > 8;                  // a second tile of i4 / of i5 in the Q phase
+    const int sZ = P4 * V * n5;
+    const long prow = (long)c34 * c35 * NP;                   // stride of v in P
+    const int nzs = P4 * F4_L45 * ldz;
+    for (int z = tid; z < nzs + F4_WARPS * (4 * ldq + F4_BSLOT); z += F4_THREADS) smem[z] = 0.0;   // pad rows and columns stay finite
+    if (lane == 0) fz_mbar_init(fz_smem_u32(&s_bar[warp]), 1);
+    if (tid == 0) asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the zeroed slots are next written by bulk copies
+    if (tid < 32) {
+        int lo = 3, hi = 0;
+        if (tid < P4)
+            for (int b45 = 0; b45 < c45; ++b45) {
+                const int2 w = p.w4B[p.box.lo[5] + b45];
+                if (tid >= w.x && tid < w.x + w.y) {
+                    lo = min(lo, b45 >> 2);
+                    hi = max(hi, (b45 >> 2) + 1);
+                }
+            }
+        s_ksr[tid] = hi > lo ? (lo | (hi << 8)) : 0;
+    }
+    const unsigned zs_u32 = fz_smem_u32(smem);                // Zs[P4][F4_L45][ldz]
+    const unsigned qs_u32 = zs_u32 + 8u * (unsigned)(nzs + warp * (4 * ldq + F4_BSLOT));   // this warp's Q tile [4][ldq]
+    const unsigned bs_u32 = qs_u32 + 8u * (unsigned)(4 * ldq);                           // and booster slot [4 k4][3 k-steps][32 lanes][2]
+    const unsigned bar_u32 = fz_smem_u32(&s_bar[warp]);
+    unsigned bphase = 0;                                      // parity of the next completion of the warp's mbarrier
+    // per-lane constants of the fragment addresses (bytes)
+    const unsigned z_lane = zs_u32 + 8u * (unsigned)(q * ldz + g);                    // A of Q: row l45 = 4 ks + q, column + g
+    constexpr unsigned z_ks = 8u * (unsigned)(4 * ldz), z_k4 = 8u * (unsigned)(F4_L45 * ldz);
+    // C of Q: rows i5 = g, 8 + g; columns i4 = 2 q, 2 q + 1, 8 + 2 q, 9 + 2 q; smask: which of the 2 x 4 entries exist
+    const unsigned qst_lane = qs_u32 + 8u * (unsigned)(g * n4 + 2 * q);
+    unsigned smask = 0;
+#pragma unroll
+    for (int t = 0; t < 2; ++t)
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+            if (8 * t + g < n5 && 8 * (e >> 1) + 2 * q + (e & 1) < n4) smask |= 1u << (4 * t + e);
+    const unsigned qld_lane = qs_u32 + 8u * (unsigned)(q * ldq + g);                  // B of P: k4 row q, column 8 j + g
+    unsigned pmask = 0;                                       // column pairs 8 j + 2 q of P this lane stores
+#pragma unroll
+    for (int j = 0; j < 16; ++j)
+        if (8 * j + 2 * q < n54) pmask |= 1u << j;
+    const unsigned b4_lane = bs_u32 + 16u * (unsigned)lane;   // B of Q: fragment-major, (column tile 0, 1) adjacent
+    unsigned ndm = 0;
+
+    for (;;) {
+        __syncthreads();                                      // everybody is done with the previous slab of Z and the tables
+        if (tid == 0) {
+            s_item = atomicAdd(a.sched, 1);
+            s_next = 0;
+        }
+        __syncthreads();
+        int it = s_item;
+        if (it >= a.n_items) break;
+        const int b35 = it % c35; it /= c35;
+        const int b25 = it % c25; it /= c25;
+        const int ac = it % p.a_cnt;
+        const int vc = it / p.a_cnt;
+        const int a1 = p.a_lo + ac, o25 = p.box.lo[2] + b25, o35 = p.box.lo[4] + b35;
+        int x0, nxs, xg0;
+        fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
+        const int v0 = vc * F4_XC, nv = min(F4_XC, nxs - v0);
+        if (nv <= 0) continue;
+        const int l35 = P.two_j[J35] + 2 * o35;
+        // k4 of the item: the union over its x of the triad (k4 l35 x), inside the l45 the box holds
+        int h4lo = P4, h4hi = 0;
+        for (int vv = 0; vv < nv; ++vv) {
+            const int2 w = fz_window(l35, x0 + 2 * (v0 + vv), P.two_k_base[2], P4);
+            if (w.y > 0) {
+                h4lo = min(h4lo, w.x);
+                h4hi = max(h4hi, w.x + w.y);
+            }
+        }
+        h4lo = max(h4lo, p.hull4B.x);
+        h4hi = min(h4hi, p.hull4B.y);
+        // the slab of Z: rows (k4, l45), nv * n5 entries (x i5) each
+        {
+            const double* Zb = p.Z + ((((long)b25 * n1 + a1) * c35 + b35) * c45) * (long)sZ + (long)v0 * n5;
+            const int rowlen = nv * n5, nrow = max(0, h4hi - h4lo) * c45;
+            for (int r = warp; r < nrow; r += F4_WARPS) {
+                const int r4 = r / c45, b45 = r - r4 * c45;
+                const double* src = Zb + ((long)b45 * P4 + h4lo + r4) * (V * n5);
+                const unsigned dst = zs_u32 + 8u * (unsigned)((r4 * F4_L45 + b45) * ldz);
+                for (int c = lane; c < rowlen; c += 32) fz_cp_async8(dst + 8u * c, src + c, 8);
+            }
+            fz_cp_commit();
+        }
+        // the units (b24, b34, x) of the item: rows k3 = (k3 l34 l35) and the triad (k3 l24 x); k4 = (k4 l24 l34), the triad
+        // (k4 l35 x), and the l45 of the box.  At most 16 rows per unit; rows beyond go to the overflow unit nun + u.
+        //   .x = q3lo | n3 << 8 | k4lo << 16 | k4hi << 24        .y = b24 | b34 << 8 | x << 16 | valid << 24
+        const int nun = c24 * c34 * nv;
+        for (int u = tid; u < nun; u += F4_THREADS) {
+            const int xl = u % nv, r = u / nv, b34 = r % c34, b24 = r / c34;
+            const int o24 = p.box.lo[1] + b24, o34 = p.box.lo[3] + b34;
+            const int x = x0 + 2 * (v0 + xl);
+            const int2 w3 = p.w3A[o34 * nl + o35], w4a = p.w4A[o24 * nl + o34];
+            const int2 wx = fz_window(P.two_j[J24] + 2 * o24, x, P.two_k_base[1], P3);
+            const int2 w4x = fz_window(l35, x, P.two_k_base[2], P4);
+            const int q3lo = max(wx.x, w3.x), q3hi = (wx.y > 0 && w3.y > 0) ? min(wx.x + wx.y, w3.x + w3.y) : 0;
+            const int n3 = max(0, q3hi - q3lo);
+            const int k4lo = max(max(w4a.x, w4x.x), h4lo);
+            int k4hi = (w4a.y > 0 && w4x.y > 0) ? min(min(w4a.x + w4a.y, w4x.x + w4x.y), h4hi) : 0;
+            if (k4hi < k4lo) k4hi = k4lo;
+            const int k4w = (k4lo << 16) | (k4hi << 24), id = b24 | (b34 << 8) | (xl << 16);
+            s_unit[u] = make_int2(q3lo | (min(n3, 16) << 8) | k4w, id | (n3 > 0 ? 1 << 24 : 0));
+            s_unit[nun + u] = make_int2((q3lo + 16) | (max(n3 - 16, 0) << 8) | k4w, id | (n3 > 16 ? 1 << 24 : 0));
+        }
+        fz_cp_wait<0>();
+        __syncthreads();
+
+        // units from the item's counter, one per warp at a time; the next unit is drawn one unit ahead, so that the S3 rows
+        // it will ask for can be sent for into L1 a whole unit earlier
+        auto draw = [&]() {
+            int u = 0;
+            if (lane == 0) u = atomicAdd(&s_next, 1);
+            return __shfl_sync(0xffffffffu, u, 0);
+        };
+        const long s3item = ((long)b35 * NX + xg0 + v0) * (long)(P3 * P4);
+        for (int u = draw(), un; u < 2 * nun; u = un) {
+            un = draw();
+            if (un < 2 * nun) {
+                const int2 dn = s_unit[un];
+                if (dn.y >> 24) {
+                    const int q3n = dn.x & 255, k4n0 = (dn.x >> 16) & 255, k4n1 = (dn.x >> 24) & 255;
+                    const long pr = (long)(dn.y & 255) * c34 + ((dn.y >> 8) & 255);
+                    const double* s3r = p.S3T + (pr * c35 * NX + ((dn.y >> 16) & 255)) * (long)(P3 * P4) + s3item + (long)(q3n + (lane & 15)) * P4;
+                    fz_prefetch_l1(s3r + (lane < 16 ? k4n0 : max(k4n1 - 1, k4n0)));
+                }
+            }
+            const int2 d = s_unit[u];
+            if (!(d.y >> 24)) continue;                       // no rows of P
+            const int q3lo = d.x & 255, n3 = (d.x >> 8) & 255, k4lo = (d.x >> 16) & 255, k4hi = (d.x >> 24) & 255;
+            const int b24 = d.y & 255, b34 = (d.y >> 8) & 255, xl = (d.y >> 16) & 255;
+            const int ng = (k4hi - k4lo + 3) >> 2;
+            const bool two3 = n3 > 8;                         // a second row tile of k3
+            // this lane's operand pointers at the first k4
+            const double* s3p = p.S3T + ((((long)b24 * c34 + b34) * c35 + b35) * NX + xg0 + v0 + xl) * (long)(P3 * P4) + (long)(q3lo + g) * P4 +
+                                k4lo + q;                     // A of P: row k3 = q3lo + 8 i + g, column k4
+            const double* b4g = a.Bw4P + (((long)b24 * c34 + b34) * P4 + k4lo) * (F4_L45 * 16);   // the unit's first k-step of fragments
+            unsigned zq = z_lane + 8u * (unsigned)(xl * n5) + (unsigned)(k4lo - h4lo) * z_k4;
+
+            double acc[2][16][2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < 16; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+            // one bulk copy per k-step into the warp's slot (every lane has read the slot: __syncwarp before)
+            auto b4_copy = [&]() {
+                if (lane == 0) {
+                    fz_mbar_expect_tx(bar_u32, 8u * F4_BSLOT);
+                    fz_bulk_g2s(bs_u32, b4g, 8u * F4_BSLOT, bar_u32);
+                }
+                b4g += F4_BSLOT;
+            };
+            // the {6j} array is exactly zero wherever a triad fails, so rows and columns beyond the unit's windows need no predicate:
+            // their k4 meet zero rows of Q or zero entries of S3, their k3 are not stored
+            double s3n[2];
+            auto s3_fetch = [&]() {
+                s3n[0] = __ldg(s3p);
+                s3n[1] = two3 ? __ldg(s3p + 8 * P4) : 0.0;
+                s3p += 4;
+            };
+            if (ng > 0) {
+                __syncwarp();                                 // the previous unit's last Q phase has read the slot
+                b4_copy();
+                s3_fetch();
+            }
+            for (int gi = 0; gi < ng; ++gi) {
+                fz_mbar_wait(bar_u32, bphase);                // the booster fragments of this k-step have landed
+                bphase ^= 1u;
+                // ---- Q of the four k4 of this k-step into the warp's tile (the P phase of the previous k-step has read it: the
+                // __syncwarp below, after that phase).  k4 beyond the window get a zero row: their booster fragments are not used ----
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk) {
+                    const int k4 = k4lo + 4 * gi + kk;
+                    const int ksr = k4 < k4hi ? s_ksr[k4] : 0;
+                    const int klo = ksr & 255, khi = ksr >> 8;
+                    double c[2][2][2];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) c[t][0][0] = c[t][0][1] = c[t][1][0] = c[t][1][1] = 0.0;
+                    if (khi > klo) {                          // uniform: all three k-steps of l45 (zeros outside [klo, khi))
+                        double af[3][2];
+                        double2 bf[3];
+#pragma unroll
+                        for (int ks = 0; ks < 3; ++ks) {
+                            af[ks][0] = f4_lds(zq + kk * z_k4 + ks * z_ks);
+                            af[ks][1] = two5 ? f4_lds(zq + kk * z_k4 + ks * z_ks + 64) : 0.0;
+                            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(bf[ks].x), "=d"(bf[ks].y) : "r"(b4_lane + 8u * (unsigned)((kk * 3 + ks) * 64)));
+                        }
+#pragma unroll
+                        for (int ks = 0; ks < 3; ++ks) {
+                            if (ks >= klo && ks < khi) {
+                                fz_dmma(c[0][0][0], c[0][0][1], af[ks][0], bf[ks].x);
+                                if (two4) fz_dmma(c[0][1][0], c[0][1][1], af[ks][0], bf[ks].y);
+                                if (two5) {
+                                    fz_dmma(c[1][0][0], c[1][0][1], af[ks][1], bf[ks].x);
+                                    if (two4) fz_dmma(c[1][1][0], c[1][1][1], af[ks][1], bf[ks].y);
+                                }
+                            }
+                        }
+                        ndm += (unsigned)((khi - klo) * (two4 ? 2 : 1) * (two5 ? 2 : 1));
+                    }
+                    const unsigned dst = qst_lane + 8u * (unsigned)(kk * ldq);
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        const unsigned rowa = dst + 8u * (unsigned)(8 * t * n4);
+                        if (smask & (1u << (4 * t))) f4_sts(rowa, c[t][0][0]);
+                        if (smask & (2u << (4 * t))) f4_sts(rowa + 8u, c[t][0][1]);
+                        if (smask & (4u << (4 * t))) f4_sts(rowa + 64u, c[t][1][0]);
+                        if (smask & (8u << (4 * t))) f4_sts(rowa + 72u, c[t][1][1]);
+                    }
+                }
+                zq += 4 * z_k4;
+                const double s30 = s3n[0], s31 = s3n[1];
+                __syncwarp();                                 // the tile is complete; every lane has read the booster slot
+                if (gi + 1 < ng) {
+                    b4_copy();                                // the next k-step's fragments arrive under this k-step's P phase
+                    s3_fetch();
+                }
+                // ---- P: all column tiles (i5 i4), K = the four k4 of the tile ----
+#pragma unroll
+                for (int jb = 0; jb < 16; jb += 4) {          // four B fragments at a time, requested before their MMAs
+                    if (jb < NT) {
+                        double bv[4];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) bv[j] = f4_lds(qld_lane + 64u * (jb + j));
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            if (jb + j < NT) {
+                                fz_dmma(acc[0][jb + j][0], acc[0][jb + j][1], s30, bv[j]);
+                                if (two3) fz_dmma(acc[1][jb + j][0], acc[1][jb + j][1], s31, bv[j]);
+                            }
+                        }
+                    }
+                }
+                ndm += (unsigned)(NT * (two3 ? 2 : 1));
+                __syncwarp();                                 // the P phase has read the tile
+            }
+            // the rows of P of this unit (zeros when no k4 survives: the readers expect every allowed row)
+            {
+                double* Pb = p.Pq + ((((long)ac * c24 + b24) * c25 + b25) * P3) * V * prow + ((long)b34 * c35 + b35) * NP +
+                             (long)(v0 + xl) * prow + 2 * q;
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const int r3 = 8 * i + g;
+                    if (r3 < n3) {
+                        double* dst = Pb + (long)(q3lo + r3) * V * prow;
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)          // NP is even and the row starts 16-byte aligned
+                            if (pmask & (1u << j)) *reinterpret_cast<double2*>(dst + 8 * j) = make_double2(acc[i][j][0], acc[i][j][1]);
+                    }
+                }
+            }
+        }
+    }
+    if (p.cnt && lane == 0 && ndm) atomicAdd(p.cnt, (unsigned long long)ndm);
+}
+
+static void f4_shape(const SfDims& D, int* ldz, size_t* smem)
+{
+    const int n5 = D.n_i[4], P4 = D.n_k_pad[2];
+    *ldz = (F4_XC - 1) * n5 + 16 <= 52 ? 52 : 68;             // the last x of a chunk reads 16 rows from its first i5; = 4 mod 16
+    *smem = sizeof(double) * ((size_t)P4 * F4_L45 * *ldz + (size_t)F4_WARPS * (4 * F4_LDQ + F4_BSLOT));
+}
+
+/* True when k_fz_qp4 holds the shape of the box (the caller then builds Bw4P, as for k_fz_qp2). */
+bool fz_qp4_supported(const FzParams& p, const SfDims& D)
+{
+    const int n4 = D.n_i[3], n5 = D.n_i[4], P3 = D.n_k_pad[1], P4 = D.n_k_pad[2];
+    if (n5 > 16 || n4 > 16 || n4 * n5 > 128 || p.box.cnt[5] > F4_L45 || P4 > 24 || P4 < 1 || P3 < 1 || P3 > 239) return false;
+    if (p.box.cnt[1] > 255 || p.box.cnt[3] > 255 || p.box.cnt[1] * p.box.cnt[3] * F4_XC > F4_MAXU) return false;
+    // k3 rows of a unit: inside the window of a pair (l34 l35), at most 32 (two units of 16)
+    for (int u = 0; u < p.box.cnt[3]; ++u)
+        for (int v = 0; v < p.box.cnt[4]; ++v) {
+            const int2 w = fz_window(D.two_j[J34] + 2 * (p.box.lo[3] + u), D.two_j[J35] + 2 * (p.box.lo[4] + v), D.two_k_base[1], P3);
+            if (w.y > 32) return false;
+        }
+    int ldz;
+    size_t smem;
+    f4_shape(D, &ldz, &smem);
+    return smem + 18 * 1024 <= 227 * 1024;                    // + the static tables
+}
+
+/* Launches k_fz_qp4 for the pass described by p (fz_qp4_supported must hold; Bw4P built by fz_launch_b4p). */
+int fz_launch_qp4(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st)
+{
+    FzQp4Args a;
+    memset(&a, 0, sizeof a);
+    size_t smem;
+    f4_shape(D, &a.ldz, &smem);
+    a.vc = (p.V + F4_XC - 1) / F4_XC;
+    const long n_items = (long)a.vc * p.a_cnt * p.box.cnt[2] * p.box.cnt[4];
+    if (n_items > 2000000000L) return SF_EARG;
+    a.n_items = (int)n_items;
+    a.sched = sched;
+    a.Bw4P = Bw4P;
+    static size_t attr52 = 0, attr68 = 0;
+    size_t& attr = a.ldz == 52 ? attr52 : attr68;
+    if (smem > attr) {
+        const cudaError_t e = a.ldz == 52 ? cudaFuncSetAttribute(k_fz_qp4<52>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                                          : cudaFuncSetAttribute(k_fz_qp4<68>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return SF_ECUDA;
+        attr = smem;
+    }
+    if (cudaMemsetAsync(sched, 0, sizeof(int), st) != cudaSuccess) return SF_ECUDA;
+    const int grid = (int)(n_items < n_sm ? n_items : n_sm);
+    if (a.ldz == 52)
+        k_fz_qp4<52><<<grid, F4_THREADS, smem, st>>>(p, a);
+    else
+        k_fz_qp4<68><<<grid, F4_THREADS, smem, st>>>(p, a);
+    sf_count_launch(1);
+    return SF_OK;
+}

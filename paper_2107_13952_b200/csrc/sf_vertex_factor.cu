@@ -1031,6 +1031,8 @@ bool fz_qp2_supported(const FzParams& p, const SfDims& D);                      
 long fz_qp2_b4p_elems(const FzParams& p, const SfDims& D);
 void fz_launch_b4p(const FzParams& p, long n, double* out, cudaStream_t st);
 int fz_launch_qp2(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st);
+bool fz_qp4_supported(const FzParams& p, const SfDims& D);                                     // sf_factor_qp4.cu
+int fz_launch_qp4(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st);
 
 enum { FZ_SLOT_SCHED = 22, FZ_SLOT_CNT = 23, FZ_SLOT_WIN = 24, FZ_SLOT_LIST, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART };
 
@@ -1113,7 +1115,8 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         p.hull4B = make_int2(lo < hi ? lo : 0, lo < hi ? hi : 0);
 
         const long nZ = c25 * n1 * c35 * c45 * ((long)P4 * sh.V * n5);
-        const bool qp2 = !(g_fz_variant & 2) && fz_qp2_supported(p, D);      // second-generation Q/P kernel and its booster layout
+        const bool qp4 = !(g_fz_variant & 6) && fz_qp4_supported(p, D);      // warp-autonomous Q/P kernel (one warp per unit)
+        const bool qp2 = qp4 || (!(g_fz_variant & 2) && fz_qp2_supported(p, D));   // second generation; both use the booster layout Bw4P
         const long nB4 = qp2 ? fz_qp2_b4p_elems(p, D) : (long)P4 * c45 * c24 * c34 * n4, nB3 = (long)P3 * c34 * c35 * c23 * n3;
         const long nS3 = c24 * c34 * c35 * D.n_x_pad * P3 * P4;
         const long nG = c24 * c25 * n1 * P3 * sh.V * c23 * n2;
@@ -1128,7 +1131,8 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         }
         if (na > n1) na = n1;
         double* Z = (double*)sf_scratch(FZ_SLOT_Z, sizeof(double) * (size_t)nZ);
-        double* B4 = (double*)sf_scratch(FZ_SLOT_B4, sizeof(double) * (size_t)nB4);
+        const long padB4 = 4L * 12 * 16;             // k_fz_qp4 copies whole k-steps (4 k4) of Bw4P: the last one may end past the array
+        double* B4 = (double*)sf_scratch(FZ_SLOT_B4, sizeof(double) * (size_t)(nB4 + padB4));
         double* B3 = (double*)sf_scratch(FZ_SLOT_B3, sizeof(double) * (size_t)nB3);
         const long padS3 = 24L * P4 + 8;             // k_fz_qp2 reads fragment rows / columns just past a block: keep them finite
         double* S3 = (double*)sf_scratch(FZ_SLOT_S3, sizeof(double) * (size_t)(nS3 + padS3));
@@ -1166,6 +1170,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         if (qp2) {
             fz_launch_b4p(p, nB4, B4, st);
             SF_CUDA_OK(cudaMemsetAsync(S3 + nS3, 0, sizeof(double) * (size_t)padS3, st));
+            SF_CUDA_OK(cudaMemsetAsync(B4 + nB4, 0, sizeof(double) * (size_t)padB4, st));
         } else {
             k_fz_b4t<<<(unsigned)((nB4 + 255) / 256), 256, 0, st>>>(p, nB4, B4);
         }
@@ -1184,7 +1189,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             }
             fz_ev_begin(0, st);
             if (qp2) {
-                const int rcq = fz_launch_qp2(p, D, B4, sched + 1, n_sm, st);
+                const int rcq = qp4 ? fz_launch_qp4(p, D, B4, sched + 1, n_sm, st) : fz_launch_qp2(p, D, B4, sched + 1, n_sm, st);
                 if (rcq != SF_OK) return rcq;
             } else {                                  // shapes the second-generation kernel does not hold
                 const long n_items = (long)p.a_cnt * c25 * c35 * c24 * c34;

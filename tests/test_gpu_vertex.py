@@ -130,6 +130,40 @@ def test_config3_blocks_and_ragged_ranges():
         assert_parity(Ag, Ao, Aabs, what=f"config 3 shells [{lo},{hi})")
 
 
+@pytest.mark.parametrize("bits", [pytest.param(1, id="R-booster-stationary"), pytest.param(2, id="qp-gen1"),
+                                  pytest.param(4, id="qp-gen2"), pytest.param(0, id="default")])
+def test_factorised_kernel_variants_against_the_oracle(bits):
+    """Every kernel variant of the factorised path (sf_set_factor_variant, include/sfoam_debug.h: the fallbacks the
+    default falls back to for shapes its kernels do not hold) against the oracle: config 0 and a half-integer set in
+    full, config 2 (Delta_l = 3) in full, a whole (l23 l24 l25) block and a ragged range of config 3, a config 4 block."""
+    sf.sf_set_path(4)
+    sf.sf_set_factor_variant(bits)
+    try:
+        for cfg, what in [(wl.CONFIGS[0], "config 0"), (wl.config2(3), "config 2 dl 3"),
+                          (dict(two_j=[4, 3, 1, 4, 2, 5, 5, 5, 4, 3], two_dl=4, boosters="random", seed=77), "half-integer")]:
+            B = boosters_for(cfg)
+            Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B)
+            assert sf.sf_last_path() == 4
+            Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B)
+            assert_parity(Ag, Ao, Aabs, what=f"variant {bits}: {what}")
+        cfg = wl.CONFIGS[3]
+        B = boosters_for(cfg)
+        Bdev = to_device(B)
+        nl3 = 11 ** 3
+        for lo, hi in [(nl3 * 613, nl3 * 614), (nl3 * 9 + 1200, nl3 * 10 + 300)]:
+            Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, lo, hi, Bdev=Bdev)
+            Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, lo, hi)
+            assert_parity(Ag, Ao, Aabs, what=f"variant {bits}: config 3 shells [{lo},{hi})")
+        cfg = _config4(2)
+        B = boosters_for(cfg)
+        Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, 7 ** 3 * 100, 7 ** 3 * 101)
+        Ao, Aabs = run_oracle(cfg["two_j"], cfg["two_dl"], B, 7 ** 3 * 100, 7 ** 3 * 101)
+        assert_parity(Ag, Ao, Aabs, what=f"variant {bits}: config 4 lambda 2 block")
+    finally:
+        sf.sf_set_factor_variant(0)
+        sf.sf_set_path(0)
+
+
 def test_paths_agree_on_a_full_tensor():
     """Config 2, Delta_l = 4 (15 625 shells) in full: the factorised and the per-shell line path give the same tensor to
     rounding, and both match the oracle."""
