@@ -41,6 +41,9 @@ struct FzQp4Args {
     const double* Bw4P;           // [b24][b34][q4][k-step 3][lane 32][column tile 2], see k_fz_b4p (sf_factor_qp.cu)
 };
 
+struct FzTrue { static constexpr bool value = true; };
+struct FzFalse { static constexpr bool value = false; };
+
 __device__ __forceinline__ double f4_lds(unsigned addr)
 {
     double v;
@@ -53,14 +56,14 @@ __device__ __forceinline__ void f4_sts(unsigned addr, double a)
 }
 
 // LDZ = row stride of the Z slab: 52 for n5 <= 12, else 68 (= 4 mod 16, >= 3 n5 + 16)
-template <int LDZ>
+// N5T, N4T = tiles of 8 over i5 and over i4 in the Q phase (1 or 2): compile-time, so that the k-step body is straight-line code
+template <int LDZ, int N5T, int N4T>
 __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant__ FzParams p, const __grid_constant__ FzQp4Args a)
 {
     extern __shared__ __align__(16) double smem[];
     __shared__ int s_item, s_next;
     __shared__ int2 s_unit[2 * F4_MAXU];                      // per (b24, b34, x) and its overflow: packed windows, see below
     __shared__ __align__(8) unsigned long long s_bar[F4_WARPS];   // per warp: completion of the bulk copy into its booster slot
-    __shared__ int s_ksr[32];                                 // per q4: k-steps [lo, hi) of the l45 the triad (k4 l45 j14) allows
     const SfProblem& P = p.P;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
     const int nl = P.nl, n1 = P.n_i[0], n4 = P.n_i[3], n5 = P.n_i[4], n54 = n4 * n5;
@@ -68,7 +71,7 @@ __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant_
     const int c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4], c45 = p.box.cnt[5];
     constexpr int ldz = LDZ, ldq = F4_LDQ;
     const int NT = (n54 + 7) >> 3;
-    const bool two4 = n4 > 8, two5 = n5 > 8;                  // a second tile of i4 / of i5 in the Q phase
+    const int KS45 = (c45 + 3) >> 2;                          // k-steps over the l45 of the box
     const int sZ = P4 * V * n5;
     const long prow = (long)c34 * c35 * NP;                   // stride of v in P
     const int nzs = P4 * F4_L45 * ldz;
@@ -76,18 +79,6 @@ __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant_
     if (lane == 0) fz_mbar_init(fz_smem_u32(&s_bar[warp]), 1);
     if (tid == 0) asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the zeroed slots are next written by bulk copies
-    if (tid < 32) {
-        int lo = 3, hi = 0;
-        if (tid < P4)
-            for (int b45 = 0; b45 < c45; ++b45) {
-                const int2 w = p.w4B[p.box.lo[5] + b45];
-                if (tid >= w.x && tid < w.x + w.y) {
-                    lo = min(lo, b45 >> 2);
-                    hi = max(hi, (b45 >> 2) + 1);
-                }
-            }
-        s_ksr[tid] = hi > lo ? (lo | (hi << 8)) : 0;
-    }
     const unsigned zs_u32 = fz_smem_u32(smem);                // Zs[P4][F4_L45][ldz]
     const unsigned qs_u32 = zs_u32 + 8u * (unsigned)(nzs + warp * (4 * ldq + F4_BSLOT));   // this warp's Q tile [4][ldq]
     const unsigned bs_u32 = qs_u32 + 8u * (unsigned)(4 * ldq);                           // and booster slot [4 k4][3 k-steps][32 lanes][2]
@@ -104,11 +95,15 @@ __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant_
 #pragma unroll
         for (int e = 0; e < 4; ++e)
             if (8 * t + g < n5 && 8 * (e >> 1) + 2 * q + (e & 1) < n4) smask |= 1u << (4 * t + e);
-    const unsigned qld_lane = qs_u32 + 8u * (unsigned)(q * ldq + g);                  // B of P: k4 row q, column 8 j + g
-    unsigned pmask = 0;                                       // column pairs 8 j + 2 q of P this lane stores
+    // B of P: one 16-byte load gives this lane's entries of TWO column tiles: k4 row q, columns 16 jp + 2 g (tile 2 jp) and
+    // 16 jp + 2 g + 1 (tile 2 jp + 1); the C fragments of the pair then hold four consecutive columns 16 jp + 4 q .. + 3
+    const unsigned qld_lane = qs_u32 + 8u * (unsigned)(q * ldq + 2 * g);
+    unsigned pmask = 0;                                       // column pairs 16 jp + 4 q (bit 2 jp) and 16 jp + 4 q + 2 (bit 2 jp + 1) this lane stores
 #pragma unroll
-    for (int j = 0; j < 16; ++j)
-        if (8 * j + 2 * q < n54) pmask |= 1u << j;
+    for (int jp = 0; jp < 8; ++jp) {
+        if (16 * jp + 4 * q < n54) pmask |= 1u << (2 * jp);
+        if (16 * jp + 4 * q + 2 < n54) pmask |= 2u << (2 * jp);
+    }
     const unsigned b4_lane = bs_u32 + 16u * (unsigned)lane;   // B of Q: fragment-major, (column tile 0, 1) adjacent
     unsigned ndm = 0;
 
@@ -242,42 +237,42 @@ __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant_
                 // __syncwarp below, after that phase).  k4 beyond the window get a zero row: their booster fragments are not used ----
 #pragma unroll
                 for (int kk = 0; kk < 4; ++kk) {
-                    const int k4 = k4lo + 4 * gi + kk;
-                    const int ksr = k4 < k4hi ? s_ksr[k4] : 0;
-                    const int klo = ksr & 255, khi = ksr >> 8;
                     double c[2][2][2];
 #pragma unroll
                     for (int t = 0; t < 2; ++t) c[t][0][0] = c[t][0][1] = c[t][1][0] = c[t][1][1] = 0.0;
-                    if (khi > klo) {                          // uniform: all three k-steps of l45 (zeros outside [klo, khi))
-                        double af[3][2];
+                    if (k4lo + 4 * gi + kk < k4hi) {          // uniform.  Every k-step of l45: where the triad (k4 l45 j14) fails, Z and
+                        double af[3][N5T];                    // the booster are exactly zero, so nothing is skipped and nothing tested
                         double2 bf[3];
 #pragma unroll
                         for (int ks = 0; ks < 3; ++ks) {
-                            af[ks][0] = f4_lds(zq + kk * z_k4 + ks * z_ks);
-                            af[ks][1] = two5 ? f4_lds(zq + kk * z_k4 + ks * z_ks + 64) : 0.0;
-                            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(bf[ks].x), "=d"(bf[ks].y) : "r"(b4_lane + 8u * (unsigned)((kk * 3 + ks) * 64)));
+                            if (ks < KS45) {
+#pragma unroll
+                                for (int t = 0; t < N5T; ++t) af[ks][t] = f4_lds(zq + kk * z_k4 + ks * z_ks + 64 * t);
+                                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(bf[ks].x), "=d"(bf[ks].y) : "r"(b4_lane + 8u * (unsigned)((kk * 3 + ks) * 64)));
+                            }
                         }
 #pragma unroll
                         for (int ks = 0; ks < 3; ++ks) {
-                            if (ks >= klo && ks < khi) {
-                                fz_dmma(c[0][0][0], c[0][0][1], af[ks][0], bf[ks].x);
-                                if (two4) fz_dmma(c[0][1][0], c[0][1][1], af[ks][0], bf[ks].y);
-                                if (two5) {
-                                    fz_dmma(c[1][0][0], c[1][0][1], af[ks][1], bf[ks].x);
-                                    if (two4) fz_dmma(c[1][1][0], c[1][1][1], af[ks][1], bf[ks].y);
+                            if (ks < KS45) {
+#pragma unroll
+                                for (int t = 0; t < N5T; ++t) {
+                                    fz_dmma(c[t][0][0], c[t][0][1], af[ks][t], bf[ks].x);
+                                    if (N4T > 1) fz_dmma(c[t][1][0], c[t][1][1], af[ks][t], bf[ks].y);
                                 }
                             }
                         }
-                        ndm += (unsigned)((khi - klo) * (two4 ? 2 : 1) * (two5 ? 2 : 1));
+                        ndm += (unsigned)(KS45 * N5T * N4T);
                     }
                     const unsigned dst = qst_lane + 8u * (unsigned)(kk * ldq);
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) {
+                    for (int t = 0; t < N5T; ++t) {
                         const unsigned rowa = dst + 8u * (unsigned)(8 * t * n4);
                         if (smask & (1u << (4 * t))) f4_sts(rowa, c[t][0][0]);
                         if (smask & (2u << (4 * t))) f4_sts(rowa + 8u, c[t][0][1]);
-                        if (smask & (4u << (4 * t))) f4_sts(rowa + 64u, c[t][1][0]);
-                        if (smask & (8u << (4 * t))) f4_sts(rowa + 72u, c[t][1][1]);
+                        if (N4T > 1) {
+                            if (smask & (4u << (4 * t))) f4_sts(rowa + 64u, c[t][1][0]);
+                            if (smask & (8u << (4 * t))) f4_sts(rowa + 72u, c[t][1][1]);
+                        }
                     }
                 }
                 zq += 4 * z_k4;
@@ -288,36 +283,45 @@ __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant_
                     s3_fetch();
                 }
                 // ---- P: all column tiles (i5 i4), K = the four k4 of the tile ----
+                auto p_phase = [&](auto rt2, auto all) {      // rt2: a second row tile of k3; all: every one of the 16 column tiles exists
 #pragma unroll
-                for (int jb = 0; jb < 16; jb += 4) {          // four B fragments at a time, requested before their MMAs
-                    if (jb < NT) {
-                        double bv[4];
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) bv[j] = f4_lds(qld_lane + 64u * (jb + j));
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            if (jb + j < NT) {
-                                fz_dmma(acc[0][jb + j][0], acc[0][jb + j][1], s30, bv[j]);
-                                if (two3) fz_dmma(acc[1][jb + j][0], acc[1][jb + j][1], s31, bv[j]);
+                    for (int jp = 0; jp < 8; ++jp) {
+                        if (decltype(all)::value || 2 * jp < NT) {
+                            double2 bv;
+                            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(bv.x), "=d"(bv.y) : "r"(qld_lane + 128u * jp));
+                            fz_dmma(acc[0][2 * jp][0], acc[0][2 * jp][1], s30, bv.x);
+                            fz_dmma(acc[0][2 * jp + 1][0], acc[0][2 * jp + 1][1], s30, bv.y);
+                            if (decltype(rt2)::value) {
+                                fz_dmma(acc[1][2 * jp][0], acc[1][2 * jp][1], s31, bv.x);
+                                fz_dmma(acc[1][2 * jp + 1][0], acc[1][2 * jp + 1][1], s31, bv.y);
                             }
                         }
                     }
+                };
+                if (NT >= 15) {
+                    if (two3) p_phase(FzTrue(), FzTrue()); else p_phase(FzFalse(), FzTrue());
+                } else {
+                    if (two3) p_phase(FzTrue(), FzFalse()); else p_phase(FzFalse(), FzFalse());
                 }
-                ndm += (unsigned)(NT * (two3 ? 2 : 1));
+                ndm += (unsigned)(((NT + 1) & ~1) * (two3 ? 2 : 1));
                 __syncwarp();                                 // the P phase has read the tile
             }
             // the rows of P of this unit (zeros when no k4 survives: the readers expect every allowed row)
             {
                 double* Pb = p.Pq + ((((long)ac * c24 + b24) * c25 + b25) * P3) * V * prow + ((long)b34 * c35 + b35) * NP +
-                             (long)(v0 + xl) * prow + 2 * q;
+                             (long)(v0 + xl) * prow + 4 * q;
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
                     const int r3 = 8 * i + g;
                     if (r3 < n3) {
                         double* dst = Pb + (long)(q3lo + r3) * V * prow;
 #pragma unroll
-                        for (int j = 0; j < 16; ++j)          // NP is even and the row starts 16-byte aligned
-                            if (pmask & (1u << j)) *reinterpret_cast<double2*>(dst + 8 * j) = make_double2(acc[i][j][0], acc[i][j][1]);
+                        for (int jp = 0; jp < 8; ++jp) {      // NP is even and the row starts 16-byte aligned
+                            if (pmask & (1u << (2 * jp)))
+                                *reinterpret_cast<double2*>(dst + 16 * jp) = make_double2(acc[i][2 * jp][0], acc[i][2 * jp + 1][0]);
+                            if (pmask & (2u << (2 * jp)))
+                                *reinterpret_cast<double2*>(dst + 16 * jp + 2) = make_double2(acc[i][2 * jp][1], acc[i][2 * jp + 1][1]);
+                        }
                     }
                 }
             }
@@ -364,20 +368,14 @@ int fz_launch_qp4(const FzParams& p, const SfDims& D, const double* Bw4P, int* s
     a.n_items = (int)n_items;
     a.sched = sched;
     a.Bw4P = Bw4P;
-    static size_t attr52 = 0, attr68 = 0;
-    size_t& attr = a.ldz == 52 ? attr52 : attr68;
-    if (smem > attr) {
-        const cudaError_t e = a.ldz == 52 ? cudaFuncSetAttribute(k_fz_qp4<52>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
-                                          : cudaFuncSetAttribute(k_fz_qp4<68>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return SF_ECUDA;
-        attr = smem;
-    }
+    const int n5t = D.n_i[4] > 8 ? 2 : 1, n4t = D.n_i[3] > 8 ? 2 : 1;
+    void (*kern)(const FzParams, const FzQp4Args) =
+        a.ldz == 68 ? (n4t == 2 ? k_fz_qp4<68, 2, 2> : k_fz_qp4<68, 2, 1>)
+                    : n5t == 2 ? (n4t == 2 ? k_fz_qp4<52, 2, 2> : k_fz_qp4<52, 2, 1>) : (n4t == 2 ? k_fz_qp4<52, 1, 2> : k_fz_qp4<52, 1, 1>);
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SF_ECUDA;
     if (cudaMemsetAsync(sched, 0, sizeof(int), st) != cudaSuccess) return SF_ECUDA;
     const int grid = (int)(n_items < n_sm ? n_items : n_sm);
-    if (a.ldz == 52)
-        k_fz_qp4<52><<<grid, F4_THREADS, smem, st>>>(p, a);
-    else
-        k_fz_qp4<68><<<grid, F4_THREADS, smem, st>>>(p, a);
+    kern<<<grid, F4_THREADS, smem, st>>>(p, a);
     sf_count_launch(1);
     return SF_OK;
 }
