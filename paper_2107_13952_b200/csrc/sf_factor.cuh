@@ -89,6 +89,14 @@ __device__ __forceinline__ void fz_dmma(double& c0, double& c1, double a, double
         : "d"(a), "d"(b));
 }
 
+// the first MMA of a sum: C = A B (no accumulator to clear)
+__device__ __forceinline__ void fz_dmma0(double& c0, double& c1, double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%4,%4};\n"
+        : "=d"(c0), "=d"(c1)
+        : "d"(a), "d"(b), "d"(0.0));
+}
+
 __device__ __forceinline__ unsigned fz_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void fz_cp_async8(unsigned dst, const void* src, int bytes)
 {

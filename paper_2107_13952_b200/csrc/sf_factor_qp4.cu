@@ -71,7 +71,6 @@ __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant_
     const int c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4], c45 = p.box.cnt[5];
     constexpr int ldz = LDZ, ldq = F4_LDQ;
     const int NT = (n54 + 7) >> 3;
-    const int KS45 = (c45 + 3) >> 2;                          // k-steps over the l45 of the box
     const int sZ = P4 * V * n5;
     const long prow = (long)c34 * c35 * NP;                   // stride of v in P
     const int nzs = P4 * F4_L45 * ldz;
@@ -231,37 +230,41 @@ __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant_
                 s3_fetch();
             }
             for (int gi = 0; gi < ng; ++gi) {
+                const double s30 = s3n[0], s31 = s3n[1];      // requested a whole k-step ago
+                if (gi + 1 < ng) s3_fetch();                  // S3 of the next k-step: a Q phase, a P phase and a Q phase to arrive
                 fz_mbar_wait(bar_u32, bphase);                // the booster fragments of this k-step have landed
                 bphase ^= 1u;
                 // ---- Q of the four k4 of this k-step into the warp's tile (the P phase of the previous k-step has read it: the
                 // __syncwarp below, after that phase).  k4 beyond the window get a zero row: their booster fragments are not used ----
 #pragma unroll
                 for (int kk = 0; kk < 4; ++kk) {
-                    double c[2][2][2];
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) c[t][0][0] = c[t][0][1] = c[t][1][0] = c[t][1][1] = 0.0;
-                    if (k4lo + 4 * gi + kk < k4hi) {          // uniform.  Every k-step of l45: where the triad (k4 l45 j14) fails, Z and
-                        double af[3][N5T];                    // the booster are exactly zero, so nothing is skipped and nothing tested
+                    double c[N5T][2][2];
+                    if (k4lo + 4 * gi + kk < k4hi) {          // uniform.  All three k-steps of l45: where the triad (k4 l45 j14) fails or the
+                        double af[3][N5T];                    // box has no l45, Z and the booster are exactly zero: nothing skipped, nothing tested
                         double2 bf[3];
 #pragma unroll
                         for (int ks = 0; ks < 3; ++ks) {
-                            if (ks < KS45) {
 #pragma unroll
-                                for (int t = 0; t < N5T; ++t) af[ks][t] = f4_lds(zq + kk * z_k4 + ks * z_ks + 64 * t);
-                                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(bf[ks].x), "=d"(bf[ks].y) : "r"(b4_lane + 8u * (unsigned)((kk * 3 + ks) * 64)));
-                            }
+                            for (int t = 0; t < N5T; ++t) af[ks][t] = f4_lds(zq + kk * z_k4 + ks * z_ks + 64 * t);
+                            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(bf[ks].x), "=d"(bf[ks].y) : "r"(b4_lane + 8u * (unsigned)((kk * 3 + ks) * 64)));
                         }
 #pragma unroll
-                        for (int ks = 0; ks < 3; ++ks) {
-                            if (ks < KS45) {
+                        for (int t = 0; t < N5T; ++t) {
+                            fz_dmma0(c[t][0][0], c[t][0][1], af[0][t], bf[0].x);
+                            if (N4T > 1) fz_dmma0(c[t][1][0], c[t][1][1], af[0][t], bf[0].y);
+                        }
 #pragma unroll
-                                for (int t = 0; t < N5T; ++t) {
-                                    fz_dmma(c[t][0][0], c[t][0][1], af[ks][t], bf[ks].x);
-                                    if (N4T > 1) fz_dmma(c[t][1][0], c[t][1][1], af[ks][t], bf[ks].y);
-                                }
+                        for (int ks = 1; ks < 3; ++ks) {
+#pragma unroll
+                            for (int t = 0; t < N5T; ++t) {
+                                fz_dmma(c[t][0][0], c[t][0][1], af[ks][t], bf[ks].x);
+                                if (N4T > 1) fz_dmma(c[t][1][0], c[t][1][1], af[ks][t], bf[ks].y);
                             }
                         }
-                        ndm += (unsigned)(KS45 * N5T * N4T);
+                        ndm += (unsigned)(3 * N5T * N4T);
+                    } else {
+#pragma unroll
+                        for (int t = 0; t < N5T; ++t) c[t][0][0] = c[t][0][1] = c[t][1][0] = c[t][1][1] = 0.0;
                     }
                     const unsigned dst = qst_lane + 8u * (unsigned)(kk * ldq);
 #pragma unroll
@@ -276,12 +279,8 @@ __global__ void __launch_bounds__(F4_THREADS, 1) k_fz_qp4(const __grid_constant_
                     }
                 }
                 zq += 4 * z_k4;
-                const double s30 = s3n[0], s31 = s3n[1];
                 __syncwarp();                                 // the tile is complete; every lane has read the booster slot
-                if (gi + 1 < ng) {
-                    b4_copy();                                // the next k-step's fragments arrive under this k-step's P phase
-                    s3_fetch();
-                }
+                if (gi + 1 < ng) b4_copy();                   // the next k-step's fragments arrive under this k-step's P phase
                 // ---- P: all column tiles (i5 i4), K = the four k4 of the tile ----
                 auto p_phase = [&](auto rt2, auto all) {      // rt2: a second row tile of k3; all: every one of the 16 column tiles exists
 #pragma unroll
