@@ -395,6 +395,8 @@ def run_ours(args, cfg, rank, world, local_rank):
 
     sf.sf_init(wl.GAMMA)
     sf.sf_set_path(args.path)
+    if args.variant:
+        sf.sf_set_factor_variant(args.variant)       # A/B timing of the factorised kernels (include/sfoam_debug.h)
     # one-off {6j} table (kernel (a)), outside the timed region, timed on its own
     t0 = time.perf_counter()
     sf.sf_sixj_table(args.table)
@@ -646,6 +648,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary rows (other workloads, contractions, per-shell path)")
     ap.add_argument("--one-step-only", action="store_true", help="profiling aid: table build + one vertex call, then exit")
+    ap.add_argument("--variant", type=int, default=0, help="kernel variants of the factorised path (sf_set_factor_variant); 0 = default")
     ap.add_argument("--path", type=int, default=0, help="0 automatic (fastest that fits), 1 staged, 3 line, 4 factorised")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

@@ -12,7 +12,7 @@
 //     gathered once per chunk by the consumer warps (8-byte cp.async);
 //   * one PRODUCER warp walks the chunk's products (one per x the triad (k3 l24 x) allows) and fills a ring of stages with
 //     16 rows of P each: one cp.async.bulk (SASS UBLKCP) per row, completion on the stage's `full` mbarrier;
-//   * eight CONSUMER warps (4 x 2, warp tile 32 rows (i5 i4) x up to 64 columns (l23 i3)) wait on `full`, run the FP64
+//   * sixteen CONSUMER warps (4 x 4, warp tile 32 rows (i5 i4) x up to 32 columns (l23 i3)) wait on `full`, run the FP64
 //     tensor-core MMAs (mma.sync m8n8k4 f64 = DMMA.8x8x4) from shared memory with conflict-free fragment loads (row strides
 //     = 4 mod 16 doubles), and release the stage through its `empty` mbarrier: no CTA-wide barrier inside a chunk.
 //
@@ -21,7 +21,7 @@
 #include "sf_factor.cuh"
 
 #define FZR_KC 16                 // rows of P per stage
-#define FZR_NWC 8                 // consumer warps
+#define FZR_NWC 16                // consumer warps: 4 x 4, warp tile 32 rows (i5 i4) x up to 32 columns (l23 i3)
 #define FZR_THREADS (32 * (FZR_NWC + 1))
 #define FZR_BM 128
 #define FZR_BN 128
@@ -46,7 +46,7 @@ __device__ __forceinline__ void fzr_mbar_arrive(unsigned bar)
 
 // the MMAs of one stage for a warp with TNA live column tiles
 template <int TNA>
-__device__ __forceinline__ void fzr_stage(double (&acc)[4][8][2], const double* as, const double* bs, int ldb, int ksn, int tma)
+__device__ __forceinline__ void fzr_stage(double (&acc)[4][4][2], const double* as, const double* bs, int ldb, int ksn, int tma)
 {
 #pragma unroll
     for (int ks = 0; ks < FZR_KC / 4; ++ks) {
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(FZR_THREADS, 1) k_fz_r2(const __grid_constant_
     int it = 0;                                               // stages used so far: slot it % ns, phase (it / ns) & 1
     int have_q3 = -1, have_nt = -1;
     unsigned ndm = 0;
-    const int wm = (warp >> 1) & 3, wn = warp & 1;
+    const int wm = (warp >> 2) & 3, wn = warp & 3;
 
     for (;;) {
         __syncthreads();                                      // everybody is done with the previous chunk (and with Bs)
@@ -163,16 +163,17 @@ __global__ void __launch_bounds__(FZR_THREADS, 1) k_fz_r2(const __grid_constant_
         } else {
             // ---------------- consumers ----------------
             const int NT = (N + 7) >> 3;
-            const int nt0 = wn ? (NT + 1) >> 1 : 0, tna = wn ? NT >> 1 : (NT + 1) >> 1;
+            const int ntb = NT >> 2, ntr = NT & 3;            // column tiles over the four warp columns
+            const int nt0 = wn * ntb + min(wn, ntr), tna = ntb + (wn < ntr ? 1 : 0);
             int tma = 0;
 #pragma unroll
             for (int i = 0; i < 4; ++i) tma += (wm * 32 + 8 * i) < M;
             const bool active = tma > 0 && tna > 0;
-            double acc[4][8][2];
+            double acc[4][4][2];
 #pragma unroll
             for (int i = 0; i < 4; ++i)
 #pragma unroll
-                for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+                for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
             const double* as0 = As + q * FZR_LDA + wm * 32 + g;
             const double* bs0 = Bs + q * ldb + nt0 * 8 + g;
             for (int slab = s_lo; slab < s_hi; ++slab) {
@@ -189,10 +190,6 @@ __global__ void __launch_bounds__(FZR_THREADS, 1) k_fz_r2(const __grid_constant_
                             const double* as = as0 + s * FZR_KC * FZR_LDA;
                             const double* bs = bs0 + (long)c * FZR_KC * ldb;
                             switch (tna) {
-                                case 8: fzr_stage<8>(acc, as, bs, ldb, ksn, tma); break;
-                                case 7: fzr_stage<7>(acc, as, bs, ldb, ksn, tma); break;
-                                case 6: fzr_stage<6>(acc, as, bs, ldb, ksn, tma); break;
-                                case 5: fzr_stage<5>(acc, as, bs, ldb, ksn, tma); break;
                                 case 4: fzr_stage<4>(acc, as, bs, ldb, ksn, tma); break;
                                 case 3: fzr_stage<3>(acc, as, bs, ldb, ksn, tma); break;
                                 case 2: fzr_stage<2>(acc, as, bs, ldb, ksn, tma); break;
@@ -210,7 +207,7 @@ __global__ void __launch_bounds__(FZR_THREADS, 1) k_fz_r2(const __grid_constant_
                         for (int i = 0; i < 4; ++i) {
                             const int m = wm * 32 + 8 * i + g;
 #pragma unroll
-                            for (int j = 0; j < 8; ++j) {
+                            for (int j = 0; j < 4; ++j) {
                                 const int n = (nt0 + j) * 8 + 2 * q;
                                 if (i < tma && j < tna && m < M) {
                                     if (n < N) C[(long)n * NP + m] = acc[i][j][0];

@@ -537,7 +537,7 @@ struct FzMapR {
 struct FzMapA {
     static constexpr bool A16 = false, ABULK = false;
     static constexpr bool B16 = true;    // columns run over the padded rows of R (i3, NP): contiguous and 16-byte aligned pairs
-    static constexpr int CNT = 2, KC = 16, ST = 3;
+    static constexpr int CNT = 2, KC = 16, ST = 2;
     static __device__ const double* srcA(const FzParams& p) { return p.G; }
     static __device__ const double* srcB(const FzParams& p) { return p.Rq; }
     static __device__ double* dstC(const FzParams& p) { return p.Apart; }
