@@ -170,6 +170,11 @@ def sf_set_path(path):
     _check(_lib().sf_set_path(int(path)), "sf_set_path")
 
 
+def sf_set_graphs(on):
+    """Recorded launch sequences for repeated identical calls (include/sfoam.h): 1 on (default), 0 off."""
+    _check(_lib().sf_set_graphs(int(bool(on))), "sf_set_graphs")
+
+
 def sf_last_path():
     return int(_lib().sf_last_path())
 

@@ -23,8 +23,14 @@ struct SfContext {
     bool poison = false;
     cudaEvent_t ev[4] = {};
     double stage_ms[3] = {};
+    long gen = 0;          // bumped by everything a recorded launch sequence depends on (scratch blocks, settings, the {6j} table)
+    bool capturing = false;
+    bool graphs = true;    // sf_set_graphs
+    cudaStream_t cap_stream = nullptr;
 };
 static SfContext g_ctx;
+
+void sf_bump_generation(void) { ++g_ctx.gen; }
 
 void sf_count_launch(int n) { g_ctx.launches += n; }
 
@@ -33,6 +39,8 @@ void* sf_scratch(int slot, size_t bytes)
     if (slot < 0 || slot >= SF_NSCRATCH) return nullptr;
     if (bytes == 0) bytes = 8;
     if (g_ctx.scratch_bytes[slot] >= bytes) return g_ctx.scratch[slot];
+    if (g_ctx.capturing) return nullptr;   // a launch sequence being recorded must not allocate: the caller falls back to a plain run
+    ++g_ctx.gen;                           // recorded launch sequences hold the old pointers
     if (g_ctx.scratch[slot]) {
         cudaDeviceSynchronize();   // the old block may still be in use on a stream
         cudaFree(g_ctx.scratch[slot]);
@@ -73,11 +81,14 @@ extern "C" int sf_init(double gamma)
     if (rc != SF_OK) return rc;
     for (int q = 0; q < 4; ++q)
         if (cudaEventCreate(&g_ctx.ev[q]) != cudaSuccess) return SF_ECUDA;
+    if (cudaStreamCreateWithFlags(&g_ctx.cap_stream, cudaStreamNonBlocking) != cudaSuccess) return SF_ECUDA;
     g_ctx.gamma = gamma;
     g_ctx.init = true;
     g_ctx.launches = 0;
     return SF_OK;
 }
+
+static void sf_graph_cache_clear(void);
 
 extern "C" int sf_finalize(void)
 {
@@ -88,8 +99,11 @@ extern "C" int sf_finalize(void)
         g_ctx.scratch[s] = nullptr;
         g_ctx.scratch_bytes[s] = 0;
     }
+    sf_graph_cache_clear();
     sf_sixj_module_free();
     for (int q = 0; q < 4; ++q) cudaEventDestroy(g_ctx.ev[q]);
+    if (g_ctx.cap_stream) cudaStreamDestroy(g_ctx.cap_stream);
+    g_ctx.cap_stream = nullptr;
     g_ctx.init = false;
     return SF_OK;
 }
@@ -113,6 +127,7 @@ extern "C" const char* sf_strerror(int status)
 extern "C" int sf_sixj_table(int two_jmax)
 {
     if (!g_ctx.init) return SF_ENOTINIT;
+    ++g_ctx.gen;
     return sf_sixj_table_build(two_jmax, 0);
 }
 
@@ -126,16 +141,19 @@ extern "C" long sf_launch_count(int reset)
 extern "C" int sf_set_timing(int on)
 {
     g_ctx.timing = on != 0;
+    ++g_ctx.gen;
     return SF_OK;
 }
 extern "C" int sf_set_counting(int on)
 {
     g_ctx.counting = on != 0;
+    ++g_ctx.gen;
     return SF_OK;
 }
 extern "C" int sf_set_debug_poison(int on)
 {
     g_ctx.poison = on != 0;
+    ++g_ctx.gen;
     return SF_OK;
 }
 extern "C" int sf_last_stage_ms(double ms[3])
@@ -149,39 +167,15 @@ extern "C" int sf_set_path(int path)
 {
     if (path < 0 || path > 4 || path == 2) return SF_EARG;
     g_ctx.path = path;
+    ++g_ctx.gen;
     return SF_OK;
 }
 extern "C" int sf_last_path(void) { return g_ctx.last_path; }
 
-// ranges of the virtual intertwiners k_a for every booster triple (step 2): the node's recoupling
-// pairs with the edge's three virtual spins at l = j + offset (superscript order of PAPER.md:171)
-__global__ void k_kranges(SfProblem P, int nt, SfKRange* __restrict__ out)
-{
-    const int q = blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= 4 * nt) return;
-    const int e = q / nt, t = q % nt, nl = P.nl;
-    const int u = 2 * (t / (nl * nl)), v = 2 * ((t / nl) % nl), w = 2 * (t % nl);
-    const int* j = P.two_j;
-    int a, b, c, d;
-    if (e == 0) {          // node 2 (l23 l24 | l25 j12), triple (l23 l24 l25)
-        a = j[J23] + u; b = j[J24] + v; c = j[J25] + w; d = j[J12];
-    } else if (e == 1) {   // node 3 (l34 l35 | j13 l23), triple (l34 l35 l23)
-        a = j[J34] + u; b = j[J35] + v; c = j[J13]; d = j[J23] + w;
-    } else if (e == 2) {   // node 4 (l45 j14 | l24 l34), triple (l45 l24 l34)
-        a = j[J45] + u; b = j[J14]; c = j[J24] + v; d = j[J34] + w;
-    } else {               // node 5 (j15 l25 | l35 l45), triple (l25 l35 l45)
-        a = j[J15]; b = j[J25] + u; c = j[J35] + v; d = j[J45] + w;
-    }
-    const int lo = max(abs(a - b), abs(c - d)), hi = min(a + b, c + d);
-    SfKRange r;
-    r.two_k_min = lo;
-    r.n_k = (((a + b) ^ (c + d)) & 1) || hi < lo ? 0 : (hi - lo) / 2 + 1;
-    out[q] = r;
-}
-
 // steps 1-2 on the device side: the problem descriptor and the per-triple k-range tables (no host->device copy)
+// (launch_kr: fill the k-range tables now; otherwise sf_build_slices does it in its own launch)
 static int setup_problem(const SfDims& D, const sf_boosters* boosters, SfProblem& P, cudaStream_t st,
-                         const int* b_rows = nullptr, const int* b_first = nullptr)
+                         const int* b_rows = nullptr, const int* b_first = nullptr, bool launch_kr = true)
 {
     memset(&P, 0, sizeof P);
     memcpy(P.two_j, D.two_j, sizeof P.two_j);
@@ -202,13 +196,12 @@ static int setup_problem(const SfDims& D, const sf_boosters* boosters, SfProblem
     SfKRange* d = (SfKRange*)sf_scratch(SLOT_KR, sizeof(SfKRange) * nt * 4);
     if (!d) return SF_ENOMEM;
     for (int e = 0; e < 4; ++e) P.kr[e] = d + (long)e * nt;
-    k_kranges<<<(4 * nt + 127) / 128, 128, 0, st>>>(P, nt, d);
-    sf_count_launch(1);
+    if (launch_kr) sf_launch_kranges(D, d, st);
     return SF_OK;
 }
 
-static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo, long shell_hi,
-                        double* out, cudaStream_t st, bool full, const int* i_first = nullptr, const int* i_count = nullptr)
+static int vertex_range_run(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo, long shell_hi,
+                            double* out, cudaStream_t st, bool full, const int* i_first, const int* i_count)
 {
     if (!g_ctx.init) return SF_ENOTINIT;
     if (!two_j || !boosters || !out) return SF_EARG;
@@ -251,7 +244,7 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
     }
 
     SfProblem P;
-    rc = setup_problem(D, boosters, P, st, b_rows, b_first);
+    rc = setup_problem(D, boosters, P, st, b_rows, b_first, false);
     if (rc != SF_OK) return rc;
 
     // step 4: the five S arrays
@@ -264,7 +257,7 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
         P.S[w] = S[w];
     }
     sf_timing_mark(0, st);
-    rc = sf_build_slices(D, S, sf_sixj_table_get(), st);
+    rc = sf_build_slices(D, S, sf_sixj_table_get(), const_cast<SfKRange*>(P.kr[0]), st);
     if (rc != SF_OK) return rc;
     sf_timing_mark(1, st);
 
@@ -294,6 +287,132 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
         g_ctx.stage_ms[2] = c;
     }
     return SF_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Recorded launch sequences.  A vertex call is 15-30 small launches (k-range tables, S arrays, the precomputations and the
+// contractions of the factorised path); on small problems their launch latency is the whole cost (config 0: 0.1 ms for
+// 3.4e6 flop).  The second time a call comes with the same arguments (spins, Delta_l, ranges, booster and output POINTERS:
+// the booster values are read when the kernels run, so they may change) and the same library state, its launches are
+// recorded into a CUDA graph on a private stream; from then on the call is one graph launch on the caller's stream.
+// Anything a recording depends on (a scratch block reallocated, a setting changed, the {6j} table rebuilt) bumps the
+// generation and drops the recordings.  Measurement modes (timing, counting, poison) never use them.
+// ---------------------------------------------------------------------------------------------------------------
+struct SfGraphKey {
+    int two_j[10], two_dl, full, has_i, i_first[5], i_count[5];
+    long shell_lo, shell_hi;
+    const void* ptr[5];
+    long gen;
+};
+struct SfGraphEntry {
+    bool used = false, no_record = false;
+    SfGraphKey key;
+    cudaGraphExec_t exec = nullptr;
+    long launches = 0;
+    int last_path = 0;
+};
+#define SF_NGRAPH 16
+static SfGraphEntry g_graphs[SF_NGRAPH];
+static int g_graph_next = 0;
+
+static void sf_graph_cache_clear(void)
+{
+    for (int e = 0; e < SF_NGRAPH; ++e) {
+        if (g_graphs[e].exec) cudaGraphExecDestroy(g_graphs[e].exec);
+        g_graphs[e] = SfGraphEntry();
+    }
+}
+
+/* 1 (default): repeated identical vertex calls replay a recorded launch sequence; 0: every call launches its kernels one by one. */
+extern "C" int sf_set_graphs(int on)
+{
+    g_ctx.graphs = on != 0;
+    ++g_ctx.gen;
+    return SF_OK;
+}
+
+static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo, long shell_hi,
+                        double* out, cudaStream_t st, bool full, const int* i_first = nullptr, const int* i_count = nullptr)
+{
+    if (!g_ctx.init) return SF_ENOTINIT;
+    if (!two_j || !boosters || !out) return SF_EARG;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (!g_ctx.graphs || g_ctx.timing || g_ctx.counting || g_ctx.poison || (i_first && !i_count) ||
+        cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        return vertex_range_run(two_j, two_dl, boosters, shell_lo, shell_hi, out, st, full, i_first, i_count);
+    }
+    SfGraphKey k;
+    memset(&k, 0, sizeof k);
+    memcpy(k.two_j, two_j, sizeof k.two_j);
+    k.two_dl = two_dl;
+    k.full = full;
+    k.shell_lo = full ? 0 : shell_lo;
+    k.shell_hi = full ? 0 : shell_hi;
+    if (i_first && i_count) {
+        k.has_i = 1;
+        memcpy(k.i_first, i_first, sizeof k.i_first);
+        memcpy(k.i_count, i_count, sizeof k.i_count);
+    }
+    for (int e = 0; e < 4; ++e) k.ptr[e] = boosters->B[e];
+    k.ptr[4] = out;
+    k.gen = g_ctx.gen;
+    SfGraphEntry* hit = nullptr;
+    for (int e = 0; e < SF_NGRAPH; ++e) {
+        SfGraphEntry& g = g_graphs[e];
+        if (!g.used) continue;
+        if (g.key.gen != g_ctx.gen) {                         // stale: the library state has changed since
+            if (g.exec) cudaGraphExecDestroy(g.exec);
+            g = SfGraphEntry();
+            continue;
+        }
+        if (!memcmp(&g.key, &k, sizeof k)) hit = &g;
+    }
+    if (hit && hit->exec) {
+        if (cudaGraphLaunch(hit->exec, st) != cudaSuccess) return SF_ECUDA;
+        g_ctx.launches += hit->launches;
+        g_ctx.last_path = hit->last_path;
+        return SF_OK;
+    }
+    if (!hit) {                                               // first sight: run it, remember the arguments
+        const long gen0 = g_ctx.gen;
+        const int rc = vertex_range_run(two_j, two_dl, boosters, shell_lo, shell_hi, out, st, full, i_first, i_count);
+        if (rc == SF_OK && gen0 == g_ctx.gen) {               // (a call that had to allocate is remembered at its next repetition)
+            SfGraphEntry& g = g_graphs[g_graph_next];
+            g_graph_next = (g_graph_next + 1) % SF_NGRAPH;
+            if (g.exec) cudaGraphExecDestroy(g.exec);
+            g = SfGraphEntry();
+            g.used = true;
+            g.key = k;
+        }
+        return rc;
+    }
+    if (hit->no_record) return vertex_range_run(two_j, two_dl, boosters, shell_lo, shell_hi, out, st, full, i_first, i_count);
+    // second sight: record the launches on the private stream, then replay them on the caller's
+    const long before = g_ctx.launches;
+    cudaGraph_t graph = nullptr;
+    int rc = SF_ECUDA;
+    if (cudaStreamBeginCapture(g_ctx.cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        g_ctx.capturing = true;
+        rc = vertex_range_run(two_j, two_dl, boosters, shell_lo, shell_hi, out, g_ctx.cap_stream, full, i_first, i_count);
+        g_ctx.capturing = false;
+        if (cudaStreamEndCapture(g_ctx.cap_stream, &graph) != cudaSuccess) rc = SF_ECUDA;
+    }
+    const long recorded = g_ctx.launches - before;
+    g_ctx.launches = before;
+    if (rc == SF_OK && graph && cudaGraphInstantiate(&hit->exec, graph, 0) == cudaSuccess) {
+        cudaGraphDestroy(graph);
+        hit->launches = recorded;
+        hit->last_path = g_ctx.last_path;
+        if (cudaGraphLaunch(hit->exec, st) != cudaSuccess) return SF_ECUDA;
+        g_ctx.launches += recorded;
+        return SF_OK;
+    }
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    hit->exec = nullptr;
+    hit->no_record = true;                                    // this call cannot be recorded (it would allocate, or failed): plain runs
+    return vertex_range_run(two_j, two_dl, boosters, shell_lo, shell_hi, out, st, full, i_first, i_count);
 }
 
 extern "C" int sf_vertex_amplitude(const int two_j[10], int two_dl, const sf_boosters* boosters, double* out,

@@ -82,6 +82,34 @@ __host__ __device__ inline int2 fz_vrange(int two_l, int two_k, int x0, int nxs)
     return r;
 }
 
+// the booster operand of the Q phase in fragment order (k_fz_qp2, k_fz_qp4), 12 rows l45 per k4:
+// Bw4P[b24][b34][q4][ks][lane][j] = (2k4+1) B4[(o45 o24 o34)][i4][q4], l45 = 4 ks + lane % 4, i4 = 8 j + lane / 4, inside the triple's
+// k-range, 0 elsewhere: one 16-byte load per lane and k-step, 512 contiguous bytes per warp
+__device__ __forceinline__ void fz_b4p_entry(const FzParams& p, long n, double* __restrict__ out, long e)
+{
+    const SfProblem& P = p.P;
+    if (e >= n) return;
+    const int nl = P.nl, n4 = P.n_i[3], P4 = P.n_k_pad[2];
+    const int c34 = p.box.cnt[3], c45 = p.box.cnt[5];
+    long r = e;
+    const int jj = (int)(r % 2); r /= 2;
+    const int ln = (int)(r % 32); r /= 32;
+    const int ks = (int)(r % 3); r /= 3;
+    const int i4 = 8 * jj + (ln >> 2), b45 = 4 * ks + (ln & 3);
+    const int q4 = (int)(r % P4); r /= P4;
+    const int b34 = (int)(r % c34);
+    const int b24 = (int)(r / c34);
+    double val = 0.0;
+    if (i4 < n4 && b45 < c45) {
+        const int t4 = ((p.box.lo[5] + b45) * nl + p.box.lo[1] + b24) * nl + p.box.lo[3] + b34;
+        const SfKRange r4 = P.kr[2][t4];
+        const int c = q4 - ((r4.two_k_min - P.two_k_base[2]) >> 1);
+        if (c >= 0 && c < r4.n_k) val = (double)(r4.two_k_min + 2 * c + 1) * sf_brow(P, 2, t4, i4)[q4];
+    }
+    out[e] = val;
+}
+
+
 __device__ __forceinline__ void fz_dmma(double& c0, double& c1, double a, double b)
 {
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};\n"

@@ -58,33 +58,6 @@ __device__ __forceinline__ void fq_sts2(unsigned addr, double a, double b)
     asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(a), "d"(b) : "memory");
 }
 
-// Bw4P[b24][b34][q4][ks][lane][j] = (2k4+1) B4[(o45 o24 o34)][i4][q4], l45 = 4 ks + lane % 4, i4 = 8 j + lane / 4, inside the triple's
-// k-range, 0 elsewhere: one 16-byte load per lane and k-step, 512 contiguous bytes per warp
-__global__ void __launch_bounds__(256) k_fz_b4p(FzParams p, long n, double* __restrict__ out)
-{
-    const SfProblem& P = p.P;
-    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    if (e >= n) return;
-    const int nl = P.nl, n4 = P.n_i[3], P4 = P.n_k_pad[2];
-    const int c34 = p.box.cnt[3], c45 = p.box.cnt[5];
-    long r = e;
-    const int jj = (int)(r % 2); r /= 2;
-    const int ln = (int)(r % 32); r /= 32;
-    const int ks = (int)(r % 3); r /= 3;
-    const int i4 = 8 * jj + (ln >> 2), b45 = 4 * ks + (ln & 3);
-    const int q4 = (int)(r % P4); r /= P4;
-    const int b34 = (int)(r % c34);
-    const int b24 = (int)(r / c34);
-    double val = 0.0;
-    if (i4 < n4 && b45 < c45) {
-        const int t4 = ((p.box.lo[5] + b45) * nl + p.box.lo[1] + b24) * nl + p.box.lo[3] + b34;
-        const SfKRange r4 = P.kr[2][t4];
-        const int c = q4 - ((r4.two_k_min - P.two_k_base[2]) >> 1);
-        if (c >= 0 && c < r4.n_k) val = (double)(r4.two_k_min + 2 * c + 1) * sf_brow(P, 2, t4, i4)[q4];
-    }
-    out[e] = val;
-}
-
 __global__ void __launch_bounds__(FQ_THREADS, 1) k_fz_qp2(const __grid_constant__ FzParams p, const __grid_constant__ FzQp2Args a)
 {
     extern __shared__ __align__(16) double smem[];
@@ -333,11 +306,6 @@ long fz_qp2_b4p_elems(const FzParams& p, const SfDims& D)
     return (long)p.box.cnt[1] * p.box.cnt[3] * D.n_k_pad[2] * FQ_L45 * 16;
 }
 
-void fz_launch_b4p(const FzParams& p, long n, double* out, cudaStream_t st)
-{
-    k_fz_b4p<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p, n, out);
-}
-
 /* Launches k_fz_qp2 for the pass described by p (fz_qp2_supported must hold; Bw4P built by fz_launch_b4p). */
 int fz_launch_qp2(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st)
 {
@@ -359,7 +327,6 @@ int fz_launch_qp2(const FzParams& p, const SfDims& D, const double* Bw4P, int* s
         if (cudaFuncSetAttribute(k_fz_qp2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SF_ECUDA;
         attr = smem;
     }
-    if (cudaMemsetAsync(sched, 0, sizeof(int), st) != cudaSuccess) return SF_ECUDA;
     const int grid = (int)(n_items < n_sm ? n_items : n_sm);
     k_fz_qp2<<<grid, FQ_THREADS, smem, st>>>(p, a);
     sf_count_launch(1);

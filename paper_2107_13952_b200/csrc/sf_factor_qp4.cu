@@ -372,7 +372,6 @@ int fz_launch_qp4(const FzParams& p, const SfDims& D, const double* Bw4P, int* s
         a.ldz == 68 ? (n4t == 2 ? k_fz_qp4<68, 2, 2> : k_fz_qp4<68, 2, 1>)
                     : n5t == 2 ? (n4t == 2 ? k_fz_qp4<52, 2, 2> : k_fz_qp4<52, 2, 1>) : (n4t == 2 ? k_fz_qp4<52, 1, 2> : k_fz_qp4<52, 1, 1>);
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SF_ECUDA;
-    if (cudaMemsetAsync(sched, 0, sizeof(int), st) != cudaSuccess) return SF_ECUDA;
     const int grid = (int)(n_items < n_sm ? n_items : n_sm);
     kern<<<grid, F4_THREADS, smem, st>>>(p, a);
     sf_count_launch(1);

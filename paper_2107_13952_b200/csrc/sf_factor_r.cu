@@ -286,7 +286,6 @@ int fz_launch_r2(const FzParams& p, const SfDims& D, int* sched, int n_sm, cudaS
         if (cudaFuncSetAttribute(k_fz_r2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SF_ECUDA;
         attr = smem;
     }
-    if (cudaMemsetAsync(sched, 0, sizeof(int), st) != cudaSuccess) return SF_ECUDA;
     const int grid = (int)(n_chunks < n_sm ? n_chunks : n_sm);
     k_fz_r2<<<grid, FZR_THREADS, smem, st>>>(p, a);
     sf_count_launch(1);

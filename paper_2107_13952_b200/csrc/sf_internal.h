@@ -102,7 +102,9 @@ struct SfSliceSizes {
     long n[5];    // elements of S1..S5
 };
 void sf_slice_sizes(const SfDims& D, SfSliceSizes* sz);
-int sf_build_slices(const SfDims& D, double* const S[5], const SfSixjTable& tab, cudaStream_t st);
+// one launch: the five S arrays and, when kr is given, the k-range tables kr[e * nl^3 + t] of the four edges (step 2)
+int sf_build_slices(const SfDims& D, double* const S[5], const SfSixjTable& tab, SfKRange* kr, cudaStream_t st);
+void sf_launch_kranges(const SfDims& D, SfKRange* out, cudaStream_t st);   // the k-range tables alone
 
 struct SfScratch;   // owned by the context (sf_api.cu)
 int sf_vertex_staged(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
@@ -114,6 +116,7 @@ bool sf_vertex_factor_supported(const SfDims& D);
 // scratch allocator owned by the context: grows on demand, freed by sf_finalize.  slot = small integer id.
 void* sf_scratch(int slot, size_t bytes);
 void sf_count_launch(int n);
+void sf_bump_generation(void);                    // drops the recorded launch sequences (sf_api.cu): call when a setting they depend on changes
 bool sf_timing_on(void);
 bool sf_counting_on(void);
 bool sf_poison_on(void);

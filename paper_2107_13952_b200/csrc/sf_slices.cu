@@ -10,6 +10,8 @@
 // o = l - j shell offsets (units of 1), a1 = (i1 - i1_min), q_a = (k_a - k_base_a) over the booster's padded k
 // layout, xx = (x - x_base) over the union range of x.  Entries whose triads fail are 0.  Values are gathered from
 // the resident canonical table when every argument fits in it, and evaluated directly otherwise.
+#include <string.h>
+
 #include "sf_sixj.cuh"
 #include "sf_slices.cuh"
 
@@ -25,9 +27,8 @@ void sf_slice_sizes(const SfDims& D, SfSliceSizes* sz)
 }
 
 template <int WHICH>
-__global__ void __launch_bounds__(128) k_slices(SliceArgs A, SfSixjTable tab, const SfFact* __restrict__ F)
+__device__ __forceinline__ void slice_entry(const SliceArgs& A, const SfSixjTable& tab, const SfFact* __restrict__ F, long q)
 {
-    const long q = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (q >= A.n[WHICH]) return;
     int a, b, c, d, e, f;
     slice_args<WHICH>(A, q, a, b, c, d, e, f);
@@ -40,7 +41,50 @@ __global__ void __launch_bounds__(128) k_slices(SliceArgs A, SfSixjTable tab, co
     A.S[WHICH][q] = v;
 }
 
-int sf_build_slices(const SfDims& D, double* const S[5], const SfSixjTable& tab, cudaStream_t st)
+// ONE launch for steps 2 and 4: blocks [first[w], first[w + 1]) fill S array w (w = 0..4), the blocks from first[5] on the
+// k-range tables of the four edges (small problems are bound by the number of dependent launches, not by their work)
+struct SliceTasks {
+    long first[7];
+    int nt;                 // triples per edge (nl^3); 0: no k-range task
+    SfKRange* kr;
+};
+__global__ void __launch_bounds__(128) k_slices(SliceArgs A, SfSixjTable tab, const SfFact* __restrict__ F, SliceTasks T)
+{
+    const long b = blockIdx.x;
+    if (b >= T.first[5]) {
+        const long q = (b - T.first[5]) * 128 + threadIdx.x;
+        if (q < 4L * T.nt) T.kr[q] = sf_krange_entry(A.two_j, A.nl, T.nt, (int)q);
+    } else if (b < T.first[1]) {
+        slice_entry<0>(A, tab, F, (b - T.first[0]) * 128 + threadIdx.x);
+    } else if (b < T.first[2]) {
+        slice_entry<1>(A, tab, F, (b - T.first[1]) * 128 + threadIdx.x);
+    } else if (b < T.first[3]) {
+        slice_entry<2>(A, tab, F, (b - T.first[2]) * 128 + threadIdx.x);
+    } else if (b < T.first[4]) {
+        slice_entry<3>(A, tab, F, (b - T.first[3]) * 128 + threadIdx.x);
+    } else {
+        slice_entry<4>(A, tab, F, (b - T.first[4]) * 128 + threadIdx.x);
+    }
+}
+
+// the k-range tables alone (callers that need no S arrays)
+__global__ void k_kranges(SliceArgs A, int nt, SfKRange* __restrict__ out)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < 4 * nt) out[q] = sf_krange_entry(A.two_j, A.nl, nt, q);
+}
+void sf_launch_kranges(const SfDims& D, SfKRange* out, cudaStream_t st)
+{
+    SliceArgs A;
+    memset(&A, 0, sizeof A);
+    for (int s = 0; s < 10; ++s) A.two_j[s] = D.two_j[s];
+    A.nl = D.nl;
+    const int nt = D.nl * D.nl * D.nl;
+    k_kranges<<<(4 * nt + 127) / 128, 128, 0, st>>>(A, nt, out);
+    sf_count_launch(1);
+}
+
+int sf_build_slices(const SfDims& D, double* const S[5], const SfSixjTable& tab, SfKRange* kr, cudaStream_t st)
 {
     SliceArgs A;
     for (int s = 0; s < 10; ++s) A.two_j[s] = D.two_j[s];
@@ -61,16 +105,16 @@ int sf_build_slices(const SfDims& D, double* const S[5], const SfSixjTable& tab,
     }
     const SfFact* F = sf_fact_table();
     if (!F) return SF_ENOTINIT;
-#define SF_LAUNCH(W)                                                                             \
-    if (A.n[W] > 0) {                                                                            \
-        k_slices<W><<<(unsigned)((A.n[W] + 127) / 128), 128, 0, st>>>(A, tab, F);                \
-        sf_count_launch(1);                                                                      \
+    SliceTasks T;
+    T.first[0] = 0;
+    for (int w = 0; w < 5; ++w) T.first[w + 1] = T.first[w] + (A.n[w] + 127) / 128;
+    T.nt = kr ? D.nl * D.nl * D.nl : 0;
+    T.kr = kr;
+    T.first[6] = T.first[5] + (4L * T.nt + 127) / 128;
+    if (T.first[6] > 2147483647L) return SF_EARG;
+    if (T.first[6] > 0) {
+        k_slices<<<(unsigned)T.first[6], 128, 0, st>>>(A, tab, F, T);
+        sf_count_launch(1);
     }
-    SF_LAUNCH(0)
-    SF_LAUNCH(1)
-    SF_LAUNCH(2)
-    SF_LAUNCH(3)
-    SF_LAUNCH(4)
-#undef SF_LAUNCH
     return cudaGetLastError() == cudaSuccess ? SF_OK : SF_ECUDA;
 }

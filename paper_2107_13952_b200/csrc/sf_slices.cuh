@@ -66,3 +66,26 @@ __device__ __forceinline__ void slice_args(const SliceArgs& A, long q, int& a, i
     }
 }
 
+
+// ranges of the virtual intertwiners k_a for every booster triple (step 2): the node's recoupling pairs with
+// the edge's three virtual spins at l = j + offset (superscript order of PAPER.md:171).  Entry q = e * nt + t.
+__device__ __forceinline__ SfKRange sf_krange_entry(const int* j, int nl, int nt, int q)
+{
+    const int e = q / nt, t = q % nt;
+    const int u = 2 * (t / (nl * nl)), v = 2 * ((t / nl) % nl), w = 2 * (t % nl);
+    int a, b, c, d;
+    if (e == 0) {          // node 2 (l23 l24 | l25 j12), triple (l23 l24 l25)
+        a = j[J23] + u; b = j[J24] + v; c = j[J25] + w; d = j[J12];
+    } else if (e == 1) {   // node 3 (l34 l35 | j13 l23), triple (l34 l35 l23)
+        a = j[J34] + u; b = j[J35] + v; c = j[J13]; d = j[J23] + w;
+    } else if (e == 2) {   // node 4 (l45 j14 | l24 l34), triple (l45 l24 l34)
+        a = j[J45] + u; b = j[J14]; c = j[J24] + v; d = j[J34] + w;
+    } else {               // node 5 (j15 l25 | l35 l45), triple (l25 l35 l45)
+        a = j[J15]; b = j[J25] + u; c = j[J35] + v; d = j[J45] + w;
+    }
+    const int lo = max(abs(a - b), abs(c - d)), hi = min(a + b, c + d);
+    SfKRange r;
+    r.two_k_min = lo;
+    r.n_k = (((a + b) ^ (c + d)) & 1) || hi < lo ? 0 : (hi - lo) / 2 + 1;
+    return r;
+}

@@ -36,9 +36,9 @@
 // ---------------------------------------------------------------------------------------------------------
 // small precomputations (step 2 windows, weighted / transposed operands)
 // ---------------------------------------------------------------------------------------------------------
-__global__ void k_fz_windows(SfProblem P, int2* w3A, int2* w3B, int2* w4A, int2* w4B)
+__device__ __forceinline__ void fz_windows_entry(const SfProblem& P, int2* w3A, int2* w3B, int2* w4A, int2* w4B, int t)
 {
-    const int nl = P.nl, t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nl = P.nl;
     const int* j = P.two_j;
     if (t < nl * nl) {
         const int u = t / nl, v = t % nl;
@@ -53,12 +53,12 @@ __global__ void k_fz_windows(SfProblem P, int2* w3A, int2* w3B, int2* w4A, int2*
 
 // Z[b25][a1][b35][b45][q4][v][i5] = (-1)^(o25+o35+o45+q4) sum_{k5 valid} (-1)^q5 {j14 k5 x; l35 k4 l45} {i1 l25 x; k5 j14 j15} (2k5+1) B5[t5][i5][q5]
 // one CTA per (b25, a1, b35, b45) and k4 (grid.y): single-shell problems (Delta_l = 0, large spins) have few (l25 l35 l45)
-__global__ void __launch_bounds__(256) k_fz_z(FzParams p, double* __restrict__ Z)
+__device__ __forceinline__ void fz_z_block(const FzParams& p, double* __restrict__ Z, long bx, int by, int gy)
 {
     const SfProblem& P = p.P;
     const int nl = P.nl, n1 = P.n_i[0], n5 = P.n_i[4], P4 = P.n_k_pad[2], P5 = P.n_k_pad[3], NX = P.n_x_pad, V = p.V;
     const int c35 = p.box.cnt[4], c45 = p.box.cnt[5];
-    long b = blockIdx.x;
+    long b = bx;
     const int b45 = (int)(b % c45); b /= c45;
     const int b35 = (int)(b % c35); b /= c35;
     const int a1 = (int)(b % n1);
@@ -69,11 +69,11 @@ __global__ void __launch_bounds__(256) k_fz_z(FzParams p, double* __restrict__ Z
     const int t5 = (o25 * nl + o35) * nl + o45;
     const SfKRange r5 = P.kr[3][t5];
     const int q5b = (r5.two_k_min - P.two_k_base[3]) >> 1;
-    double* z = Z + (long)blockIdx.x * P4 * V * n5;
-    const int nq4 = (P4 - (int)blockIdx.y + (int)gridDim.y - 1) / (int)gridDim.y;      // the k4 of this CTA: blockIdx.y + gridDim.y * n
+    double* z = Z + bx * P4 * V * n5;
+    const int nq4 = (P4 - by + gy - 1) / gy;      // the k4 of this block: by + gy * n
     const double* s1b = P.S[0] + (((long)(o25 * n1 + a1) * P5 + q5b) * NX) + xg0;
     for (int e = threadIdx.x; e < nq4 * nxs * n5; e += blockDim.x) {
-        const int i5 = e % n5, r = e / n5, v = r % nxs, q4 = blockIdx.y + gridDim.y * (r / nxs);
+        const int i5 = e % n5, r = e / n5, v = r % nxs, q4 = by + gy * (r / nxs);
         const double* s2 = P.S[1] + ((((long)(o35 * nl + o45) * P4 + q4) * P5 + q5b) * NX) + xg0 + v;
         const double* s1 = s1b + v;
         const double* b5 = sf_brow(P, 3, t5, i5) + q5b;
@@ -89,10 +89,9 @@ __global__ void __launch_bounds__(256) k_fz_z(FzParams p, double* __restrict__ Z
 }
 
 // Bw4T[q4][b45][b24][b34][i4] = (2k4+1) B4[(o45 o24 o34)][i4][q4] inside the triple's k-range, 0 outside
-__global__ void __launch_bounds__(256) k_fz_b4t(FzParams p, long n, double* __restrict__ out)
+__device__ __forceinline__ void fz_b4t_entry(const FzParams& p, long n, double* __restrict__ out, long e)
 {
     const SfProblem& P = p.P;
-    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (e >= n) return;
     const int nl = P.nl, n4 = P.n_i[3], P4 = P.n_k_pad[2];
     const int c24 = p.box.cnt[1], c34 = p.box.cnt[3], c45 = p.box.cnt[5];
@@ -111,10 +110,9 @@ __global__ void __launch_bounds__(256) k_fz_b4t(FzParams p, long n, double* __re
 }
 
 // Bw3T[q3][b34][b35][b23][i3] = (2k3+1) B3[(o34 o35 o23)][i3][q3] inside the triple's k-range, 0 outside
-__global__ void __launch_bounds__(256) k_fz_b3t(FzParams p, long n, double* __restrict__ out)
+__device__ __forceinline__ void fz_b3t_entry(const FzParams& p, long n, double* __restrict__ out, long e)
 {
     const SfProblem& P = p.P;
-    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (e >= n) return;
     const int nl = P.nl, n3 = P.n_i[2], P3 = P.n_k_pad[1];
     const int c23 = p.box.cnt[0], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
@@ -133,10 +131,9 @@ __global__ void __launch_bounds__(256) k_fz_b3t(FzParams p, long n, double* __re
 }
 
 // S3T[b24][b34][b35][xx][q3][q4] = (-1)^o34 {k4 l35 x; k3 l24 l34}
-__global__ void __launch_bounds__(256) k_fz_s3t(FzParams p, long n, double* __restrict__ out)
+__device__ __forceinline__ void fz_s3t_entry(const FzParams& p, long n, double* __restrict__ out, long e)
 {
     const SfProblem& P = p.P;
-    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (e >= n) return;
     const int nl = P.nl, P3 = P.n_k_pad[1], P4 = P.n_k_pad[2], NX = P.n_x_pad;
     const int c34 = p.box.cnt[3], c35 = p.box.cnt[4];
@@ -156,10 +153,9 @@ __global__ void __launch_bounds__(256) k_fz_s3t(FzParams p, long n, double* __re
 //                                   {k2 j13 x; i1 l25 j12} {l24 k3 x; j13 k2 l23}
 // h0 = (sum of boundary spins + i1 + sum of the k bases) / 2: with the signs folded into Z and S3T this is the
 // (-1)^R of eq. (5), 2R = sum of all fifteen labels (reading G1)
-__global__ void __launch_bounds__(256) k_fz_g(FzParams p, long n, double* __restrict__ out)
+__device__ __forceinline__ void fz_g_entry(const FzParams& p, long n, double* __restrict__ out, long e)
 {
     const SfProblem& P = p.P;
-    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (e >= n) return;
     const int nl = P.nl, n1 = P.n_i[0], n2 = P.n_i[1], P2 = P.n_k_pad[0], P3 = P.n_k_pad[1], NX = P.n_x_pad, V = p.V;
     const int c23 = p.box.cnt[0], c25 = p.box.cnt[2];
@@ -177,7 +173,7 @@ __global__ void __launch_bounds__(256) k_fz_g(FzParams p, long n, double* __rest
     // only the entries k_fz_gemm<FzMapA> reads: x of this (i1 l25), k3 allowed by (j13 l23) and by the triad (k3 l24 x)
     if (v >= nxs) return;
     {
-        const int2 wb = p.w3B[o23];
+        const int2 wb = fz_window(P.two_j[J13], P.two_j[J23] + 2 * o23, P.two_k_base[1], P3);   // = w3B[o23] (written by this very launch)
         const int k3 = P.two_k_base[1] + 2 * q3, l24 = P.two_j[J24] + 2 * o24, x = x0 + 2 * v;
         const int d = l24 > x ? l24 - x : x - l24;
         if (q3 < wb.x || q3 >= wb.x + wb.y || k3 < d || k3 > l24 + x || ((l24 + x + k3) & 1)) return;
@@ -204,14 +200,15 @@ __global__ void __launch_bounds__(256) k_fz_g(FzParams p, long n, double* __rest
 }
 
 // per k3: the l23 of the box that allow it (contiguous: |k3 - j13| <= l23 <= k3 + j13) and the (l34 l35) pairs that do
-__global__ void __launch_bounds__(32) k_fz_lists(FzParams p, int2* __restrict__ win23, int* __restrict__ kl3)
+__device__ __forceinline__ void fz_lists_warp(const FzParams& p, int2* __restrict__ win23, int* __restrict__ kl3, int q3, int lane)
 {
-    const int q3 = blockIdx.x, lane = threadIdx.x, nl = p.P.nl;
+    const SfProblem& P = p.P;
+    const int P3 = P.n_k_pad[1];
     const int c23 = p.box.cnt[0], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
     if (lane == 0) {
         int blo = -1, bcnt = 0;
         for (int b = 0; b < c23; ++b) {
-            const int2 w = p.w3B[p.box.lo[0] + b];
+            const int2 w = fz_window(P.two_j[J13], P.two_j[J23] + 2 * (p.box.lo[0] + b), P.two_k_base[1], P3);
             if (q3 >= w.x && q3 < w.x + w.y) {
                 if (blo < 0) blo = b;
                 ++bcnt;
@@ -225,7 +222,7 @@ __global__ void __launch_bounds__(32) k_fz_lists(FzParams p, int2* __restrict__ 
         const int c = base + lane;
         bool ok = false;
         if (c < c34 * c35) {
-            const int2 w = p.w3A[(p.box.lo[3] + c / c35) * nl + p.box.lo[4] + c % c35];
+            const int2 w = fz_window(P.two_j[J34] + 2 * (p.box.lo[3] + c / c35), P.two_j[J35] + 2 * (p.box.lo[4] + c % c35), P.two_k_base[1], P3);
             ok = q3 >= w.x && q3 < w.x + w.y;
         }
         const unsigned mask = __ballot_sync(0xffffffffu, ok);
@@ -233,6 +230,55 @@ __global__ void __launch_bounds__(32) k_fz_lists(FzParams p, int2* __restrict__ 
         cnt += __popc(mask);
     }
     if (lane == 0) list[0] = cnt;
+}
+
+// ONE launch for all the precomputations of a box: small problems are bound by the number of dependent launches, not by their
+// work (config 0: 3.4e6 flop per tensor).  Blocks [first[t], first[t + 1]) run task t; the tasks are independent of one another
+// (the windows the lists and G need are recomputed in place: a handful of integer operations).
+struct FzPreArgs {
+    long first[9];              // 0 G, 1 Z, 2 Bw4P / Bw4T, 3 Bw3T, 4 S3T, 5 windows, 6 lists, 7 scheduler counters; first[8] = all blocks
+    long nB4, padB4, nB3, nS3, padS3, nG;     // elements (pad: zeros behind the array, for whole-fragment reads)
+    int gy, b4p;                // k4 split of the Z blocks; booster layout: Bw4P (1, k_fz_qp2 / k_fz_qp4) or Bw4T (0, k_fz_qp)
+    int n_sched;
+    double *Z, *B4, *B3, *S3, *G;
+    int2 *w3A, *w3B, *w4A, *w4B, *win23;
+    int *kl3, *sched;
+};
+__global__ void __launch_bounds__(256) k_fz_pre(const __grid_constant__ FzParams p, const __grid_constant__ FzPreArgs a)
+{
+    const long b = blockIdx.x;
+    const int tid = threadIdx.x;
+    if (b < a.first[1]) {                                     // the heavy tasks first: their blocks must not start last
+        fz_g_entry(p, a.nG, a.G, (b - a.first[0]) * 256 + tid);
+    } else if (b < a.first[2]) {
+        const long bz = b - a.first[1];
+        fz_z_block(p, a.Z, bz / a.gy, (int)(bz % a.gy), a.gy);
+    } else if (b < a.first[3]) {
+        const long e = (b - a.first[2]) * 256 + tid;
+        if (e >= a.nB4) {
+            if (e < a.nB4 + a.padB4) a.B4[e] = 0.0;
+        } else if (a.b4p) {
+            fz_b4p_entry(p, a.nB4, a.B4, e);
+        } else {
+            fz_b4t_entry(p, a.nB4, a.B4, e);
+        }
+    } else if (b < a.first[4]) {
+        fz_b3t_entry(p, a.nB3, a.B3, (b - a.first[3]) * 256 + tid);
+    } else if (b < a.first[5]) {
+        const long e = (b - a.first[4]) * 256 + tid;
+        if (e >= a.nS3) {
+            if (e < a.nS3 + a.padS3) a.S3[e] = 0.0;
+        } else {
+            fz_s3t_entry(p, a.nS3, a.S3, e);
+        }
+    } else if (b < a.first[6]) {
+        fz_windows_entry(p.P, a.w3A, a.w3B, a.w4A, a.w4B, (int)(b - a.first[5]) * 256 + tid);
+    } else if (b < a.first[7]) {
+        const int q3 = (int)(b - a.first[6]) * 8 + (tid >> 5);
+        if (q3 < p.P.n_k_pad[1]) fz_lists_warp(p, a.win23, a.kl3, q3, tid & 31);
+    } else {
+        for (int i = tid; i < a.n_sched; i += 256) a.sched[i] = 0;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -966,9 +1012,17 @@ static FzShape fz_shape(const SfDims& D)
 bool sf_vertex_factor_supported(const SfDims& D) { return fz_shape(D).ok; }
 
 static int g_fz_variant = 0;                         // sf_set_factor_variant: bit 0 = R through the booster-stationary kernel
-extern "C" void sf_set_factor_variant(int bits) { g_fz_variant = bits; }
+extern "C" void sf_set_factor_variant(int bits)
+{
+    g_fz_variant = bits;
+    sf_bump_generation();
+}
 static size_t g_fz_budget = 0;                       // sf_set_factor_budget: bytes for P and R of one pass (0 = a third of the device)
-extern "C" void sf_set_factor_budget(unsigned long bytes) { g_fz_budget = bytes; }
+extern "C" void sf_set_factor_budget(unsigned long bytes)
+{
+    g_fz_budget = bytes;
+    sf_bump_generation();
+}
 
 template <class Map, int WGM, int WGN, int TM, int TN>
 static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
@@ -1029,7 +1083,6 @@ extern "C" int sf_last_dmma(double n[3])
 int fz_launch_r2(const FzParams& p, const SfDims& D, int* sched, int n_sm, cudaStream_t st);   // sf_factor_r.cu
 bool fz_qp2_supported(const FzParams& p, const SfDims& D);                                     // sf_factor_qp.cu
 long fz_qp2_b4p_elems(const FzParams& p, const SfDims& D);
-void fz_launch_b4p(const FzParams& p, long n, double* out, cudaStream_t st);
 int fz_launch_qp2(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st);
 bool fz_qp4_supported(const FzParams& p, const SfDims& D);                                     // sf_factor_qp4.cu
 int fz_launch_qp4(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st);
@@ -1060,7 +1113,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     p.VG = sh.VG;
     for (int s = 0; s < 10; ++s) p.jsum += D.two_j[s];
 
-    int* sched = (int*)sf_scratch(FZ_SLOT_SCHED, 64);
+    int* sched = (int*)sf_scratch(FZ_SLOT_SCHED, sizeof(int) * 1024);   // work counters: [pass] Q/P kernel, [512 + pass] R kernel
     if (!sched) return SF_ENOMEM;
     int2* win = (int2*)sf_scratch(FZ_SLOT_WIN, sizeof(int2) * (2 * (size_t)nl * nl + 2 * nl));
     double* Apart = (double*)sf_scratch(FZ_SLOT_PART, sizeof(double) * (size_t)(parts > 0 ? parts : 1) * D.n_out);
@@ -1071,10 +1124,6 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     p.w4A = w4A;
     p.w4B = w4B;
     p.Apart = Apart;
-    if (nbox > 0) {
-        k_fz_windows<<<(nl * nl + 127) / 128, 128, 0, st>>>(P, w3A, w3B, w4A, w4B);
-        sf_count_launch(1);
-    }
     static bool qp_attr = false;
     if (!qp_attr) {
         if (cudaFuncSetAttribute(k_fz_qp, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024) != cudaSuccess) return SF_ECUDA;
@@ -1162,25 +1211,43 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             SF_CUDA_OK(cudaMemsetAsync(G, 0xFF, sizeof(double) * (size_t)nG, st));
         }
         fz_ev_begin(3, st);
-        {   // few (l25 i1 l35 l45): spread the k4 over grid.y as well
-            const long nz = c25 * n1 * c35 * c45;
-            const int gy = nz >= 592 ? 1 : (int)((592 + nz - 1) / nz < P4 ? (592 + nz - 1) / nz : P4);
-            k_fz_z<<<dim3((unsigned)nz, (unsigned)gy), 256, 0, st>>>(p, Z);
+        {   // every precomputation of the box in one launch (k_fz_pre)
+            FzPreArgs a;
+            memset(&a, 0, sizeof a);
+            const long nz = c25 * n1 * c35 * c45;            // few (l25 i1 l35 l45): spread the k4 over more blocks as well
+            a.gy = nz >= 592 ? 1 : (int)((592 + nz - 1) / nz < P4 ? (592 + nz - 1) / nz : P4);
+            a.b4p = qp2;
+            a.nB4 = nB4;
+            a.padB4 = qp2 ? padB4 : 0;
+            a.nB3 = nB3;
+            a.nS3 = nS3;
+            a.padS3 = padS3;
+            a.nG = nG;
+            a.n_sched = 1024;
+            a.Z = Z;
+            a.B4 = B4;
+            a.B3 = B3;
+            a.S3 = S3;
+            a.G = G;
+            a.w3A = w3A;
+            a.w3B = w3B;
+            a.w4A = w4A;
+            a.w4B = w4B;
+            a.win23 = (int2*)lists;
+            a.kl3 = lists + 2 * P3;
+            a.sched = sched;
+            const long nb[8] = {(nG + 255) / 256, nz * a.gy, (a.nB4 + a.padB4 + 255) / 256, (nB3 + 255) / 256,
+                                (nS3 + padS3 + 255) / 256, (nl * nl + 255) / 256, (P3 + 7) / 8, 1};
+            a.first[0] = 0;
+            for (int t = 0; t < 8; ++t) a.first[t + 1] = a.first[t] + nb[t];
+            if (a.first[8] > 2147483647L) return SF_EARG;
+            if (n1 > 512) return SF_EARG;                    // one counter per pass over i1
+            k_fz_pre<<<(unsigned)a.first[8], 256, 0, st>>>(p, a);
         }
-        if (qp2) {
-            fz_launch_b4p(p, nB4, B4, st);
-            SF_CUDA_OK(cudaMemsetAsync(S3 + nS3, 0, sizeof(double) * (size_t)padS3, st));
-            SF_CUDA_OK(cudaMemsetAsync(B4 + nB4, 0, sizeof(double) * (size_t)padB4, st));
-        } else {
-            k_fz_b4t<<<(unsigned)((nB4 + 255) / 256), 256, 0, st>>>(p, nB4, B4);
-        }
-        k_fz_b3t<<<(unsigned)((nB3 + 255) / 256), 256, 0, st>>>(p, nB3, B3);
-        k_fz_s3t<<<(unsigned)((nS3 + 255) / 256), 256, 0, st>>>(p, nS3, S3);
-        k_fz_g<<<(unsigned)((nG + 255) / 256), 256, 0, st>>>(p, nG, G);
-        k_fz_lists<<<P3, 32, 0, st>>>(p, (int2*)lists, lists + 2 * P3);
-        sf_count_launch(6);
+        sf_count_launch(1);
         fz_ev_end(st);
-        for (int a_lo = 0; a_lo < n1; a_lo += (int)na) {
+        int pass = 0;
+        for (int a_lo = 0; a_lo < n1; a_lo += (int)na, ++pass) {
             p.a_lo = a_lo;
             p.a_cnt = (int)(a_lo + na <= n1 ? na : n1 - a_lo);
             if (sf_poison_on()) {
@@ -1189,7 +1256,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             }
             fz_ev_begin(0, st);
             if (qp2) {
-                const int rcq = qp4 ? fz_launch_qp4(p, D, B4, sched + 1, n_sm, st) : fz_launch_qp2(p, D, B4, sched + 1, n_sm, st);
+                const int rcq = qp4 ? fz_launch_qp4(p, D, B4, sched + pass, n_sm, st) : fz_launch_qp2(p, D, B4, sched + pass, n_sm, st);
                 if (rcq != SF_OK) return rcq;
             } else {                                  // shapes the second-generation kernel does not hold
                 const long n_items = (long)p.a_cnt * c25 * c35 * c24 * c34;
@@ -1199,7 +1266,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             }
             fz_ev_end(st);
             fz_ev_begin(1, st);
-            int rc = g_fz_variant & 1 ? fz_launch_r2(p, D, sched, n_sm, st) : SF_EARG;         // booster block stationary, P streamed once
+            int rc = g_fz_variant & 1 ? fz_launch_r2(p, D, sched + 512 + pass, n_sm, st) : SF_EARG;         // booster block stationary, P streamed once
             if (rc == SF_EARG) rc = fz_launch_gemm<FzMapR, 8, 1, 2, 8>(p, (int)(c34 * c35), st);   // shapes it does not hold
             fz_ev_end(st);
             if (rc != SF_OK) return rc;

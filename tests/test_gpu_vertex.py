@@ -164,6 +164,55 @@ def test_factorised_kernel_variants_against_the_oracle(bits):
         sf.sf_set_path(0)
 
 
+def test_recorded_launch_sequences_replay_the_plain_call():
+    """sf_set_graphs (include/sfoam.h): from the third identical call on, a vertex call replays a recorded CUDA graph.  The
+    replay must equal the plain call bit for bit, follow booster VALUES changed in place, and be dropped when a setting
+    changes (here: the path)."""
+    cfg = wl.config2(2)
+    two_j, two_dl = cfg["two_j"], cfg["two_dl"]
+    B = boosters_for(cfg)
+    Bdev = to_device(B)
+    _, n_i = sf.sf_vertex_dims(two_j)
+    out = torch.full(tuple(n_i), float("nan"), dtype=torch.float64, device="cuda")
+    st = torch.cuda.current_stream()
+
+    def call():
+        out.fill_(float("nan"))
+        sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, st)
+        torch.cuda.synchronize()
+        return out.cpu().numpy().copy()
+
+    try:
+        sf.sf_set_graphs(0)
+        plain = call()
+        sf.sf_set_graphs(1)
+        runs = [call() for _ in range(5)]                 # 1: plain, 2: plain + remembered, 3: recorded + replayed, 4, 5: replayed
+        for r in runs:
+            assert np.array_equal(r, plain)
+        n0 = sf.sf_launch_count()
+        call()
+        assert sf.sf_launch_count() > n0                  # a replay still reports the launches it stands for
+        # new booster values behind the same pointers
+        Bdev[3].mul_(-2.0)
+        scaled = call()
+        sf.sf_set_graphs(0)
+        assert np.array_equal(call(), scaled)
+        assert np.abs(scaled + 2.0 * plain).max() <= 1e-12 * np.abs(plain).max()      # multilinear in every booster
+        sf.sf_set_graphs(1)
+        # another path: the recordings of the old setting must not be replayed
+        for _ in range(3):
+            call()
+        sf.sf_set_path(3)
+        line = call()
+        assert sf.sf_last_path() == 3
+        assert np.abs(line - scaled).max() <= 1e-12 * np.abs(scaled).max()
+        Ao, Aabs = run_oracle(two_j, two_dl, {e: Bdev[e].cpu().numpy() for e in Bdev})
+        assert_parity(scaled, Ao, Aabs, what="replayed call")
+    finally:
+        sf.sf_set_graphs(1)
+        sf.sf_set_path(0)
+
+
 def test_paths_agree_on_a_full_tensor():
     """Config 2, Delta_l = 4 (15 625 shells) in full: the factorised and the per-shell line path give the same tensor to
     rounding, and both match the oracle."""
