@@ -36,9 +36,10 @@
  * entry point returns SF_ECUDA.
  *
  * Concurrency: one context per process, bound to the device that was current at sf_init; the library keeps its scratch
- * buffers and path selection in that context, so calls must not overlap (issue them from one thread, or serialise them).
- * Calls are asynchronous on the stream they are given; two vertex calls on different streams share the scratch buffers and
- * must be ordered by the caller.
+ * buffers and settings in that context.  Compute calls are therefore SERIALISED by the library: host threads by a mutex,
+ * streams by an event -- a call on another stream than the previous call's first waits (on the device) for that call, so
+ * two vertex calls on different streams are correct but do not overlap.  Calls are asynchronous on the stream they are
+ * given.  Inside the caller's own stream capture the library adds no event: ordering is then the caller's graph.
  */
 #ifndef SFOAM_H
 #define SFOAM_H

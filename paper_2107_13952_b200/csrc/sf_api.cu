@@ -4,6 +4,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "sf_internal.h"
 
 #define SF_NSCRATCH 40
@@ -27,8 +29,34 @@ struct SfContext {
     bool capturing = false;
     bool graphs = true;    // sf_set_graphs
     cudaStream_t cap_stream = nullptr;
+    cudaEvent_t done = nullptr;     // end of the last compute call (SfCallGuard)
+    cudaStream_t last_stream = nullptr;
+    bool have_last = false;
 };
 static SfContext g_ctx;
+static std::recursive_mutex g_call_mutex;
+
+SfCallGuard::SfCallGuard(cudaStream_t s) : st(s), events(false)
+{
+    g_call_mutex.lock();
+    if (!g_ctx.init || !g_ctx.done) return;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        return;                        // inside the caller's own capture: ordering is the caller's graph
+    }
+    events = true;
+    if (g_ctx.have_last && g_ctx.last_stream != st) cudaStreamWaitEvent(st, g_ctx.done, 0);   // the scratch buffers are shared
+}
+SfCallGuard::~SfCallGuard()
+{
+    if (events) {
+        cudaEventRecord(g_ctx.done, st);
+        g_ctx.last_stream = st;
+        g_ctx.have_last = true;
+    }
+    g_call_mutex.unlock();
+}
 
 void sf_bump_generation(void) { ++g_ctx.gen; }
 
@@ -82,6 +110,8 @@ extern "C" int sf_init(double gamma)
     for (int q = 0; q < 4; ++q)
         if (cudaEventCreate(&g_ctx.ev[q]) != cudaSuccess) return SF_ECUDA;
     if (cudaStreamCreateWithFlags(&g_ctx.cap_stream, cudaStreamNonBlocking) != cudaSuccess) return SF_ECUDA;
+    if (cudaEventCreateWithFlags(&g_ctx.done, cudaEventDisableTiming) != cudaSuccess) return SF_ECUDA;
+    g_ctx.have_last = false;
     g_ctx.gamma = gamma;
     g_ctx.init = true;
     g_ctx.launches = 0;
@@ -104,6 +134,9 @@ extern "C" int sf_finalize(void)
     for (int q = 0; q < 4; ++q) cudaEventDestroy(g_ctx.ev[q]);
     if (g_ctx.cap_stream) cudaStreamDestroy(g_ctx.cap_stream);
     g_ctx.cap_stream = nullptr;
+    if (g_ctx.done) cudaEventDestroy(g_ctx.done);
+    g_ctx.done = nullptr;
+    g_ctx.have_last = false;
     g_ctx.init = false;
     return SF_OK;
 }
@@ -418,12 +451,14 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
 extern "C" int sf_vertex_amplitude(const int two_j[10], int two_dl, const sf_boosters* boosters, double* out,
                                    sf_stream_t stream)
 {
+    SfCallGuard guard((cudaStream_t)stream);
     return vertex_range(two_j, two_dl, boosters, 0, 0, out, (cudaStream_t)stream, true);
 }
 
 extern "C" int sf_vertex_amplitude_range(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo,
                                          long shell_hi, double* out, sf_stream_t stream)
 {
+    SfCallGuard guard((cudaStream_t)stream);
     return vertex_range(two_j, two_dl, boosters, shell_lo, shell_hi, out, (cudaStream_t)stream, false);
 }
 
@@ -431,6 +466,7 @@ extern "C" int sf_vertex_amplitude_intertwiners(const int two_j[10], int two_dl,
                                                 const int i_first[5], const int i_count[5], double* out, sf_stream_t stream)
 {
     if (!i_first || !i_count) return SF_EARG;
+    SfCallGuard guard((cudaStream_t)stream);
     return vertex_range(two_j, two_dl, boosters, 0, 0, out, (cudaStream_t)stream, true, i_first, i_count);
 }
 
@@ -448,6 +484,7 @@ extern "C" int sf_vertex_amplitude_batch(int n, const int* two_j, const int* two
     if (!g_ctx.init) return SF_ENOTINIT;
     if (n < 0 || (n > 0 && (!two_j || !two_dl || !boosters || !out))) return SF_EARG;
     if (n == 0) return SF_OK;
+    SfCallGuard guard((cudaStream_t)stream);
     return sf_vertex_batch_run(n, two_j, two_dl, boosters, out, (cudaStream_t)stream);
 }
 
@@ -457,6 +494,7 @@ extern "C" int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const d
     if (!g_ctx.init) return SF_ENOTINIT;
     if (!two_j || !host_boosters || !host_out) return SF_EARG;
     cudaStream_t st = (cudaStream_t)stream;
+    SfCallGuard guard(st);
     SfDims D;
     int rc = sf_host_dims(two_j, two_dl, &D);
     if (rc != SF_OK) return rc;

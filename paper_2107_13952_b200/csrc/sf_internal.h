@@ -116,6 +116,14 @@ bool sf_vertex_factor_supported(const SfDims& D);
 // scratch allocator owned by the context: grows on demand, freed by sf_finalize.  slot = small integer id.
 void* sf_scratch(int slot, size_t bytes);
 void sf_count_launch(int n);
+// Guard of every compute entry point of the C ABI: the library keeps ONE set of scratch buffers, so calls are serialised --
+// host threads by a mutex, streams by an event (a call on another stream than the previous call's first waits for that call).
+struct SfCallGuard {
+    explicit SfCallGuard(cudaStream_t st);
+    ~SfCallGuard();
+    cudaStream_t st;
+    bool events;
+};
 void sf_bump_generation(void);                    // drops the recorded launch sequences (sf_api.cu): call when a setting they depend on changes
 bool sf_timing_on(void);
 bool sf_counting_on(void);

@@ -213,6 +213,35 @@ def test_recorded_launch_sequences_replay_the_plain_call():
         sf.sf_set_path(0)
 
 
+def test_calls_on_two_streams_share_the_scratch_buffers_safely():
+    """The library has one set of scratch buffers; calls on different streams are serialised by an event (include/sfoam.h,
+    Concurrency).  Two different problems issued back to back on two streams, no synchronisation in between, must both
+    come out bit for bit as when they run alone."""
+    cfgs = [wl.config2(4), wl.config2(3), wl.CONFIGS[0]]
+    prob = []
+    for cfg in cfgs:
+        B = boosters_for(cfg)
+        prob.append((cfg["two_j"], cfg["two_dl"], to_device(B), sf.sf_vertex_dims(cfg["two_j"])[1]))
+    alone = []
+    for two_j, two_dl, Bdev, n_i in prob:
+        out = torch.full(tuple(n_i), float("nan"), dtype=torch.float64, device="cuda")
+        sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        alone.append(out.cpu().numpy())
+    streams = [torch.cuda.Stream() for _ in prob]
+    for rep in range(3):
+        outs = []
+        for (two_j, two_dl, Bdev, n_i), st in zip(prob, streams):
+            out = torch.full(tuple(n_i), float("nan"), dtype=torch.float64, device="cuda")
+            torch.cuda.synchronize()                      # the fill is done; from here on only the library orders the streams
+            outs.append(out)
+        for (two_j, two_dl, Bdev, n_i), st, out in zip(prob, streams, outs):
+            sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, st)
+        torch.cuda.synchronize()
+        for out, ref in zip(outs, alone):
+            assert np.array_equal(out.cpu().numpy(), ref)
+
+
 def test_paths_agree_on_a_full_tensor():
     """Config 2, Delta_l = 4 (15 625 shells) in full: the factorised and the per-shell line path give the same tensor to
     rounding, and both match the oracle."""
