@@ -66,6 +66,8 @@ void sf_set_factor_budget(unsigned long bytes);
  * (k_fz_qp); bit 2 = take Q/P through the second-generation kernel (k_fz_qp2) instead of the warp-autonomous one (k_fz_qp4).
  * 0 = default (the fastest kernels that hold the shape).  All variants compute the same sums. */
 void sf_set_factor_variant(int bits);
+/* The Q/P kernel the last factorised call (its last box) took: 1 = k_fz_qp, 2 = k_fz_qp2, 4 = k_fz_qp4; 0 before any call. */
+int sf_last_qp_kernel(void);
 
 #ifdef __cplusplus
 }

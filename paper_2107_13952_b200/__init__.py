@@ -188,6 +188,11 @@ def sf_set_factor_variant(bits):
     _lib().sf_set_factor_variant(int(bits))
 
 
+def sf_last_qp_kernel():
+    """Q/P kernel of the last factorised call: 1 k_fz_qp, 2 k_fz_qp2, 4 k_fz_qp4 (include/sfoam_debug.h)."""
+    return int(_lib().sf_last_qp_kernel())
+
+
 def sf_set_factor_budget(nbytes):
     """Device bytes the factorised path may use for P and R of one pass over i1 (0 = default, a third of the device)."""
     _lib().sf_set_factor_budget(int(nbytes))

@@ -1011,6 +1011,8 @@ static FzShape fz_shape(const SfDims& D)
 
 bool sf_vertex_factor_supported(const SfDims& D) { return fz_shape(D).ok; }
 
+static int g_fz_last_qp = 0;                         // Q/P kernel of the last call: 1 k_fz_qp, 2 k_fz_qp2, 4 k_fz_qp4 (sf_last_qp_kernel)
+extern "C" int sf_last_qp_kernel(void) { return g_fz_last_qp; }
 static int g_fz_variant = 0;                         // sf_set_factor_variant: bit 0 = R through the booster-stationary kernel
 extern "C" void sf_set_factor_variant(int bits)
 {
@@ -1166,6 +1168,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         const long nZ = c25 * n1 * c35 * c45 * ((long)P4 * sh.V * n5);
         const bool qp4 = !(g_fz_variant & 6) && fz_qp4_supported(p, D);      // warp-autonomous Q/P kernel (one warp per unit)
         const bool qp2 = qp4 || (!(g_fz_variant & 2) && fz_qp2_supported(p, D));   // second generation; both use the booster layout Bw4P
+        g_fz_last_qp = qp4 ? 4 : qp2 ? 2 : 1;
         const long nB4 = qp2 ? fz_qp2_b4p_elems(p, D) : (long)P4 * c45 * c24 * c34 * n4, nB3 = (long)P3 * c34 * c35 * c23 * n3;
         const long nS3 = c24 * c34 * c35 * D.n_x_pad * P3 * P4;
         const long nG = c24 * c25 * n1 * P3 * sh.V * c23 * n2;

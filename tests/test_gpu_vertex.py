@@ -242,6 +242,38 @@ def test_calls_on_two_streams_share_the_scratch_buffers_safely():
             assert np.array_equal(out.cpu().numpy(), ref)
 
 
+QP4_CLASSES = [      # (two_j, two_dl, shells or None = all): one spin set per instantiation k_fz_qp4<LDZ, N5T, N4T> (sf_factor_qp4.cu)
+    pytest.param([11, 0, 0, 11, 9, 2, 0, 13, 10, 11], 2, None, id="ldz52-n5t1-n4t1"),
+    pytest.param([0, 10, 12, 12, 11, 13, 8, 9, 0, 10], 2, None, id="ldz52-n5t1-n4t2"),
+    pytest.param([13, 5, 2, 8, 0, 6, 11, 10, 11, 8], 2, None, id="ldz52-n5t2-n4t1"),
+    pytest.param([1, 1, 9, 11, 4, 8, 11, 13, 8, 12], 2, None, id="ldz52-n5t2-n4t2"),
+    pytest.param([3, 12, 3, 12, 3, 7, 13, 3, 12, 13], 2, None, id="ldz68-n5t2-n4t1"),
+    pytest.param([13, 10, 13, 12, 12, 9, 14, 8, 14, 12], 2, (21, 27), id="ldz68-n5t2-n4t2"),
+]
+
+
+@pytest.mark.parametrize("two_j,two_dl,shells", QP4_CLASSES)
+def test_qp4_template_classes_against_the_oracle(two_j, two_dl, shells):
+    """k_fz_qp4 is compiled for one or two tiles of i5 and of i4 and two strides of its Z slab; the five workloads reach two
+    of the six instantiations.  One irregular spin set per instantiation (found by a seeded search over 2j <= 14), each on
+    the factorised path with the Q/P kernel checked, against the oracle."""
+    cfg = dict(two_j=two_j, two_dl=two_dl, boosters="random", seed=4100 + sum(two_j))
+    B = boosters_for(cfg)
+    sf.sf_set_path(4)
+    try:
+        if shells is None:
+            Ag = run_gpu(two_j, two_dl, B)
+            Ao, Aabs = run_oracle(two_j, two_dl, B)
+        else:
+            Ag = run_gpu(two_j, two_dl, B, shells[0], shells[1])
+            Ao, Aabs = run_oracle(two_j, two_dl, B, shells[0], shells[1])
+        assert sf.sf_last_path() == 4 and sf.sf_last_qp_kernel() == 4
+        assert np.abs(Ao).max() > 0
+        assert_parity(Ag, Ao, Aabs, what=f"qp4 class {two_j}")
+    finally:
+        sf.sf_set_path(0)
+
+
 def test_paths_agree_on_a_full_tensor():
     """Config 2, Delta_l = 4 (15 625 shells) in full: the factorised and the per-shell line path give the same tensor to
     rounding, and both match the oracle."""
