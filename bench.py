@@ -500,7 +500,7 @@ def run_ours(args, cfg, rank, world, local_rank):
 
     ms_step = ms / args.steps
     value = whole_job_value(n_shells, args.steps, world, ms * 1e-3)
-    kern_ms = stage[1] / args.steps                                     # the fused (or staged) steps 5-6(iii) kernel(s)
+    kern_ms = stage[1] / args.steps                                     # the kernel(s) of steps 5-6(iii)
     achieved = (f_con + f_asm) / (kern_ms * 1e-3) / 1e12
     peak_dfma, peak_dmma = sf.sf_fp64_peak(0), sf.sf_fp64_peak(1)
     peak = max(peak_dfma, peak_dmma)

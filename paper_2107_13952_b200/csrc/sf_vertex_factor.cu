@@ -9,11 +9,11 @@
 // one shell and contracts it with that shell's four boosters; by linearity the same sum can be taken one virtual spin
 // at a time, keeping the recoupling spin x open.  The order used here, all FP64:
 //
-//   Z [l25 i1 l35 l45; k4 x i5]        = sum_k5   S2 S1 Bw5                      (k_fz_z: two {6j} of eq. (5) and the edge-5 product)
-//   Q [.. l24 l34; k4 x i5 i4]         = sum_l45  Z Bw4                          (k_fz_qp, first half: the shells of a line l45 = j..j+Dl)
-//   P [l24 l25 i1; k3 x; l34 l35; i5 i4] = sum_k4 S3 Q                           (k_fz_qp, second half: third {6j}, edge-4 mode product)
+//   Z [l25 i1 l35 l45; k4 x i5]        = sum_k5   S2 S1 Bw5                      (k_fz_pre, task Z: two {6j} of eq. (5) and the edge-5 product)
+//   Q [.. l24 l34; k4 x i5 i4]         = sum_l45  Z Bw4                          (k_fz_qp4, Q phase: the shells of a line l45 = j..j+Dl)
+//   P [l24 l25 i1; k3 x; l34 l35; i5 i4] = sum_k4 S3 Q                           (k_fz_qp4, P phase: third {6j}, edge-4 mode product)
 //   R [l24 l25 i1; k3 x; l23 i3; i5 i4]  = sum_{l34 l35} Bw3 P                   (k_fz_gemm<FzMapR>: edge-3 mode product + shell sum)
-//   G [l23 l24 l25 i1; k3 x; i2]       = sum_k2   Bw2 (-1)^.. (2x+1) S5 S4       (k_fz_g: last two {6j}, edge-2 booster)
+//   G [l23 l24 l25 i1; k3 x; i2]       = sum_k2   Bw2 (-1)^.. (2x+1) S5 S4       (k_fz_pre, task G: last two {6j}, edge-2 booster)
 //   A'[l24 l25; i1 i2 i3 i4 i5]        = sum_{k3 x l23} G R                      (k_fz_gemm<FzMapA>: sum over x of eq. (5), edge-2 product)
 //   A [i1..i5]                         = N(i) sum_{l24 l25} A'                   (k_fz_reduce: fixed order, step 6(iv) + eq. (3))
 //
@@ -1261,7 +1261,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             if (qp2) {
                 const int rcq = qp4 ? fz_launch_qp4(p, D, B4, sched + pass, n_sm, st) : fz_launch_qp2(p, D, B4, sched + pass, n_sm, st);
                 if (rcq != SF_OK) return rcq;
-            } else {                                  // shapes the second-generation kernel does not hold
+            } else {                                  // shapes the newer kernels do not hold
                 const long n_items = (long)p.a_cnt * c25 * c35 * c24 * c34;
                 const long grid = n_items < 2L * n_sm ? n_items : 2L * n_sm;
                 k_fz_qp<<<(unsigned)grid, FZ_QP_THREADS, sh.qp_smem, st>>>(p, n_items);
