@@ -1182,6 +1182,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             na = 1;                                  // a test budget below one i1 still runs, one i1 per pass
         }
         if (na > n1) na = n1;
+        na = (n1 + (n1 + na - 1) / na - 1) / ((n1 + na - 1) / na);   // the same number of passes, of equal size (config 3: 4 + 4 + 3, not 5 + 5 + 1)
         double* Z = (double*)sf_scratch(FZ_SLOT_Z, sizeof(double) * (size_t)nZ);
         const long padB4 = 4L * 12 * 16;             // k_fz_qp4 copies whole k-steps (4 k4) of Bw4P: the last one may end past the array
         double* B4 = (double*)sf_scratch(FZ_SLOT_B4, sizeof(double) * (size_t)(nB4 + padB4));
