@@ -78,7 +78,12 @@ __device__ __forceinline__ void fz_z_block(const FzParams& p, double* __restrict
         const double* s1 = s1b + v;
         const double* b5 = sf_brow(P, 3, t5, i5) + q5b;
         double val = 0.0;
-        for (int c = 0; c < r5.n_k; ++c) {
+        // {j14 k5 x; l35 k4 l45} vanishes unless the triads (j14 k4 l45) and (l35 k4 x) hold: such entries are exact zeros
+        const int k4 = P.two_k_base[2] + 2 * q4, x = x0 + 2 * v;
+        const int l35 = P.two_j[J35] + 2 * o35, l45 = P.two_j[J45] + 2 * o45, j14 = P.two_j[J14];
+        const bool live = k4 >= abs(j14 - l45) && k4 <= j14 + l45 && !((j14 + l45 + k4) & 1) && k4 >= abs(l35 - x) && k4 <= l35 + x &&
+                          !((l35 + x + k4) & 1);
+        for (int c = 0; live && c < r5.n_k; ++c) {
             double term = s2[(long)c * NX] * s1[(long)c * NX] * ((double)(r5.two_k_min + 2 * c + 1) * b5[c]);
             if ((q5b + c) & 1) term = -term;
             val += term;
@@ -153,41 +158,48 @@ __device__ __forceinline__ void fz_s3t_entry(const FzParams& p, long n, double* 
 //                                   {k2 j13 x; i1 l25 j12} {l24 k3 x; j13 k2 l23}
 // h0 = (sum of boundary spins + i1 + sum of the k bases) / 2: with the signs folded into Z and S3T this is the
 // (-1)^R of eq. (5), 2R = sum of all fifteen labels (reading G1)
-__device__ __forceinline__ void fz_g_entry(const FzParams& p, long n, double* __restrict__ out, long e)
+// One block per (b24 b25 a1 q3): only the x of the triad (k3 l24 x) and the l23 of the pair (j13 l23) that allow this k3 are
+// visited (three quarters of the dense index space (v, l23) are excluded by them: a thread per dense entry spent its time
+// on early exits), entries (v, b23, i2) in memory order.
+__device__ __forceinline__ void fz_g_block(const FzParams& p, double* __restrict__ out, long blk_id)
 {
     const SfProblem& P = p.P;
-    if (e >= n) return;
     const int nl = P.nl, n1 = P.n_i[0], n2 = P.n_i[1], P2 = P.n_k_pad[0], P3 = P.n_k_pad[1], NX = P.n_x_pad, V = p.V;
     const int c23 = p.box.cnt[0], c25 = p.box.cnt[2];
-    long r = e;
-    const int i2 = (int)(r % n2); r /= n2;
-    const int b23 = (int)(r % c23); r /= c23;
-    const int v = (int)(r % V); r /= V;
+    long r = blk_id;
     const int q3 = (int)(r % P3); r /= P3;
     const int a1 = (int)(r % n1); r /= n1;
     const int b25 = (int)(r % c25);
     const int b24 = (int)(r / c25);
-    const int o23 = p.box.lo[0] + b23, o24 = p.box.lo[1] + b24, o25 = p.box.lo[2] + b25;
+    const int o24 = p.box.lo[1] + b24, o25 = p.box.lo[2] + b25;
     int x0, nxs, xg0;
     fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, a1, o25, x0, nxs, xg0);
-    // only the entries k_fz_gemm<FzMapA> reads: x of this (i1 l25), k3 allowed by (j13 l23) and by the triad (k3 l24 x)
-    if (v >= nxs) return;
-    {
-        const int2 wb = fz_window(P.two_j[J13], P.two_j[J23] + 2 * o23, P.two_k_base[1], P3);   // = w3B[o23] (written by this very launch)
-        const int k3 = P.two_k_base[1] + 2 * q3, l24 = P.two_j[J24] + 2 * o24, x = x0 + 2 * v;
-        const int d = l24 > x ? l24 - x : x - l24;
-        if (q3 < wb.x || q3 >= wb.x + wb.y || k3 < d || k3 > l24 + x || ((l24 + x + k3) & 1)) return;
+    // only the entries k_fz_gemm<FzMapA> reads: x of this (i1 l25) with the triad (k3 l24 x), k3 allowed by (j13 l23)
+    const int2 vr = fz_vrange(P.two_j[J24] + 2 * o24, P.two_k_base[1] + 2 * q3, x0, nxs);
+    if (vr.y == 0) return;
+    int blo = 0, bcnt = 0;                                    // the l23 of the box whose pair (j13 l23) allows k3: contiguous
+    for (int b = 0; b < c23; ++b) {
+        const int2 wb = fz_window(P.two_j[J13], P.two_j[J23] + 2 * (p.box.lo[0] + b), P.two_k_base[1], P3);
+        if (q3 >= wb.x && q3 < wb.x + wb.y) {
+            if (!bcnt) blo = b;
+            ++bcnt;
+        }
     }
-    double val = 0.0;
-    {
+    if (bcnt == 0) return;
+    const int i1 = P.two_i_min[0] + 2 * a1;
+    const int h0 = (p.jsum + i1 + P.two_k_base[0] + P.two_k_base[1] + P.two_k_base[2] + P.two_k_base[3]) >> 1;
+    double* ob = out + ((((long)b24 * c25 + b25) * n1 + a1) * P3 + q3) * ((long)V * c23 * n2);
+    const int per_v = bcnt * n2, total = vr.y * per_v;
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        const int vi = e / per_v, r2i = e - vi * per_v, bi = r2i / n2, i2 = r2i - bi * n2;
+        const int v = vr.x + vi, b23 = blo + bi, o23 = p.box.lo[0] + b23;
         const int blk = (o23 * nl + o24) * nl + o25;
         const SfKRange r2 = P.kr[0][blk];
         const int q2b = (r2.two_k_min - P.two_k_base[0]) >> 1;
-        const int i1 = P.two_i_min[0] + 2 * a1;
-        const int h0 = (p.jsum + i1 + P.two_k_base[0] + P.two_k_base[1] + P.two_k_base[2] + P.two_k_base[3]) >> 1;
         const double* s5 = P.S[4] + (((long)o25 * n1 + a1) * P2 + q2b) * NX + xg0 + v;
         const double* s4 = P.S[3] + ((((long)o23 * nl + o24) * P2 + q2b) * P3 + q3) * NX + xg0 + v;
         const double* b2 = sf_brow(P, 0, blk, i2) + q2b;
+        double val = 0.0;
         for (int c = 0; c < r2.n_k; ++c) {
             double term = (double)(r2.two_k_min + 2 * c + 1) * b2[c] * s5[(long)c * NX] * s4[(long)c * P3 * NX];
             if ((q2b + c) & 1) term = -term;
@@ -195,8 +207,8 @@ __device__ __forceinline__ void fz_g_entry(const FzParams& p, long n, double* __
         }
         val *= (double)(x0 + 2 * v + 1);
         if ((h0 + o23 + o24 + q3) & 1) val = -val;
+        ob[((long)v * c23 + b23) * n2 + i2] = val;
     }
-    out[e] = val;
 }
 
 // per k3: the l23 of the box that allow it (contiguous: |k3 - j13| <= l23 <= k3 + j13) and the (l34 l35) pairs that do
@@ -237,7 +249,7 @@ __device__ __forceinline__ void fz_lists_warp(const FzParams& p, int2* __restric
 // (the windows the lists and G need are recomputed in place: a handful of integer operations).
 struct FzPreArgs {
     long first[9];              // 0 G, 1 Z, 2 Bw4P / Bw4T, 3 Bw3T, 4 S3T, 5 windows, 6 lists, 7 scheduler counters; first[8] = all blocks
-    long nB4, padB4, nB3, nS3, padS3, nG;     // elements (pad: zeros behind the array, for whole-fragment reads)
+    long nB4, padB4, nB3, nS3, padS3;         // elements (pad: zeros behind the array, for whole-fragment reads)
     int gy, b4p;                // k4 split of the Z blocks; booster layout: Bw4P (1, k_fz_qp2 / k_fz_qp4) or Bw4T (0, k_fz_qp)
     int n_sched;
     double *Z, *B4, *B3, *S3, *G;
@@ -249,7 +261,7 @@ __global__ void __launch_bounds__(256) k_fz_pre(const __grid_constant__ FzParams
     const long b = blockIdx.x;
     const int tid = threadIdx.x;
     if (b < a.first[1]) {                                     // the heavy tasks first: their blocks must not start last
-        fz_g_entry(p, a.nG, a.G, (b - a.first[0]) * 256 + tid);
+        fz_g_block(p, a.G, b - a.first[0]);
     } else if (b < a.first[2]) {
         const long bz = b - a.first[1];
         fz_z_block(p, a.Z, bz / a.gy, (int)(bz % a.gy), a.gy);
@@ -1226,7 +1238,6 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             a.nB3 = nB3;
             a.nS3 = nS3;
             a.padS3 = padS3;
-            a.nG = nG;
             a.n_sched = 1024;
             a.Z = Z;
             a.B4 = B4;
@@ -1240,7 +1251,7 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             a.win23 = (int2*)lists;
             a.kl3 = lists + 2 * P3;
             a.sched = sched;
-            const long nb[8] = {(nG + 255) / 256, nz * a.gy, (a.nB4 + a.padB4 + 255) / 256, (nB3 + 255) / 256,
+            const long nb[8] = {c24 * c25 * n1 * P3, nz * a.gy, (a.nB4 + a.padB4 + 255) / 256, (nB3 + 255) / 256,
                                 (nS3 + padS3 + 255) / 256, (nl * nl + 255) / 256, (P3 + 7) / 8, 1};
             a.first[0] = 0;
             for (int t = 0; t < 8; ++t) a.first[t + 1] = a.first[t] + nb[t];
