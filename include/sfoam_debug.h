@@ -32,7 +32,9 @@ int sf_factor_work(const int two_j[10], int two_dl, double mac[6], double elems[
 long sf_slice_elems(const int two_j[10], int two_dl);
 
 /* FP64 roofline denominators measured in this process: TFLOP/s of dependent-chain microbenchmarks,
- * kind 0 = DFMA (vector FP64 fused multiply-add), kind 1 = DMMA (mma.sync m8n8k4 f64 on the tensor cores).
+ * kind 0 = DFMA (vector FP64 fused multiply-add), kind 1 = DMMA (mma.sync m8n8k4 f64 on the tensor cores), kind 2 = the inner
+ * loop of a shared-memory-fed GEMM (10 conflict-free LDS.64 per 16 DMMA, 16 warps per SM, nothing else): the practical ceiling
+ * of the gather-GEMM kernels, reported beside the peak, never used as the denominator.
  * Best of 5 launches of a few ms each; synchronises the default stream.  Requires sf_init. */
 int sf_fp64_peak(int kind, double *tflops);
 
@@ -64,6 +66,7 @@ void sf_set_factor_budget(unsigned long bytes);
 /* Kernel variants of the factorised path, for cross-checks and A/B timing: bit 0 = take the edge-3 contraction (R) through
  * the booster-stationary kernel (sf_factor_r.cu) instead of the general gather-GEMM; bit 1 = take Q/P through the first-generation kernel
  * (k_fz_qp); bit 2 = take Q/P through the second-generation kernel (k_fz_qp2) instead of the warp-autonomous one (k_fz_qp4).
+ * bit 3 = take R through the general gather-GEMM (k_fz_gemm<FzMapR>) instead of the producer-warp kernel (k_fz_r3).
  * 0 = default (the fastest kernels that hold the shape).  All variants compute the same sums. */
 void sf_set_factor_variant(int bits);
 /* The Q/P kernel the last factorised call (its last box) took: 1 = k_fz_qp, 2 = k_fz_qp2, 4 = k_fz_qp4; 0 before any call. */

@@ -291,3 +291,274 @@ int fz_launch_r2(const FzParams& p, const SfDims& D, int* sched, int n_sm, cudaS
     sf_count_launch(1);
     return SF_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// k_fz_r3: the same contraction, tile and occupancy as k_fz_gemm<FzMapR> (128 x 64, ring of two 32-row stages, two CTAs per SM), with
+// the loader taken out of the compute warps.  A microbenchmark of the bare inner loop (sf_fp64_peak kind 2: 10 conflict-free
+// LDS.64 per 16 DMMA, 16 warps per SM) reaches the full DMMA peak, so whatever k_fz_gemm<FzMapR> loses (0.67 pipe) it loses to
+// its loader code (~250 instructions per chunk and warp, 8-byte cp.async for the booster rows), its CTA barrier per chunk and
+// its epilogue.  Here
+//   * a ninth PRODUCER warp fills the ring: one bulk copy per row of P and one per booster row (the booster is stored windowed
+//     and padded, Bw3W[q3][pair][ldw], columns from the first l23 that allows k3: every tile row starts 16-byte aligned), rows
+//     between K and the next k-step boundary come from a zero row, completion on the stage's `full` mbarrier;
+//   * the eight CONSUMER warps run the inner loop, wait on `full` and release the stage through `empty`: no CTA barrier, no
+//     loader instruction, between the first and the last chunk of an item.
+// ---------------------------------------------------------------------------------------------------------------------------
+#define FZ3_KC 32
+#define FZ3_ST 2
+#define FZ3_BM 128
+#define FZ3_BN 64
+#define FZ3_LDA 132
+#define FZ3_LDB 68
+#define FZ3_NWC 8
+#define FZ3_THREADS (32 * (FZ3_NWC + 1))
+
+struct FzR3Args {
+    const double* Bw;             // Bw3W[q3][n-tile][kcap][FZ3_LDB]: the booster tile of every (k3, n-tile) as it sits in shared memory
+    int kcap;                     // rows per tile: the pairs (l34 l35) of the box rounded up to FZ3_KC (rows beyond the list: zeros)
+    int ntm, ntn;
+};
+
+// Bw3W[q3][nt][kk][c] = Bw3T[q3][pair kk of the list of k3][(first l23 that allows k3) n3 + 64 nt + c], 0 beyond the list, the window
+// and in the 4 padding columns: a 32-row chunk of a tile is ONE contiguous, 16-byte aligned block with the pitch of the ring
+__global__ void __launch_bounds__(256) k_fz_b3w(FzParams p, int kcap, int ntn, long n, double* __restrict__ out)
+{
+    const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const SfProblem& P = p.P;
+    const int n3 = P.n_i[2], c23 = p.box.cnt[0], c34 = p.box.cnt[3], c35 = p.box.cnt[4], npair = c34 * c35;
+    const int c = (int)(e % FZ3_LDB);
+    long r = e / FZ3_LDB;
+    const int kk = (int)(r % kcap); r /= kcap;
+    const int nt = (int)(r % ntn);
+    const int q3 = (int)(r / ntn);
+    const int2 win = p.win23[q3];
+    const int* list = p.kl3 + (long)q3 * (1 + npair);
+    const int col = nt * FZ3_BN + c;
+    double val = 0.0;
+    if (c < FZ3_BN && kk < list[0] && col < win.y * n3) val = p.Bw3T[((long)q3 * npair + list[1 + kk]) * (c23 * n3) + (long)win.x * n3 + col];
+    out[e] = val;
+}
+
+struct Fz3Job {
+    const double *as0, *bs0;      // this lane's fragment bases in stage 0 of the ring
+    unsigned full0, empty0;
+    double* C;                    // this lane's first entry of the first product (row warp 16 + g, column 0)
+    long sC;                      // products are sC apart
+    int NP, nsub, nchunks, K, N, lane, q;
+    bool mok0, mok1;              // rows g and 8 + g of the warp tile exist
+};
+
+// all chunks of all products of an item for a warp with TNA live column tiles and TMA row tiles
+template <int TNA, int TMA>
+__device__ __forceinline__ unsigned fz3_consume(const Fz3Job& J)
+{
+    double acc[TMA > 0 ? TMA : 1][TNA > 0 ? TNA : 1][2];
+#pragma unroll
+    for (int i = 0; i < (TMA > 0 ? TMA : 1); ++i)
+#pragma unroll
+        for (int j = 0; j < (TNA > 0 ? TNA : 1); ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    unsigned ndm = 0;
+    int it = 0;
+    for (int sub = 0; sub < J.nsub; ++sub) {
+        for (int c = 0; c < J.nchunks; ++c, ++it) {
+            const int s = it % FZ3_ST;
+            fz_mbar_wait(J.full0 + 8 * s, (unsigned)((it / FZ3_ST) & 1));
+            if (TMA > 0) {
+                const int ksn = min(FZ3_KC / 4, (J.K - c * FZ3_KC + 3) >> 2);
+                const double* as = J.as0 + s * FZ3_KC * FZ3_LDA;
+                const double* bs = J.bs0 + s * FZ3_KC * FZ3_LDB;
+#pragma unroll
+                for (int ks = 0; ks < FZ3_KC / 4; ++ks) {
+                    if (ks < ksn) {
+                        double av[TMA > 0 ? TMA : 1], bv[TNA > 0 ? TNA : 1];
+#pragma unroll
+                        for (int i = 0; i < TMA; ++i) av[i] = as[ks * 4 * FZ3_LDA + 8 * i];
+#pragma unroll
+                        for (int j = 0; j < TNA; ++j) bv[j] = bs[ks * 4 * FZ3_LDB + 8 * j];
+#pragma unroll
+                        for (int i = 0; i < TMA; ++i)
+#pragma unroll
+                            for (int j = 0; j < TNA; ++j) fz_dmma(acc[i][j][0], acc[i][j][1], av[i], bv[j]);
+                    }
+                }
+                ndm += (unsigned)(TMA * TNA * ksn);
+            }
+            __syncwarp();
+            if (J.lane == 0) fzr_mbar_arrive(J.empty0 + 8 * s);
+        }
+        // the product of this x: rows (l23 i3) of R, NP entries (i5 i4) each
+        if (TMA > 0) {
+            double* Cs = J.C + (long)sub * J.sC;
+#pragma unroll
+            for (int i = 0; i < TMA; ++i) {
+                const bool mok = i ? J.mok1 : J.mok0;
+#pragma unroll
+                for (int j = 0; j < TNA; ++j) {
+                    const int n = 8 * j + 2 * J.q;
+                    if (mok) {
+                        if (n < J.N) Cs[(long)n * J.NP + 8 * i] = acc[i][j][0];
+                        if (n + 1 < J.N) Cs[(long)(n + 1) * J.NP + 8 * i] = acc[i][j][1];
+                    }
+                    acc[i][j][0] = acc[i][j][1] = 0.0;
+                }
+            }
+        }
+    }
+    return ndm;
+}
+
+__global__ void __maxnreg__(112) k_fz_r3(const __grid_constant__ FzParams p, const __grid_constant__ FzR3Args a)
+{
+    extern __shared__ __align__(16) double smem[];
+    __shared__ __align__(8) unsigned long long bars[2 * FZ3_ST];     // full[ST], empty[ST]
+    const SfProblem& P = p.P;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
+    double* As = smem;                                        // [ST][KC][LDA]
+    double* Bs = As + FZ3_ST * FZ3_KC * FZ3_LDA;              // [ST][KC][LDB]
+    const unsigned full0 = fz_smem_u32(&bars[0]), empty0 = fz_smem_u32(&bars[FZ3_ST]);
+    const int n3 = P.n_i[2], n54 = P.n_i[3] * P.n_i[4], P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
+    const int c23 = p.box.cnt[0], c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
+    const int npair = c34 * c35;
+    // the item: (i1, l24, l25, k3, tile), every x of the triad (k3 l24 x) in turn
+    long item = blockIdx.x;
+    const int nt = (int)(item % a.ntn); item /= a.ntn;
+    const int mt = (int)(item % a.ntm); item /= a.ntm;
+    const int q3 = (int)(item % P3); item /= P3;
+    const int b25 = (int)(item % c25); item /= c25;
+    const int b24 = (int)(item % c24);
+    const int ac = (int)(item / c24);
+    int x0, nxs, xg0;
+    fz_xrange(P.two_i_min[0], P.two_j[J25], P.two_x_base, p.a_lo + ac, p.box.lo[2] + b25, x0, nxs, xg0);
+    const int2 win = p.win23[q3];
+    const int* list = p.kl3 + (long)q3 * (1 + npair);
+    const int2 vr = fz_vrange(P.two_j[J24] + 2 * (p.box.lo[1] + b24), P.two_k_base[1] + 2 * q3, x0, nxs);
+    const int m0 = mt * FZ3_BM, n0 = nt * FZ3_BN, N = min(FZ3_BN, win.y * n3 - n0), K = list[0];
+    const int M = (N > 0 && vr.y > 0) ? min(FZ3_BM, n54 - m0) : 0;
+    if (M <= 0) return;
+    const int nsub = vr.y, nchunks = (K + FZ3_KC - 1) / FZ3_KC;
+    const long slab = ((((long)ac * c24 + b24) * c25 + b25) * P3 + q3) * V + vr.x;
+    const double* A = p.Pq + slab * npair * NP + m0;          // product sub: + sub * npair * NP; row kk: + NP * list[1 + kk]
+    double* C = p.Rq + ((slab * c23 + win.x) * n3 + n0) * NP + m0;   // product sub: + sub * c23 n3 NP; entry (m, n): + n NP + m
+
+    for (int z = tid; z < FZ3_ST * FZ3_KC * (FZ3_LDA + FZ3_LDB); z += FZ3_THREADS) smem[z] = 0.0;   // rows never copied stay finite
+    if (tid == 0) {
+        for (int s = 0; s < FZ3_ST; ++s) {
+            fz_mbar_init(full0 + 8 * s, 1);
+            fz_mbar_init(empty0 + 8 * s, FZ3_NWC);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the zeroed ring is next written by bulk copies
+    __syncthreads();
+    if (nchunks == 0) {                                       // nothing to sum: the destination rows are exact zeros
+        for (int sub = 0; sub < nsub; ++sub)
+            for (int e = tid; e < M * N; e += FZ3_THREADS) C[(long)sub * c23 * n3 * NP + (long)(e / M) * NP + e % M] = 0.0;
+        return;
+    }
+    if (warp == FZ3_NWC) {
+        // ---------------- producer ----------------
+        const unsigned rowa = (unsigned)(((M + 1) & ~1) * 8);
+        const double* Bq = a.Bw + ((long)q3 * a.ntn + nt) * a.kcap * FZ3_LDB;       // the tile of this (k3, n-tile), chunk c at + c KC LDB
+        int it = 0;
+        for (int sub = 0; sub < nsub; ++sub) {
+            const double* Ap = A + (long)sub * npair * NP;
+            for (int c = 0; c < nchunks; ++c, ++it) {
+                const int s = it % FZ3_ST, k0 = c * FZ3_KC, kv = min(FZ3_KC, K - k0);
+                fz_mbar_wait(empty0 + 8 * s, (unsigned)(((it / FZ3_ST) & 1) ^ 1));
+                if (lane == 0) {
+                    fz_mbar_expect_tx(full0 + 8 * s, rowa * (unsigned)kv + 8u * FZ3_KC * FZ3_LDB);
+                    fz_bulk_g2s(fz_smem_u32(Bs + s * FZ3_KC * FZ3_LDB), Bq + (long)k0 * FZ3_LDB, 8u * FZ3_KC * FZ3_LDB, full0 + 8 * s);
+                }
+                __syncwarp();
+                if (lane < kv)
+                    fz_bulk_g2s(fz_smem_u32(As + (s * FZ3_KC + lane) * FZ3_LDA), Ap + (long)NP * __ldg(list + 1 + k0 + lane), rowa, full0 + 8 * s);
+            }
+        }
+        return;
+    }
+    // ---------------- consumers: warp tile 16 rows (i5 i4) x up to 64 columns (l23 i3) ----------------
+    const int NT = (N + 7) >> 3;
+    const int tma = (warp * 16 < M ? 1 : 0) + (warp * 16 + 8 < M ? 1 : 0);
+    Fz3Job job;
+    job.as0 = As + q * FZ3_LDA + warp * 16 + g;
+    job.bs0 = Bs + q * FZ3_LDB + g;
+    job.full0 = full0;
+    job.empty0 = empty0;
+    job.C = C + warp * 16 + g;
+    job.sC = (long)c23 * n3 * NP;
+    job.NP = NP;
+    job.nsub = nsub;
+    job.nchunks = nchunks;
+    job.K = K;
+    job.N = N;
+    job.mok0 = warp * 16 + g < M;
+    job.mok1 = warp * 16 + 8 + g < M;
+    job.lane = lane;
+    job.q = q;
+    unsigned ndm = 0;
+    // the whole loop exists once per shape of the warp tile (live column tiles 1..8, one or two row tiles): straight-line MMA code
+    if (tma == 2) {
+        switch (NT) {
+            case 8: ndm = fz3_consume<8, 2>(job); break;
+            case 7: ndm = fz3_consume<7, 2>(job); break;
+            case 6: ndm = fz3_consume<6, 2>(job); break;
+            case 5: ndm = fz3_consume<5, 2>(job); break;
+            case 4: ndm = fz3_consume<4, 2>(job); break;
+            case 3: ndm = fz3_consume<3, 2>(job); break;
+            case 2: ndm = fz3_consume<2, 2>(job); break;
+            default: ndm = fz3_consume<1, 2>(job); break;
+        }
+    } else if (tma == 1) {
+        switch (NT) {
+            case 8: ndm = fz3_consume<8, 1>(job); break;
+            case 7: ndm = fz3_consume<7, 1>(job); break;
+            case 6: ndm = fz3_consume<6, 1>(job); break;
+            case 5: ndm = fz3_consume<5, 1>(job); break;
+            case 4: ndm = fz3_consume<4, 1>(job); break;
+            case 3: ndm = fz3_consume<3, 1>(job); break;
+            case 2: ndm = fz3_consume<2, 1>(job); break;
+            default: ndm = fz3_consume<1, 1>(job); break;
+        }
+    } else {
+        ndm = fz3_consume<0, 0>(job);                         // no rows of the tile: keeps the barriers moving
+    }
+    if (p.cnt && lane == 0 && ndm) atomicAdd(p.cnt + 1, (unsigned long long)ndm);
+}
+
+/* Elements of the tile-major booster copy Bw3W for the box of p. */
+long fz_r3_b3w_elems(const FzParams& p, const SfDims& D, int* kcap)
+{
+    const int npair = p.box.cnt[3] * p.box.cnt[4], ntn = (p.box.cnt[0] * D.n_i[2] + FZ3_BN - 1) / FZ3_BN;
+    *kcap = (npair + FZ3_KC - 1) / FZ3_KC * FZ3_KC;
+    return (long)D.n_k_pad[1] * ntn * *kcap * FZ3_LDB;
+}
+
+/* Builds Bw3W (after k_fz_pre: it reads Bw3T, win23 and the lists) and launches k_fz_r3 for the pass described by p. */
+int fz_launch_r3(const FzParams& p, const SfDims& D, double* Bw3W, bool build, cudaStream_t st)
+{
+    FzR3Args a;
+    memset(&a, 0, sizeof a);
+    const long nW = fz_r3_b3w_elems(p, D, &a.kcap);
+    const int ntn_b = (p.box.cnt[0] * D.n_i[2] + FZ3_BN - 1) / FZ3_BN;
+    if (build) {
+        k_fz_b3w<<<(unsigned)((nW + 255) / 256), 256, 0, st>>>(p, a.kcap, ntn_b, nW, Bw3W);
+        sf_count_launch(1);
+    }
+    a.Bw = Bw3W;
+    const int n3 = D.n_i[2], n54 = D.n_i[3] * D.n_i[4];
+    a.ntm = (n54 + FZ3_BM - 1) / FZ3_BM;
+    a.ntn = (p.box.cnt[0] * n3 + FZ3_BN - 1) / FZ3_BN;
+    const long items = (long)a.ntn * a.ntm * D.n_k_pad[1] * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
+    if (items <= 0) return SF_OK;
+    if (items > 2147483647L) return SF_EARG;
+    const size_t smem = sizeof(double) * FZ3_ST * FZ3_KC * (FZ3_LDA + FZ3_LDB);
+    static bool attr = false;
+    if (!attr) {
+        if (cudaFuncSetAttribute(k_fz_r3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SF_ECUDA;
+        attr = true;
+    }
+    k_fz_r3<<<(unsigned)items, FZ3_THREADS, smem, st>>>(p, a);
+    sf_count_launch(1);
+    return SF_OK;
+}

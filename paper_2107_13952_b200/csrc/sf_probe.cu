@@ -42,10 +42,54 @@ __global__ void __launch_bounds__(256) k_peak_dmma(double* out, int iters, doubl
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
-// kind 0: DFMA (vector FP64 FMA), kind 1: DMMA (mma.sync m8n8k4 f64).  Best of 5 launches of ~10 ms each.
+// kind 2: the inner loop of a shared-memory-fed GEMM on the FP64 tensor cores, nothing else: per k-step a warp loads 2 A and 8 B
+// fragments (conflict-free LDS.64, row strides = 4 mod 16 doubles, as k_fz_gemm<FzMapR>) and issues 16 DMMA; 8 warps per CTA, two
+// CTAs per SM, no global traffic, no barrier.  What this reaches is the ceiling of such a loop, below the register-only chains
+// of kind 1: the MMA operands come through the shared-memory pipe.
+__global__ void __launch_bounds__(256, 2) k_peak_dmma_smem(double* out, int iters)
+{
+    extern __shared__ __align__(16) double probe_smem[];
+    double *As = probe_smem, *Bs = probe_smem + 32 * 132;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
+    for (int i = tid; i < 32 * 132; i += 256) As[i] = 1.0 + 1e-9 * i;
+    for (int i = tid; i < 32 * 68; i += 256) Bs[i] = 1e-9 * (i & 7);
+    __syncthreads();
+    double acc[2][8][2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    const double* as = As + q * 132 + warp * 16 + g;
+    const double* bs = Bs + q * 68 + g;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+            double a[2], b[8];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) a[i] = as[ks * 4 * 132 + 8 * i];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) b[j] = bs[ks * 4 * 68 + 8 * j];
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};\n"
+                                 : "+d"(acc[i][j][0]), "+d"(acc[i][j][1])
+                                 : "d"(a[i]), "d"(b[j]));
+        }
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += acc[i][j][0] + acc[i][j][1];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// kind 0: DFMA (vector FP64 FMA), kind 1: DMMA (mma.sync m8n8k4 f64), kind 2: DMMA fed from shared memory.  Best of 5 launches.
 extern "C" int sf_fp64_peak(int kind, double* tflops)
 {
-    if (!tflops || (kind != 0 && kind != 1)) return SF_EARG;
+    if (!tflops || kind < 0 || kind > 2) return SF_EARG;
     int dev = 0, n_sm = 0;
     SF_CUDA_OK(cudaGetDevice(&dev));
     SF_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
@@ -55,13 +99,18 @@ extern "C" int sf_fp64_peak(int kind, double* tflops)
     cudaEvent_t e0, e1;
     SF_CUDA_OK(cudaEventCreate(&e0));
     SF_CUDA_OK(cudaEventCreate(&e1));
+    if (kind == 2 &&
+        cudaFuncSetAttribute(k_peak_dmma_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double) * 32 * (132 + 68))) != cudaSuccess)
+        return SF_ECUDA;
     float best = 1e30f;
     for (int rep = 0; rep < 6; ++rep) {
         cudaEventRecord(e0, 0);
         if (kind == 0)
             k_peak_dfma<16><<<grid, 256>>>(out, iters, 1.0000001, 1e-9);
-        else
+        else if (kind == 1)
             k_peak_dmma<8><<<grid, 256>>>(out, iters, 1.0000001, 1e-9);
+        else
+            k_peak_dmma_smem<<<grid, 256, sizeof(double) * 32 * (132 + 68)>>>(out, iters / 16);
         cudaEventRecord(e1, 0);
         if (cudaEventSynchronize(e1) != cudaSuccess) return SF_ECUDA;
         float ms = 0;
@@ -70,7 +119,9 @@ extern "C" int sf_fp64_peak(int kind, double* tflops)
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    const double flop = kind == 0 ? 2.0 * 16 * iters * 256.0 * grid : 2.0 * 256 * 8 * iters * 8.0 * grid;
+    const double flop = kind == 0   ? 2.0 * 16 * iters * 256.0 * grid
+                        : kind == 1 ? 2.0 * 256 * 8 * iters * 8.0 * grid
+                                    : 512.0 * 128 * (iters / 16) * 8.0 * grid;   // 128 DMMA per warp and iteration, 512 flop each
     *tflops = flop / (best * 1e-3) / 1e12;
     return SF_OK;
 }

@@ -1095,13 +1095,15 @@ extern "C" int sf_last_dmma(double n[3])
 }
 
 int fz_launch_r2(const FzParams& p, const SfDims& D, int* sched, int n_sm, cudaStream_t st);   // sf_factor_r.cu
+long fz_r3_b3w_elems(const FzParams& p, const SfDims& D, int* kcap);
+int fz_launch_r3(const FzParams& p, const SfDims& D, double* Bw3W, bool build, cudaStream_t st);
 bool fz_qp2_supported(const FzParams& p, const SfDims& D);                                     // sf_factor_qp.cu
 long fz_qp2_b4p_elems(const FzParams& p, const SfDims& D);
 int fz_launch_qp2(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st);
 bool fz_qp4_supported(const FzParams& p, const SfDims& D);                                     // sf_factor_qp4.cu
 int fz_launch_qp4(const FzParams& p, const SfDims& D, const double* Bw4P, int* sched, int n_sm, cudaStream_t st);
 
-enum { FZ_SLOT_SCHED = 22, FZ_SLOT_CNT = 23, FZ_SLOT_WIN = 24, FZ_SLOT_LIST, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART };
+enum { FZ_SLOT_SCHED = 22, FZ_SLOT_CNT = 23, FZ_SLOT_WIN = 24, FZ_SLOT_LIST, FZ_SLOT_Z, FZ_SLOT_B4, FZ_SLOT_B3, FZ_SLOT_S3, FZ_SLOT_G, FZ_SLOT_P, FZ_SLOT_R, FZ_SLOT_PART, FZ_SLOT_B3W };
 
 int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st)
 {
@@ -1210,7 +1212,10 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             na = (na + 1) / 2;
         }
         int* lists = (int*)sf_scratch(FZ_SLOT_LIST, sizeof(int2) * P3 + sizeof(int) * (size_t)P3 * (1 + c34 * c35));
-        if (!Z || !B4 || !B3 || !S3 || !G || !Pq || !Rq || !lists) return SF_ENOMEM;
+        int ldw = 0;
+        const bool r3 = !(g_fz_variant & 9);             // R through the producer-warp kernel (bit 0: k_fz_r2, bit 3: the gather-GEMM)
+        double* B3W = r3 ? (double*)sf_scratch(FZ_SLOT_B3W, sizeof(double) * (size_t)fz_r3_b3w_elems(p, D, &ldw)) : nullptr;
+        if (!Z || !B4 || !B3 || !S3 || !G || !Pq || !Rq || !lists || (r3 && !B3W)) return SF_ENOMEM;
         p.win23 = (const int2*)lists;
         p.kl3 = lists + 2 * P3;
         p.Z = Z;
@@ -1281,7 +1286,8 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             }
             fz_ev_end(st);
             fz_ev_begin(1, st);
-            int rc = g_fz_variant & 1 ? fz_launch_r2(p, D, sched + 512 + pass, n_sm, st) : SF_EARG;         // booster block stationary, P streamed once
+            int rc = r3 ? fz_launch_r3(p, D, B3W, pass == 0, st)                                          // producer warp, bulk copies for both operands
+                        : g_fz_variant & 1 ? fz_launch_r2(p, D, sched + 512 + pass, n_sm, st) : SF_EARG;      // booster block stationary
             if (rc == SF_EARG) rc = fz_launch_gemm<FzMapR, 8, 1, 2, 8>(p, (int)(c34 * c35), st);   // shapes it does not hold
             fz_ev_end(st);
             if (rc != SF_OK) return rc;

@@ -130,7 +130,7 @@ def test_config3_blocks_and_ragged_ranges():
         assert_parity(Ag, Ao, Aabs, what=f"config 3 shells [{lo},{hi})")
 
 
-@pytest.mark.parametrize("bits", [pytest.param(1, id="R-booster-stationary"), pytest.param(2, id="qp-gen1"),
+@pytest.mark.parametrize("bits", [pytest.param(1, id="R-booster-stationary"), pytest.param(8, id="R-gather-gemm"), pytest.param(2, id="qp-gen1"),
                                   pytest.param(4, id="qp-gen2"), pytest.param(0, id="default")])
 def test_factorised_kernel_variants_against_the_oracle(bits):
     """Every kernel variant of the factorised path (sf_set_factor_variant, include/sfoam_debug.h: the fallbacks the
