@@ -46,7 +46,7 @@ PATH_NAMES = {1: "staged", 3: "line", 4: "factorised"}
 # DRAM traffic per launch comes from the committed ncu launch list of one config-3 step (every kernel of one
 # sf_vertex_amplitude call with dram__bytes_read.sum, dram__bytes_write.sum, gpu__time_duration.sum); null for other workloads
 NCU_LAUNCHES_CONFIG3 = os.path.join("profiles", "r2_config3_step_launches.csv")
-FZ_KERNELS = {"qp": "k_fz_qp", "R": "k_fz_gemm<FzMapR", "A": "k_fz_gemm<FzMapA", "R2": "k_fz_r2"}
+FZ_KERNELS = {"qp": ("k_fz_qp",), "R": ("k_fz_r3", "k_fz_r2", "k_fz_gemm<FzMapR"), "A": ("k_fz_gemm<FzMapA",)}
 UNIT = "shells/s"
 
 
@@ -308,7 +308,7 @@ def ncu_dram_per_step():
         name = r[k_name].split("(")[0].replace("void ", "")
         if not name.startswith(("k_fz_", "k_slices", "k_kranges")):
             continue                                  # the one-off {6j} table build is not part of a step
-        cls = next((c for c, pat in FZ_KERNELS.items() if name.startswith(pat)), "other")
+        cls = next((c for c, pats in FZ_KERNELS.items() if name.startswith(pats)), "other")
         n, tot = per.get(cls, (0, 0.0))
         seen.setdefault(cls, set()).add(r[k_id])
         per[cls] = (len(seen[cls]), tot + b)
@@ -520,7 +520,9 @@ def run_ours(args, cfg, rank, world, local_rank):
         # inequalities allow (host count, no padding).  The executed work (512 flop per issued DMMA.8x8x4, counted by the
         # kernels themselves, padding included) is reported as executed_over_useful, the padding tax.
         flop, mac, elems = factor_work(sf, two_j, two_dl)
-        names = {"qp": "k_fz_qp2 (Q = sum_l45, P = sum_k4)", "R": "k_fz_gemm<FzMapR> (R = sum_{l34 l35})",
+        qpk = {4: "k_fz_qp4", 2: "k_fz_qp2", 1: "k_fz_qp"}.get(sf.sf_last_qp_kernel(), "k_fz_qp")
+        rk = "k_fz_r2" if args.variant & 1 else "k_fz_gemm<FzMapR>" if args.variant & 8 else "k_fz_r3"
+        names = {"qp": qpk + " (Q = sum_l45, P = sum_k4)", "R": rk + " (R = sum_{l34 l35})",
                  "A": "k_fz_gemm<FzMapA> (A' = sum_{k3 x l23})"}
         per = {}
         for k, key in enumerate(("qp", "R", "A")):
