@@ -504,7 +504,9 @@ def run_ours(args, cfg, rank, world, local_rank):
     achieved = (f_con + f_asm) / (kern_ms * 1e-3) / 1e12
     peak_dfma, peak_dmma = sf.sf_fp64_peak(0), sf.sf_fp64_peak(1)
     peak = max(peak_dfma, peak_dmma)
-    peak_source = ("measured in this process: FP64 DFMA %.2f, DMMA(mma.sync m8n8k4) %.2f TFLOP/s" % (peak_dfma, peak_dmma))
+    peak_smem = sf.sf_fp64_peak(2)       # the bare shared-memory-fed MMA loop of the gather-GEMMs (10 LDS.64 per 16 DMMA): context, not the denominator
+    peak_source = ("measured in this process: FP64 DFMA %.2f, DMMA(mma.sync m8n8k4) %.2f TFLOP/s; a shared-memory-fed DMMA loop "
+                   "reaches %.2f" % (peak_dfma, peak_dmma, peak_smem))
     hbm, hbm_src = hbm_peak()
     # {6j} gathers (step 4): the S arrays, 8 B read from the table + 8 B written per element, over the event time of the stage
     n_s_elems = sf.sf_slice_elems(two_j, two_dl)
