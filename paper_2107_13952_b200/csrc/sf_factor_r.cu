@@ -304,24 +304,21 @@ int fz_launch_r2(const FzParams& p, const SfDims& D, int* sched, int n_sm, cudaS
 //   * the eight CONSUMER warps run the inner loop, wait on `full` and release the stage through `empty`: no CTA barrier, no
 //     loader instruction, between the first and the last chunk of an item.
 // ---------------------------------------------------------------------------------------------------------------------------
-#define FZ3_KC 32
-#define FZ3_ST 2
 #define FZ3_BM 128
 #define FZ3_BN 64
-#define FZ3_LDA 132
 #define FZ3_LDB 68
 #define FZ3_NWC 8
 #define FZ3_THREADS (32 * (FZ3_NWC + 1))
 
 struct FzR3Args {
     const double* Bw;             // Bw3W[q3][n-tile][kcap][FZ3_LDB]: the booster tile of every (k3, n-tile) as it sits in shared memory
-    int kcap;                     // rows per tile: the pairs (l34 l35) of the box rounded up to FZ3_KC (rows beyond the list: zeros)
+    int kcap;                     // rows per tile: the pairs (l34 l35) of the box rounded up to a multiple of 96 (rows beyond the list: zeros)
     int ntm, ntn;
 };
 
 // Bw3W[q3][nt][kk][c] = Bw3T[q3][pair kk of the list of k3][(first l23 that allows k3) n3 + 64 nt + c], 0 beyond the list, the window
 // and in the 4 padding columns: a 32-row chunk of a tile is ONE contiguous, 16-byte aligned block with the pitch of the ring
-__global__ void __launch_bounds__(256) k_fz_b3w(FzParams p, int kcap, int ntn, long n, double* __restrict__ out)
+__global__ void __launch_bounds__(256) k_fz_b3w(FzParams p, int kcap, int ntn, long n, double* __restrict__ out)   // kcap: multiple of the stage depth
 {
     const long e = blockIdx.x * (long)blockDim.x + threadIdx.x;
     if (e >= n) return;
@@ -350,7 +347,7 @@ struct Fz3Job {
 };
 
 // all chunks of all products of an item for a warp with TNA live column tiles and TMA row tiles
-template <int TNA, int TMA>
+template <int TNA, int TMA, int KC, int ST, int LDA>
 __device__ __forceinline__ unsigned fz3_consume(const Fz3Job& J)
 {
     double acc[TMA > 0 ? TMA : 1][TNA > 0 ? TNA : 1][2];
@@ -362,18 +359,18 @@ __device__ __forceinline__ unsigned fz3_consume(const Fz3Job& J)
     int it = 0;
     for (int sub = 0; sub < J.nsub; ++sub) {
         for (int c = 0; c < J.nchunks; ++c, ++it) {
-            const int s = it % FZ3_ST;
-            fz_mbar_wait(J.full0 + 8 * s, (unsigned)((it / FZ3_ST) & 1));
+            const int s = it % ST;
+            fz_mbar_wait(J.full0 + 8 * s, (unsigned)((it / ST) & 1));
             if (TMA > 0) {
-                const int ksn = min(FZ3_KC / 4, (J.K - c * FZ3_KC + 3) >> 2);
-                const double* as = J.as0 + s * FZ3_KC * FZ3_LDA;
-                const double* bs = J.bs0 + s * FZ3_KC * FZ3_LDB;
+                const int ksn = min(KC / 4, (J.K - c * KC + 3) >> 2);
+                const double* as = J.as0 + s * KC * LDA;
+                const double* bs = J.bs0 + s * KC * FZ3_LDB;
 #pragma unroll
-                for (int ks = 0; ks < FZ3_KC / 4; ++ks) {
+                for (int ks = 0; ks < KC / 4; ++ks) {
                     if (ks < ksn) {
                         double av[TMA > 0 ? TMA : 1], bv[TNA > 0 ? TNA : 1];
 #pragma unroll
-                        for (int i = 0; i < TMA; ++i) av[i] = as[ks * 4 * FZ3_LDA + 8 * i];
+                        for (int i = 0; i < TMA; ++i) av[i] = as[ks * 4 * LDA + 8 * i];
 #pragma unroll
                         for (int j = 0; j < TNA; ++j) bv[j] = bs[ks * 4 * FZ3_LDB + 8 * j];
 #pragma unroll
@@ -408,15 +405,19 @@ __device__ __forceinline__ unsigned fz3_consume(const Fz3Job& J)
     return ndm;
 }
 
+// KC rows per stage, ST stages, LDA = row pitch of the P rows in the ring (= 4 or 12 mod 16: conflict-free fragment loads).  Two
+// shapes: 3 x 24 rows at pitch 124 when a row of P (n5 n4 <= 122 entries) fits it -- the deeper ring covers the HBM latency that
+// 2 x 32 does not (consumers waiting on `full`: 16.2 -> 15.3 ms at config 3) -- else 2 x 32 at pitch 132
+template <int KC, int ST, int LDA>
 __global__ void __maxnreg__(112) k_fz_r3(const __grid_constant__ FzParams p, const __grid_constant__ FzR3Args a)
 {
     extern __shared__ __align__(16) double smem[];
-    __shared__ __align__(8) unsigned long long bars[2 * FZ3_ST];     // full[ST], empty[ST]
+    __shared__ __align__(8) unsigned long long bars[2 * ST];     // full[ST], empty[ST]
     const SfProblem& P = p.P;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
     double* As = smem;                                        // [ST][KC][LDA]
-    double* Bs = As + FZ3_ST * FZ3_KC * FZ3_LDA;              // [ST][KC][LDB]
-    const unsigned full0 = fz_smem_u32(&bars[0]), empty0 = fz_smem_u32(&bars[FZ3_ST]);
+    double* Bs = As + ST * KC * LDA;              // [ST][KC][LDB]
+    const unsigned full0 = fz_smem_u32(&bars[0]), empty0 = fz_smem_u32(&bars[ST]);
     const int n3 = P.n_i[2], n54 = P.n_i[3] * P.n_i[4], P3 = P.n_k_pad[1], V = p.V, NP = p.NP;
     const int c23 = p.box.cnt[0], c24 = p.box.cnt[1], c25 = p.box.cnt[2], c34 = p.box.cnt[3], c35 = p.box.cnt[4];
     const int npair = c34 * c35;
@@ -436,14 +437,14 @@ __global__ void __maxnreg__(112) k_fz_r3(const __grid_constant__ FzParams p, con
     const int m0 = mt * FZ3_BM, n0 = nt * FZ3_BN, N = min(FZ3_BN, win.y * n3 - n0), K = list[0];
     const int M = (N > 0 && vr.y > 0) ? min(FZ3_BM, n54 - m0) : 0;
     if (M <= 0) return;
-    const int nsub = vr.y, nchunks = (K + FZ3_KC - 1) / FZ3_KC;
+    const int nsub = vr.y, nchunks = (K + KC - 1) / KC;
     const long slab = ((((long)ac * c24 + b24) * c25 + b25) * P3 + q3) * V + vr.x;
     const double* A = p.Pq + slab * npair * NP + m0;          // product sub: + sub * npair * NP; row kk: + NP * list[1 + kk]
     double* C = p.Rq + ((slab * c23 + win.x) * n3 + n0) * NP + m0;   // product sub: + sub * c23 n3 NP; entry (m, n): + n NP + m
 
-    for (int z = tid; z < FZ3_ST * FZ3_KC * (FZ3_LDA + FZ3_LDB); z += FZ3_THREADS) smem[z] = 0.0;   // rows never copied stay finite
+    for (int z = tid; z < ST * KC * (LDA + FZ3_LDB); z += FZ3_THREADS) smem[z] = 0.0;   // rows never copied stay finite
     if (tid == 0) {
-        for (int s = 0; s < FZ3_ST; ++s) {
+        for (int s = 0; s < ST; ++s) {
             fz_mbar_init(full0 + 8 * s, 1);
             fz_mbar_init(empty0 + 8 * s, FZ3_NWC);
         }
@@ -464,15 +465,15 @@ __global__ void __maxnreg__(112) k_fz_r3(const __grid_constant__ FzParams p, con
         for (int sub = 0; sub < nsub; ++sub) {
             const double* Ap = A + (long)sub * npair * NP;
             for (int c = 0; c < nchunks; ++c, ++it) {
-                const int s = it % FZ3_ST, k0 = c * FZ3_KC, kv = min(FZ3_KC, K - k0);
-                fz_mbar_wait(empty0 + 8 * s, (unsigned)(((it / FZ3_ST) & 1) ^ 1));
+                const int s = it % ST, k0 = c * KC, kv = min(KC, K - k0);
+                fz_mbar_wait(empty0 + 8 * s, (unsigned)(((it / ST) & 1) ^ 1));
                 if (lane == 0) {
-                    fz_mbar_expect_tx(full0 + 8 * s, rowa * (unsigned)kv + 8u * FZ3_KC * FZ3_LDB);
-                    fz_bulk_g2s(fz_smem_u32(Bs + s * FZ3_KC * FZ3_LDB), Bq + (long)k0 * FZ3_LDB, 8u * FZ3_KC * FZ3_LDB, full0 + 8 * s);
+                    fz_mbar_expect_tx(full0 + 8 * s, rowa * (unsigned)kv + 8u * KC * FZ3_LDB);
+                    fz_bulk_g2s(fz_smem_u32(Bs + s * KC * FZ3_LDB), Bq + (long)k0 * FZ3_LDB, 8u * KC * FZ3_LDB, full0 + 8 * s);
                 }
                 __syncwarp();
                 if (lane < kv)
-                    fz_bulk_g2s(fz_smem_u32(As + (s * FZ3_KC + lane) * FZ3_LDA), Ap + (long)NP * __ldg(list + 1 + k0 + lane), rowa, full0 + 8 * s);
+                    fz_bulk_g2s(fz_smem_u32(As + (s * KC + lane) * LDA), Ap + (long)NP * __ldg(list + 1 + k0 + lane), rowa, full0 + 8 * s);
             }
         }
         return;
@@ -481,7 +482,7 @@ __global__ void __maxnreg__(112) k_fz_r3(const __grid_constant__ FzParams p, con
     const int NT = (N + 7) >> 3;
     const int tma = (warp * 16 < M ? 1 : 0) + (warp * 16 + 8 < M ? 1 : 0);
     Fz3Job job;
-    job.as0 = As + q * FZ3_LDA + warp * 16 + g;
+    job.as0 = As + q * LDA + warp * 16 + g;
     job.bs0 = Bs + q * FZ3_LDB + g;
     job.full0 = full0;
     job.empty0 = empty0;
@@ -500,28 +501,28 @@ __global__ void __maxnreg__(112) k_fz_r3(const __grid_constant__ FzParams p, con
     // the whole loop exists once per shape of the warp tile (live column tiles 1..8, one or two row tiles): straight-line MMA code
     if (tma == 2) {
         switch (NT) {
-            case 8: ndm = fz3_consume<8, 2>(job); break;
-            case 7: ndm = fz3_consume<7, 2>(job); break;
-            case 6: ndm = fz3_consume<6, 2>(job); break;
-            case 5: ndm = fz3_consume<5, 2>(job); break;
-            case 4: ndm = fz3_consume<4, 2>(job); break;
-            case 3: ndm = fz3_consume<3, 2>(job); break;
-            case 2: ndm = fz3_consume<2, 2>(job); break;
-            default: ndm = fz3_consume<1, 2>(job); break;
+            case 8: ndm = fz3_consume<8, 2, KC, ST, LDA>(job); break;
+            case 7: ndm = fz3_consume<7, 2, KC, ST, LDA>(job); break;
+            case 6: ndm = fz3_consume<6, 2, KC, ST, LDA>(job); break;
+            case 5: ndm = fz3_consume<5, 2, KC, ST, LDA>(job); break;
+            case 4: ndm = fz3_consume<4, 2, KC, ST, LDA>(job); break;
+            case 3: ndm = fz3_consume<3, 2, KC, ST, LDA>(job); break;
+            case 2: ndm = fz3_consume<2, 2, KC, ST, LDA>(job); break;
+            default: ndm = fz3_consume<1, 2, KC, ST, LDA>(job); break;
         }
     } else if (tma == 1) {
         switch (NT) {
-            case 8: ndm = fz3_consume<8, 1>(job); break;
-            case 7: ndm = fz3_consume<7, 1>(job); break;
-            case 6: ndm = fz3_consume<6, 1>(job); break;
-            case 5: ndm = fz3_consume<5, 1>(job); break;
-            case 4: ndm = fz3_consume<4, 1>(job); break;
-            case 3: ndm = fz3_consume<3, 1>(job); break;
-            case 2: ndm = fz3_consume<2, 1>(job); break;
-            default: ndm = fz3_consume<1, 1>(job); break;
+            case 8: ndm = fz3_consume<8, 1, KC, ST, LDA>(job); break;
+            case 7: ndm = fz3_consume<7, 1, KC, ST, LDA>(job); break;
+            case 6: ndm = fz3_consume<6, 1, KC, ST, LDA>(job); break;
+            case 5: ndm = fz3_consume<5, 1, KC, ST, LDA>(job); break;
+            case 4: ndm = fz3_consume<4, 1, KC, ST, LDA>(job); break;
+            case 3: ndm = fz3_consume<3, 1, KC, ST, LDA>(job); break;
+            case 2: ndm = fz3_consume<2, 1, KC, ST, LDA>(job); break;
+            default: ndm = fz3_consume<1, 1, KC, ST, LDA>(job); break;
         }
     } else {
-        ndm = fz3_consume<0, 0>(job);                         // no rows of the tile: keeps the barriers moving
+        ndm = fz3_consume<0, 0, KC, ST, LDA>(job);                         // no rows of the tile: keeps the barriers moving
     }
     if (p.cnt && lane == 0 && ndm) atomicAdd(p.cnt + 1, (unsigned long long)ndm);
 }
@@ -530,7 +531,7 @@ __global__ void __maxnreg__(112) k_fz_r3(const __grid_constant__ FzParams p, con
 long fz_r3_b3w_elems(const FzParams& p, const SfDims& D, int* kcap)
 {
     const int npair = p.box.cnt[3] * p.box.cnt[4], ntn = (p.box.cnt[0] * D.n_i[2] + FZ3_BN - 1) / FZ3_BN;
-    *kcap = (npair + FZ3_KC - 1) / FZ3_KC * FZ3_KC;
+    *kcap = (npair + 95) / 96 * 96;                          // a multiple of both stage depths (24 and 32)
     return (long)D.n_k_pad[1] * ntn * *kcap * FZ3_LDB;
 }
 
@@ -552,13 +553,19 @@ int fz_launch_r3(const FzParams& p, const SfDims& D, double* Bw3W, bool build, c
     const long items = (long)a.ntn * a.ntm * D.n_k_pad[1] * p.box.cnt[2] * p.box.cnt[1] * p.a_cnt;
     if (items <= 0) return SF_OK;
     if (items > 2147483647L) return SF_EARG;
-    const size_t smem = sizeof(double) * FZ3_ST * FZ3_KC * (FZ3_LDA + FZ3_LDB);
-    static bool attr = false;
-    if (!attr) {
-        if (cudaFuncSetAttribute(k_fz_r3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SF_ECUDA;
-        attr = true;
+    const bool deep = n54 <= 122;                             // a row of P fits the pitch of the 3 x 24 ring
+    const size_t smem = deep ? sizeof(double) * 3 * 24 * (124 + FZ3_LDB) : sizeof(double) * 2 * 32 * (132 + FZ3_LDB);
+    static bool attr[2] = {false, false};
+    if (!attr[deep]) {
+        const cudaError_t e = deep ? cudaFuncSetAttribute(k_fz_r3<24, 3, 124>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                                   : cudaFuncSetAttribute(k_fz_r3<32, 2, 132>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return SF_ECUDA;
+        attr[deep] = true;
     }
-    k_fz_r3<<<(unsigned)items, FZ3_THREADS, smem, st>>>(p, a);
+    if (deep)
+        k_fz_r3<24, 3, 124><<<(unsigned)items, FZ3_THREADS, smem, st>>>(p, a);
+    else
+        k_fz_r3<32, 2, 132><<<(unsigned)items, FZ3_THREADS, smem, st>>>(p, a);
     sf_count_launch(1);
     return SF_OK;
 }
