@@ -406,10 +406,10 @@ __device__ __forceinline__ unsigned fz3_consume(const Fz3Job& J)
 }
 
 // KC rows per stage, ST stages, LDA = row pitch of the P rows in the ring (= 4 or 12 mod 16: conflict-free fragment loads).  Two
-// shapes: 3 x 24 rows at pitch 124 when a row of P (n5 n4 <= 122 entries) fits it, else 2 x 32 at pitch 132.  Measured at config 3
-// (two runs each): 15.3 ms against 16.2 ms.  Stage count, stage depth and pitch changed together; the deeper ring is the
-// suspected cause (the 2 x 32 build's consumers waited on `full` for ~12 % of their cycles), not an isolated one: 4 x 16 rows at
-// pitch 132, the same 48 rows of lookahead, was slower (16.5 ms).  See profiles/r2_hot_kernels.md for the isolating runs.
+// shapes: 3 x 24 rows at pitch 124 when a row of P (n5 n4 <= 122 entries) fits it, else 2 x 32 at pitch 132.  Chosen by
+// measurement (config 3, bench.py, three runs): 15.3 ms against 16.1-16.2 ms.  The pitch is not the cause (2 x 32 at 124: 16.1;
+// 4 x 16 at 124 / 132: 16.4 / 16.5), and the mechanism is NOT identified: under ncu the share of mbarrier waits (11.5 %) and
+// the first-pass time are the same for both shapes (profiles/r2_hot_kernels.md).
 template <int KC, int ST, int LDA>
 __global__ void __maxnreg__(112) k_fz_r3(const __grid_constant__ FzParams p, const __grid_constant__ FzR3Args a)
 {
