@@ -55,7 +55,8 @@ typedef enum {
     SF_ESPIN    = -3,   /* a boundary node's four spins have an odd sum or an empty intertwiner range      */
     SF_ETABLE   = -4,   /* {6j} table requested but absent / too small                                     */
     SF_ENOMEM   = -5,   /* host or device allocation failed                                                */
-    SF_ECUDA    = -6    /* CUDA runtime error (no device, launch failure)                                  */
+    SF_ECUDA    = -6,   /* CUDA runtime error (no device, launch failure)                                  */
+    SF_ELIMIT   = -7    /* input larger than the fixed built-in scratch of an allocation-free entry point  */
 } sf_status;
 
 /* CUDA stream handle (a cudaStream_t), passed as an opaque pointer so that this header needs no CUDA include. */
@@ -149,6 +150,28 @@ int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const double *cons
  * SF_EARG on a null pointer, n < 0 or an n_i < 1. */
 int sf_contract_vertices(const double *a, const double *b, long n, double *result, sf_stream_t stream);
 int sf_contract_vectors(const double *A, const int n_i[5], const double *const psi[5], double *result, sf_stream_t stream);
+
+/* sf_contract_vertices for callers that cannot allocate device memory (Fig. 3: result[0] = sum_z a[z] b[z]).
+ * Meant for a program that calls the contraction inside a long loop (a sum or a Monte Carlo walk over bulk spins) while all
+ * device memory belongs to an allocator of its own (CUDA.jl's pool, PyTorch's caching allocator, a fixed MIG / MPS slice) --
+ * there a cudaMalloc made by this library fails or shrinks that pool -- or that cannot take the device-wide synchronisation
+ * cudaMalloc / cudaFree bring with them.  sf_contract_vertices gets its partial-sum buffer from the library's growable
+ * scratch; this entry point calls no cudaMalloc, no cudaFree and no other allocating routine, needs no sf_init, and keeps
+ * its partial sums in a fixed array built into the library's device code: 65 792 bytes that every GPU running this library
+ * holds until the process exits.
+ *   Limit: n <= sf_contract_noalloc_max_n() = 33 554 432 entries (one slot of the array per 4096 entries; 32^5, the
+ *     paper's largest tensors are 21^5).  Beyond it the call returns SF_ELIMIT and launches nothing.
+ *   a, b, result: DEVICE pointers, the caller's (n, n and 1 doubles); asynchronous, ordered on `stream`, on the CURRENT device.
+ *   First call on each device: looks up the device address of the built-in array (a one-off query that may make the CUDA
+ *     runtime load the library's device code).  Make that first call before any stream capture is begun.
+ *   The array is shared by all calls on a device and keeps the previous call's contents; each call re-zeroes the one word
+ *     that must start at zero, on `stream`, ahead of its kernel.  Calls that can overlap on the GPU (two streams with no
+ *     ordering between them, several host threads) race on the array and return wrong sums: keep them on one stream or
+ *     order them yourself.  The library's call guard (see Concurrency above) does NOT cover this entry point.
+ *   Bitwise reproducible for a given n; equal to sf_contract_vertices up to rounding (a different, also fixed, order).
+ * SF_EARG on a null pointer or n < 0, SF_ELIMIT on n above the limit, SF_ECUDA without a device. */
+int sf_contract_vertices_noalloc(const double *a, const double *b, long n, double *result, sf_stream_t stream);
+long sf_contract_noalloc_max_n(void);
 
 /* Number of kernels the library launched since sf_init / the last reset (bench.py's gpu_launches). */
 long sf_launch_count(int reset);

@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsfoam.so")
 
-SF_OK, SF_ENOTINIT, SF_EARG, SF_ESPIN, SF_ETABLE, SF_ENOMEM, SF_ECUDA = 0, -1, -2, -3, -4, -5, -6
+SF_OK, SF_ENOTINIT, SF_EARG, SF_ESPIN, SF_ETABLE, SF_ENOMEM, SF_ECUDA, SF_ELIMIT = 0, -1, -2, -3, -4, -5, -6, -7
 
 
 class SfError(RuntimeError):
@@ -67,6 +67,9 @@ def _lib():
         lib.sf_vertex_amplitude_batch.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                                   ctypes.c_void_p]
         lib.sf_contract_vertices.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
+        lib.sf_contract_vertices_noalloc.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_long, ctypes.c_void_p,
+                                                     ctypes.c_void_p]
+        lib.sf_contract_noalloc_max_n.restype = ctypes.c_long
         lib.sf_contract_vectors.argtypes = [ctypes.c_void_p, ctypes.c_int * 5, ctypes.c_void_p * 5, ctypes.c_void_p,
                                             ctypes.c_void_p]
         lib.sf_vertex_amplitude_host.argtypes = [_I10, ctypes.c_int, ctypes.c_void_p * 4, ctypes.c_void_p,
@@ -367,6 +370,22 @@ def sf_contract_vertices(a, b, result, stream=None):
     _check(_lib().sf_contract_vertices(_ptr(a), _ptr(b), ctypes.c_long(a.numel()), _ptr(result), _stream(stream)),
            "sf_contract_vertices")
     return result
+
+
+def sf_contract_vertices_noalloc(a, b, result, stream=None):
+    """sf_contract_vertices for a caller that cannot allocate device memory (all of it sits in the caller's own pool, or a
+    cudaMalloc's device-wide synchronisation is not acceptable where the call is made): the partial sums live in a fixed
+    65 792-byte array inside the library instead of cudaMalloc'd scratch.  a.numel() <= sf_contract_noalloc_max_n()
+    (33 554 432), else SfError with status SF_ELIMIT.  Needs no sf_init.  All calls on a device share that array: calls
+    that may overlap on the GPU race, keep them on one stream.  Make the first call on a device before any stream capture."""
+    _check(_lib().sf_contract_vertices_noalloc(_ptr(a), _ptr(b), ctypes.c_long(a.numel()), _ptr(result), _stream(stream)),
+           "sf_contract_vertices_noalloc")
+    return result
+
+
+def sf_contract_noalloc_max_n():
+    """Largest number of entries sf_contract_vertices_noalloc accepts."""
+    return int(_lib().sf_contract_noalloc_max_n())
 
 
 def sf_contract_vectors(A, psi, result, stream=None):

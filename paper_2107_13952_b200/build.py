@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsfoam.so")
-SOURCES = ["sf_api.cu", "sf_ranges.cpp", "sf_sixj.cu", "sf_slices.cu", "sf_vertex_staged.cu", "sf_vertex_line.cu", "sf_vertex_factor.cu", "sf_factor_r.cu", "sf_factor_qp.cu", "sf_factor_qp4.cu", "sf_vertex_batch.cu", "sf_contract.cu", "sf_probe.cu"]
+SOURCES = ["sf_api.cu", "sf_ranges.cpp", "sf_sixj.cu", "sf_slices.cu", "sf_vertex_staged.cu", "sf_vertex_line.cu", "sf_vertex_factor.cu", "sf_factor_r.cu", "sf_factor_qp.cu", "sf_factor_qp4.cu", "sf_vertex_batch.cu", "sf_contract.cu", "sf_contract_noalloc.cu", "sf_probe.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fno-fast-math", "--fmad=true",

@@ -153,6 +153,7 @@ extern "C" const char* sf_strerror(int status)
         case SF_ETABLE: return "6j table absent or too small";
         case SF_ENOMEM: return "out of memory";
         case SF_ECUDA: return "CUDA error (no device or launch failure)";
+        case SF_ELIMIT: return "input exceeds the fixed built-in scratch of this allocation-free entry point";
         default: return "unknown status";
     }
 }
