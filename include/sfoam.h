@@ -39,7 +39,15 @@
  * buffers and settings in that context.  Compute calls are therefore SERIALISED by the library: host threads by a mutex,
  * streams by an event -- a call on another stream than the previous call's first waits (on the device) for that call, so
  * two vertex calls on different streams are correct but do not overlap.  Calls are asynchronous on the stream they are
- * given.  Inside the caller's own stream capture the library adds no event: ordering is then the caller's graph.
+ * given.
+ *
+ * Stream capture: every compute entry point that works in the library's scratch -- the sf_vertex_amplitude* calls and
+ * sf_contract_vertices / sf_contract_vectors -- REFUSES a `stream` that the caller is capturing into a CUDA graph and returns
+ * SF_ECAPTURE before issuing any CUDA work (the capture stays valid and can be ended normally).  Reasons: the scratch blocks
+ * a captured launch would point to are freed or regrown by later calls; growing one synchronises the device and allocates,
+ * which invalidates a capture; the batch call copies its descriptors from host memory that is gone when the graph replays;
+ * and the serialisation above cannot order a replay against other calls.  For repeated identical calls use the library's own
+ * recordings (sf_set_graphs), which track all of that.
  */
 #ifndef SFOAM_H
 #define SFOAM_H
@@ -56,7 +64,8 @@ typedef enum {
     SF_ETABLE   = -4,   /* {6j} table requested but absent / too small                                     */
     SF_ENOMEM   = -5,   /* host or device allocation failed                                                */
     SF_ECUDA    = -6,   /* CUDA runtime error (no device, launch failure)                                  */
-    SF_ELIMIT   = -7    /* input larger than the fixed built-in scratch of an allocation-free entry point  */
+    SF_ELIMIT   = -7,   /* input larger than the fixed built-in scratch of an allocation-free entry point  */
+    SF_ECAPTURE = -8    /* `stream` is being captured by the caller (see Concurrency)                      */
 } sf_status;
 
 /* CUDA stream handle (a cudaStream_t), passed as an opaque pointer so that this header needs no CUDA include. */
@@ -199,7 +208,7 @@ int sf_last_path(void);
  * the same arguments (spins, Delta_l, ranges, booster and output POINTERS -- the booster VALUES are read when the kernels
  * run and may change) and unchanged library state, its launches are recorded into a CUDA graph, and every later repetition
  * is one graph launch on the caller's stream (config 0: 0.1 -> 0.03 ms per tensor).  The result is bit for bit the one of
- * the plain call.  A call made while the caller's stream is itself being captured is never recorded.  0 switches the
+ * the plain call.  (A call on a stream the caller is capturing is refused: SF_ECAPTURE.)  0 switches the
  * recordings off (every call launches its kernels one by one).  Always SF_OK. */
 int sf_set_graphs(int on);
 

@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsfoam.so")
 
-SF_OK, SF_ENOTINIT, SF_EARG, SF_ESPIN, SF_ETABLE, SF_ENOMEM, SF_ECUDA, SF_ELIMIT = 0, -1, -2, -3, -4, -5, -6, -7
+SF_OK, SF_ENOTINIT, SF_EARG, SF_ESPIN, SF_ETABLE, SF_ENOMEM, SF_ECUDA, SF_ELIMIT, SF_ECAPTURE = 0, -1, -2, -3, -4, -5, -6, -7, -8
 
 
 class SfError(RuntimeError):

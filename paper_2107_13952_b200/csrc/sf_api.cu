@@ -43,7 +43,7 @@ SfCallGuard::SfCallGuard(cudaStream_t s) : st(s), events(false)
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
         cudaGetLastError();
-        return;                        // inside the caller's own capture: ordering is the caller's graph
+        return;                        // (a captured stream never gets here: the entry points refuse it with SF_ECAPTURE)
     }
     events = true;
     if (g_ctx.have_last && g_ctx.last_stream != st) cudaStreamWaitEvent(st, g_ctx.done, 0);   // the scratch buffers are shared
@@ -56,6 +56,25 @@ SfCallGuard::~SfCallGuard()
         g_ctx.have_last = true;
     }
     g_call_mutex.unlock();
+}
+
+// True when `st` is inside a stream capture begun by the CALLER (the library's own recordings run on g_ctx.cap_stream and never
+// come through the extern "C" entry points).  Every entry point that uses the context's scratch refuses such a call: the
+// scratch blocks may be freed or regrown by a later call, a batch's descriptors are copied from host memory that is gone at
+// replay, growing a block calls cudaDeviceSynchronize / cudaFree / cudaMalloc (which invalidate the capture), and the call guard
+// orders nothing when the caller's graph replays.  The legacy stream queried while another stream captures in global mode
+// (cudaErrorStreamCaptureImplicit) counts as captured; without a context (no sf_init, no device) the answer is no and the
+// entry point reports its usual error.
+bool sf_stream_is_captured(cudaStream_t st)
+{
+    if (!g_ctx.init) return false;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    const cudaError_t e = cudaStreamIsCapturing(st, &cs);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return e == cudaErrorStreamCaptureImplicit;
+    }
+    return cs != cudaStreamCaptureStatusNone;
 }
 
 void sf_bump_generation(void) { ++g_ctx.gen; }
@@ -154,6 +173,7 @@ extern "C" const char* sf_strerror(int status)
         case SF_ENOMEM: return "out of memory";
         case SF_ECUDA: return "CUDA error (no device or launch failure)";
         case SF_ELIMIT: return "input exceeds the fixed built-in scratch of this allocation-free entry point";
+        case SF_ECAPTURE: return "the stream is being captured: this entry point uses library-owned scratch and cannot be recorded into a caller's CUDA graph";
         default: return "unknown status";
     }
 }
@@ -452,6 +472,7 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
 extern "C" int sf_vertex_amplitude(const int two_j[10], int two_dl, const sf_boosters* boosters, double* out,
                                    sf_stream_t stream)
 {
+    if (sf_stream_is_captured((cudaStream_t)stream)) return SF_ECAPTURE;
     SfCallGuard guard((cudaStream_t)stream);
     return vertex_range(two_j, two_dl, boosters, 0, 0, out, (cudaStream_t)stream, true);
 }
@@ -459,6 +480,7 @@ extern "C" int sf_vertex_amplitude(const int two_j[10], int two_dl, const sf_boo
 extern "C" int sf_vertex_amplitude_range(const int two_j[10], int two_dl, const sf_boosters* boosters, long shell_lo,
                                          long shell_hi, double* out, sf_stream_t stream)
 {
+    if (sf_stream_is_captured((cudaStream_t)stream)) return SF_ECAPTURE;
     SfCallGuard guard((cudaStream_t)stream);
     return vertex_range(two_j, two_dl, boosters, shell_lo, shell_hi, out, (cudaStream_t)stream, false);
 }
@@ -467,6 +489,7 @@ extern "C" int sf_vertex_amplitude_intertwiners(const int two_j[10], int two_dl,
                                                 const int i_first[5], const int i_count[5], double* out, sf_stream_t stream)
 {
     if (!i_first || !i_count) return SF_EARG;
+    if (sf_stream_is_captured((cudaStream_t)stream)) return SF_ECAPTURE;
     SfCallGuard guard((cudaStream_t)stream);
     return vertex_range(two_j, two_dl, boosters, 0, 0, out, (cudaStream_t)stream, true, i_first, i_count);
 }
@@ -485,6 +508,7 @@ extern "C" int sf_vertex_amplitude_batch(int n, const int* two_j, const int* two
     if (!g_ctx.init) return SF_ENOTINIT;
     if (n < 0 || (n > 0 && (!two_j || !two_dl || !boosters || !out))) return SF_EARG;
     if (n == 0) return SF_OK;
+    if (sf_stream_is_captured((cudaStream_t)stream)) return SF_ECAPTURE;   // (its descriptors are copied from host memory of this call)
     SfCallGuard guard((cudaStream_t)stream);
     return sf_vertex_batch_run(n, two_j, two_dl, boosters, out, (cudaStream_t)stream);
 }
@@ -495,6 +519,7 @@ extern "C" int sf_vertex_amplitude_host(const int two_j[10], int two_dl, const d
     if (!g_ctx.init) return SF_ENOTINIT;
     if (!two_j || !host_boosters || !host_out) return SF_EARG;
     cudaStream_t st = (cudaStream_t)stream;
+    if (sf_stream_is_captured(st)) return SF_ECAPTURE;
     SfCallGuard guard(st);
     SfDims D;
     int rc = sf_host_dims(two_j, two_dl, &D);

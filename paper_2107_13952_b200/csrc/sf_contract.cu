@@ -307,6 +307,7 @@ extern "C" int sf_contract_vertices(const double* a, const double* b, long n, do
 {
     if (!a || !b || !result || n < 0) return SF_EARG;
     cudaStream_t st = (cudaStream_t)stream;
+    if (sf_stream_is_captured(st)) return SF_ECAPTURE;
     SfCallGuard guard(st);
     const int grid = ke_grid(n);
     double* partial = (double*)sf_scratch(KE_SLOT_PART, sizeof(double) * 2 * KE_MAX_CTAS);
@@ -328,6 +329,7 @@ extern "C" int sf_contract_vectors(const double* A, const int n_i[5], const doub
     for (int e = 0; e < 5; ++e)
         if (n_i[e] < 1 || !psi[e]) return SF_EARG;
     cudaStream_t st = (cudaStream_t)stream;
+    if (sf_stream_is_captured(st)) return SF_ECAPTURE;
     SfCallGuard guard(st);
     const long rows = (long)n_i[0] * n_i[1] * n_i[2] * n_i[3];
     if (n_i[4] > KE_TILE || rows > 2147483647L) return SF_EARG;

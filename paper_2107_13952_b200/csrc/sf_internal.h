@@ -124,6 +124,7 @@ struct SfCallGuard {
     cudaStream_t st;
     bool events;
 };
+bool sf_stream_is_captured(cudaStream_t st);      // the caller is capturing `st`: entry points that use the scratch return SF_ECAPTURE
 void sf_bump_generation(void);                    // drops the recorded launch sequences (sf_api.cu): call when a setting they depend on changes
 bool sf_timing_on(void);
 bool sf_counting_on(void);
