@@ -138,9 +138,10 @@ int sf_vertex_amplitude_intertwiners(const int two_j[10], int two_dl, const sf_b
  * sf_vertex_amplitude.  two_j, two_dl, boosters and out are HOST arrays (of spins, of device-pointer quadruples and of device
  * pointers); they may be freed when the call returns.  Every tensor whose {6j} arrays and per-shell intermediates fit one SM's
  * shared memory (small spins, few shells) is computed by ONE kernel launch, one CTA per tensor, everything on chip; larger ones
- * are computed afterwards by the single-tensor path.  Asynchronous on `stream`; bitwise reproducible; uses no library scratch
- * for the small tensors, so batches on different streams may overlap.  All arguments are validated before anything is
- * launched: on SF_EARG / SF_ESPIN no output is written. */
+ * are computed afterwards by the single-tensor path.  Asynchronous on `stream`; bitwise reproducible.  Like every compute
+ * call it is serialised with the calls before it (Concurrency above): a batch issued on another stream than the previous
+ * call's waits for that call, so batches on different streams are correct but do not overlap.  All arguments are validated
+ * before anything is launched: on SF_EARG / SF_ESPIN no output is written. */
 int sf_vertex_amplitude_batch(int n, const int *two_j, const int *two_dl, const sf_boosters *boosters,
                               double *const *out, sf_stream_t stream);
 /* End-to-end variant with HOST buffers (pinned or pageable): copies the four boosters to the device, computes, copies
