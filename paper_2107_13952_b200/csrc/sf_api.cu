@@ -77,6 +77,9 @@ bool sf_stream_is_captured(cudaStream_t st)
     return cs != cudaStreamCaptureStatusNone;
 }
 
+SfHostLock::SfHostLock() { g_call_mutex.lock(); }
+SfHostLock::~SfHostLock() { g_call_mutex.unlock(); }
+
 void sf_bump_generation(void) { ++g_ctx.gen; }
 
 void sf_count_launch(int n) { g_ctx.launches += n; }
@@ -115,6 +118,7 @@ void sf_timing_mark(int idx, cudaStream_t st)
 
 extern "C" int sf_init(double gamma)
 {
+    SfHostLock lock;
     if (g_ctx.init) {
         g_ctx.gamma = gamma;
         return SF_OK;
@@ -141,6 +145,7 @@ static void sf_graph_cache_clear(void);
 
 extern "C" int sf_finalize(void)
 {
+    SfHostLock lock;
     if (!g_ctx.init) return SF_OK;
     cudaDeviceSynchronize();
     for (int s = 0; s < SF_NSCRATCH; ++s) {
@@ -181,6 +186,7 @@ extern "C" const char* sf_strerror(int status)
 extern "C" int sf_sixj_table(int two_jmax)
 {
     if (!g_ctx.init) return SF_ENOTINIT;
+    SfCallGuard guard(0);                  // a vertex call in flight on another stream may still be gathering from the old table
     ++g_ctx.gen;
     return sf_sixj_table_build(two_jmax, 0);
 }
@@ -194,18 +200,21 @@ extern "C" long sf_launch_count(int reset)
 
 extern "C" int sf_set_timing(int on)
 {
+    SfHostLock lock;
     g_ctx.timing = on != 0;
     ++g_ctx.gen;
     return SF_OK;
 }
 extern "C" int sf_set_counting(int on)
 {
+    SfHostLock lock;
     g_ctx.counting = on != 0;
     ++g_ctx.gen;
     return SF_OK;
 }
 extern "C" int sf_set_debug_poison(int on)
 {
+    SfHostLock lock;
     g_ctx.poison = on != 0;
     ++g_ctx.gen;
     return SF_OK;
@@ -220,6 +229,7 @@ extern "C" int sf_last_stage_ms(double ms[3])
 extern "C" int sf_set_path(int path)
 {
     if (path < 0 || path > 4 || path == 2) return SF_EARG;
+    SfHostLock lock;
     g_ctx.path = path;
     ++g_ctx.gen;
     return SF_OK;
@@ -380,6 +390,7 @@ static void sf_graph_cache_clear(void)
 /* 1 (default): repeated identical vertex calls replay a recorded launch sequence; 0: every call launches its kernels one by one. */
 extern "C" int sf_set_graphs(int on)
 {
+    SfHostLock lock;
     g_ctx.graphs = on != 0;
     ++g_ctx.gen;
     return SF_OK;
@@ -553,6 +564,7 @@ extern "C" int sf_vertex_terms(const int two_j[10], int two_dl, long shell_lo, l
     int rc = sf_host_dims(two_j, two_dl, &D);
     if (rc != SF_OK) return rc;
     if (shell_lo < 0 || shell_hi > D.n_shells || shell_lo > shell_hi) return SF_EARG;
+    SfCallGuard guard(0);                  // writes the shared k-range tables: ordered after a vertex call still reading them
     SfProblem P;
     rc = setup_problem(D, nullptr, P, 0);
     if (rc != SF_OK) return rc;

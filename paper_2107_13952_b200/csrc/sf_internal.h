@@ -116,13 +116,21 @@ bool sf_vertex_factor_supported(const SfDims& D);
 // scratch allocator owned by the context: grows on demand, freed by sf_finalize.  slot = small integer id.
 void* sf_scratch(int slot, size_t bytes);
 void sf_count_launch(int n);
-// Guard of every compute entry point of the C ABI: the library keeps ONE set of scratch buffers, so calls are serialised --
-// host threads by a mutex, streams by an event (a call on another stream than the previous call's first waits for that call).
+// Guard of every compute entry point of the C ABI (the vertex calls, the contractions, sf_vertex_terms, sf_sixj_table and
+// sf_sixj_batch / sf_sixj_get, the last three on the legacy stream): the library keeps ONE set of scratch buffers and one {6j}
+// table, so calls are serialised -- host threads by a mutex, streams by an event (a call on another stream than the previous
+// call's first waits for that call).  sf_contract_vertices_noalloc is outside it by design (sf_contract_noalloc.cu).
 struct SfCallGuard {
     explicit SfCallGuard(cudaStream_t st);
     ~SfCallGuard();
     cudaStream_t st;
     bool events;
+};
+// Host-side part of the guard alone (the mutex): for the setters, sf_init and sf_finalize, which change the state the compute
+// calls read (generation, graph cache, settings, table pointers) but launch nothing.
+struct SfHostLock {
+    SfHostLock();
+    ~SfHostLock();
 };
 bool sf_stream_is_captured(cudaStream_t st);      // the caller is capturing `st`: entry points that use the scratch return SF_ECAPTURE
 void sf_bump_generation(void);                    // drops the recorded launch sequences (sf_api.cu): call when a setting they depend on changes

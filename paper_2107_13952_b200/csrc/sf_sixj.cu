@@ -188,6 +188,7 @@ extern "C" int sf_sixj_batch(const int* two_j6, long n, int mode, double* host_o
         if (two_j6[q] < 0) return SF_EARG;
         if (two_j6[q] > jmax) jmax = two_j6[q];
     }
+    SfCallGuard guard(0);                                        // reads the table another thread's sf_sixj_table may replace
     if (mode == 1 && (g_tab_two_jmax < 0 || jmax > g_tab_two_jmax)) return SF_ETABLE;
     if (mode == 0 && jmax > SF_SIXJ_MAX_TWO_J) return SF_EARG;   // beyond the validated accuracy envelope (sf_internal.h)
     int* dargs = nullptr;

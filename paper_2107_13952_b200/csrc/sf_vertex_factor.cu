@@ -1028,12 +1028,14 @@ extern "C" int sf_last_qp_kernel(void) { return g_fz_last_qp; }
 static int g_fz_variant = 0;                         // sf_set_factor_variant: bit 0 = R through the booster-stationary kernel
 extern "C" void sf_set_factor_variant(int bits)
 {
+    SfHostLock lock;
     g_fz_variant = bits;
     sf_bump_generation();
 }
 static size_t g_fz_budget = 0;                       // sf_set_factor_budget: bytes for P and R of one pass (0 = a third of the device)
 extern "C" void sf_set_factor_budget(unsigned long bytes)
 {
+    SfHostLock lock;
     g_fz_budget = bytes;
     sf_bump_generation();
 }

@@ -175,6 +175,7 @@ void sf_launch_finalize(const SfProblem& P, long n_out, const double* acc, doubl
 static size_t g_staged_budget = (size_t)6 << 30;   // bytes for the two ping-pong buffers
 extern "C" void sf_set_staged_budget(unsigned long bytes)
 {
+    SfHostLock lock;
     g_staged_budget = bytes;
     sf_bump_generation();
 }
