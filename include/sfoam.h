@@ -205,10 +205,12 @@ int sf_set_path(int path);
  * disjoint, in ascending shell order, their union is the range.  SF_EARG on a bad range or an odd / negative two_dl. */
 int sf_shell_boxes(int two_dl, long shell_lo, long shell_hi, int boxes[16][12], int* n_boxes);
 int sf_last_path(void);
-/* Recorded launch sequences (default on).  A vertex call is 15-30 small kernel launches; the second time a call arrives with
- * the same arguments (spins, Delta_l, ranges, booster and output POINTERS -- the booster VALUES are read when the kernels
- * run and may change) and unchanged library state, its launches are recorded into a CUDA graph, and every later repetition
- * is one graph launch on the caller's stream (config 0: 0.1 -> 0.03 ms per tensor).  The result is bit for bit the one of
+/* Recorded launch sequences (default on).  A vertex call is 15-30 small kernel launches.  A call that ran without the library
+ * having to grow a scratch block is remembered; when it arrives again with the same arguments (spins, Delta_l, ranges, booster
+ * and output POINTERS -- the booster VALUES are read when the kernels run and may change) and unchanged library state, its
+ * launches are recorded into a CUDA graph, and every later repetition is one graph launch on the caller's stream (config 0:
+ * 0.1 -> 0.03 ms per tensor).  In a fresh context: call 1 allocates (plain), call 2 is remembered (plain), call 3 records and
+ * replays, calls 4.. replay.  The result is bit for bit the one of
  * the plain call.  (A call on a stream the caller is capturing is refused: SF_ECAPTURE.)  0 switches the
  * recordings off (every call launches its kernels one by one).  Always SF_OK. */
 int sf_set_graphs(int on);

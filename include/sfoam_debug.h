@@ -31,6 +31,11 @@ int sf_factor_work(const int two_j[10], int two_dl, double mac[6], double elems[
  * arguments.  Host integer function. */
 long sf_slice_elems(const int two_j[10], int two_dl);
 
+/* Number of vertex calls answered by replaying a recorded launch sequence (sf_set_graphs) since sf_init / the last reset:
+ * lets a test see that repeated identical calls do reach the recording (they never do while every call changes the library
+ * state, e.g. by re-growing a scratch block). */
+long sf_graph_replays(int reset);
+
 /* FP64 roofline denominators measured in this process: TFLOP/s of dependent-chain microbenchmarks,
  * kind 0 = DFMA (vector FP64 fused multiply-add), kind 1 = DMMA (mma.sync m8n8k4 f64 on the tensor cores), kind 2 = the inner
  * loop of a shared-memory-fed GEMM (10 conflict-free LDS.64 per 16 DMMA, 16 warps per SM, nothing else): the practical ceiling

@@ -47,6 +47,7 @@ def _lib():
         lib.sf_init.argtypes = [ctypes.c_double]
         lib.sf_sixj_table_slots.restype = ctypes.c_long
         lib.sf_launch_count.restype = ctypes.c_long
+        lib.sf_graph_replays.restype = ctypes.c_long
         lib.sf_sixj_batch.argtypes = [ctypes.c_void_p, ctypes.c_long, ctypes.c_int, ctypes.c_void_p]
         lib.sf_vertex_work.argtypes = [_I10, ctypes.c_int, ctypes.c_long, ctypes.c_long,
                                        ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_long),
@@ -189,6 +190,11 @@ def sf_set_staged_budget(nbytes):
 def sf_set_factor_variant(bits):
     """Kernel variants of the factorised path (include/sfoam_debug.h): 0 = default."""
     _lib().sf_set_factor_variant(int(bits))
+
+
+def sf_graph_replays(reset=False):
+    """Vertex calls answered by replaying a recorded launch sequence since sf_init / the last reset (debug hook)."""
+    return int(_lib().sf_graph_replays(1 if reset else 0))
 
 
 def sf_last_qp_kernel():

@@ -18,6 +18,7 @@ struct SfContext {
     void* scratch[SF_NSCRATCH] = {};
     size_t scratch_bytes[SF_NSCRATCH] = {};
     long launches = 0;
+    long replays = 0;      // vertex calls answered by a recorded launch sequence (sf_graph_replays)
     int path = 0;          // sf_set_path: 0 automatic, 1 staged, 3 line, 4 factorised
     int last_path = 0;
     bool timing = false;
@@ -107,6 +108,17 @@ void* sf_scratch(int slot, size_t bytes)
     return p;
 }
 
+// Gives a block back before its size is known to be wrong for what comes next (the pass-size loop of the factorised path).
+void sf_scratch_release(int slot)
+{
+    if (slot < 0 || slot >= SF_NSCRATCH || !g_ctx.scratch[slot] || g_ctx.capturing) return;
+    ++g_ctx.gen;
+    cudaDeviceSynchronize();
+    cudaFree(g_ctx.scratch[slot]);
+    g_ctx.scratch[slot] = nullptr;
+    g_ctx.scratch_bytes[slot] = 0;
+}
+
 bool sf_timing_on(void) { return g_ctx.timing; }
 bool sf_counting_on(void) { return g_ctx.counting; }
 bool sf_poison_on(void) { return g_ctx.poison; }
@@ -138,6 +150,7 @@ extern "C" int sf_init(double gamma)
     g_ctx.gamma = gamma;
     g_ctx.init = true;
     g_ctx.launches = 0;
+    g_ctx.replays = 0;
     return SF_OK;
 }
 
@@ -154,6 +167,7 @@ extern "C" int sf_finalize(void)
         g_ctx.scratch_bytes[s] = 0;
     }
     sf_graph_cache_clear();
+    sf_vertex_factor_forget();
     sf_sixj_module_free();
     for (int q = 0; q < 4; ++q) cudaEventDestroy(g_ctx.ev[q]);
     if (g_ctx.cap_stream) cudaStreamDestroy(g_ctx.cap_stream);
@@ -195,6 +209,14 @@ extern "C" long sf_launch_count(int reset)
 {
     long n = g_ctx.launches;
     if (reset) g_ctx.launches = 0;
+    return n;
+}
+
+extern "C" long sf_graph_replays(int reset)
+{
+    SfHostLock lock;
+    const long n = g_ctx.replays;
+    if (reset) g_ctx.replays = 0;
     return n;
 }
 
@@ -356,9 +378,11 @@ static int vertex_range_run(const int two_j[10], int two_dl, const sf_boosters* 
 // ---------------------------------------------------------------------------------------------------------------
 // Recorded launch sequences.  A vertex call is 15-30 small launches (k-range tables, S arrays, the precomputations and the
 // contractions of the factorised path); on small problems their launch latency is the whole cost (config 0: 0.1 ms for
-// 3.4e6 flop).  The second time a call comes with the same arguments (spins, Delta_l, ranges, booster and output POINTERS:
-// the booster values are read when the kernels run, so they may change) and the same library state, its launches are
-// recorded into a CUDA graph on a private stream; from then on the call is one graph launch on the caller's stream.
+// 3.4e6 flop).  A call that runs without changing the library state (no scratch block had to grow) is remembered; when it
+// comes again with the same arguments (spins, Delta_l, ranges, booster and output POINTERS: the booster values are read when
+// the kernels run, so they may change) and the same library state, its launches are recorded into a CUDA graph on a private
+// stream and replayed; from then on the call is one graph launch on the caller's stream.  In a fresh context that makes the
+// first call a plain run that allocates, the second a plain run that is remembered, the third the recording.
 // Anything a recording depends on (a scratch block reallocated, a setting changed, the {6j} table rebuilt) bumps the
 // generation and drops the recordings.  Measurement modes (timing, counting, poison) never use them.
 // ---------------------------------------------------------------------------------------------------------------
@@ -435,6 +459,7 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
     }
     if (hit && hit->exec) {
         if (cudaGraphLaunch(hit->exec, st) != cudaSuccess) return SF_ECUDA;
+        ++g_ctx.replays;
         g_ctx.launches += hit->launches;
         g_ctx.last_path = hit->last_path;
         return SF_OK;
@@ -448,7 +473,7 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
             if (g.exec) cudaGraphExecDestroy(g.exec);
             g = SfGraphEntry();
             g.used = true;
-            g.key = k;
+            memcpy(&g.key, &k, sizeof k);                     // byte copy: the key is compared with memcmp, padding included
         }
         return rc;
     }
@@ -470,6 +495,7 @@ static int vertex_range(const int two_j[10], int two_dl, const sf_boosters* boos
         hit->launches = recorded;
         hit->last_path = g_ctx.last_path;
         if (cudaGraphLaunch(hit->exec, st) != cudaSuccess) return SF_ECUDA;
+        ++g_ctx.replays;
         g_ctx.launches += recorded;
         return SF_OK;
     }

@@ -112,9 +112,11 @@ int sf_vertex_line(const SfDims& D, const SfProblem& P, long shell_lo, long shel
 bool sf_vertex_line_supported(const SfDims& D);
 int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long shell_hi, double* out, cudaStream_t st);
 bool sf_vertex_factor_supported(const SfDims& D);
+void sf_vertex_factor_forget(void);               // drops what the factorised path remembers about refused allocations (sf_finalize)
 
 // scratch allocator owned by the context: grows on demand, freed by sf_finalize.  slot = small integer id.
 void* sf_scratch(int slot, size_t bytes);
+void sf_scratch_release(int slot);                // frees the slot's block (synchronises the device); no-op while recording
 void sf_count_launch(int n);
 // Guard of every compute entry point of the C ABI (the vertex calls, the contractions, sf_vertex_terms, sf_sixj_table and
 // sf_sixj_batch / sf_sixj_get, the last three on the legacy stream): the library keeps ONE set of scratch buffers and one {6j}

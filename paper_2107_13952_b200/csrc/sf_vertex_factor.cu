@@ -1033,10 +1033,16 @@ extern "C" void sf_set_factor_variant(int bits)
     sf_bump_generation();
 }
 static size_t g_fz_budget = 0;                       // sf_set_factor_budget: bytes for P and R of one pass (0 = a third of the device)
+// Smallest P + R request (bytes of one pass) the device has refused so far (0 = none): later calls start below it instead of
+// repeating, on every call, a cudaDeviceSynchronize, a cudaFree and a cudaMalloc that fails -- and a generation bump that keeps
+// the call from ever being recorded.  Forgotten when the budget is set and by sf_finalize (the other tenant may be gone).
+static size_t g_fz_refused = 0;
+void sf_vertex_factor_forget(void) { g_fz_refused = 0; }
 extern "C" void sf_set_factor_budget(unsigned long bytes)
 {
     SfHostLock lock;
     g_fz_budget = bytes;
+    g_fz_refused = 0;
     sf_bump_generation();
 }
 
@@ -1207,10 +1213,14 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
         double* S3 = (double*)sf_scratch(FZ_SLOT_S3, sizeof(double) * (size_t)(nS3 + padS3));
         double* G = (double*)sf_scratch(FZ_SLOT_G, sizeof(double) * (size_t)nG);
         double *Pq = nullptr, *Rq = nullptr;
+        while (na > 1 && g_fz_refused && sizeof(double) * (size_t)((pP + pR) * na) >= g_fz_refused) na = (na + 1) / 2;
         for (;;) {                                   // other tenants of the device may hold memory: shrink the pass until it fits
             Pq = (double*)sf_scratch(FZ_SLOT_P, sizeof(double) * (size_t)(pP * na));
             Rq = Pq ? (double*)sf_scratch(FZ_SLOT_R, sizeof(double) * (size_t)(pR * na)) : nullptr;
             if ((Pq && Rq) || na == 1) break;
+            const size_t asked = sizeof(double) * (size_t)((pP + pR) * na);
+            if (!g_fz_refused || asked < g_fz_refused) g_fz_refused = asked;
+            if (Pq) sf_scratch_release(FZ_SLOT_P);   // P fitted, R did not: P's block of this size would starve the smaller R as well
             na = (na + 1) / 2;
         }
         int* lists = (int*)sf_scratch(FZ_SLOT_LIST, sizeof(int2) * P3 + sizeof(int) * (size_t)P3 * (1 + c34 * c35));
