@@ -96,8 +96,11 @@ int sf_sixj_table_two_jmax(void);
 /* Test hooks for {6j} parity.  two_j6 = (a b c d e f) for {a b c; d e f}; HOST pointers.
  * sf_sixj_get evaluates one symbol on the device (direct Racah sum).  sf_sixj_batch evaluates n symbols;
  * mode 0 = direct evaluation, mode 1 = gather from the resident table (SF_ETABLE if absent or an argument exceeds it).
- * Accuracy of the direct evaluation: relative 1e-12 for every 2j <= 150, ~1e-9 at 2j = 200; arguments above 2j = 256 are
- * refused (SF_EARG), and so is a vertex call whose largest {6j} label 2 * (max two_j + two_dl) exceeds 256. */
+ * Accuracy of the direct evaluation (double-double Racah sum) against the exact value: relative 1e-12 for every label
+ * 2j <= 240 -- measured: correctly rounded up to 2j ~ 176, <= 4e-15 up to 220, <= 2.5e-13 up to 244 on the symbols that cancel
+ * most (six near-equal large labels); from 248 on, symbols near a zero of the {6j} miss 1e-12.  Arguments above 2j = 240 are
+ * therefore refused (SF_EARG), and so is a vertex call whose largest {6j} label 2 * (max two_j + two_dl) exceeds 240: inside
+ * that bound every {6j} entering a vertex tensor is good to 1e-12 and the tensor meets 1e-11 * sum|terms|. */
 int sf_sixj_get(const int two_j6[6], double *host_out);
 int sf_sixj_batch(const int *two_j6, long n, int mode, double *host_out);
 

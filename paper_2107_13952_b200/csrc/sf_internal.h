@@ -78,10 +78,13 @@ __host__ __device__ inline void sf_triples(const int o[6], int nl, int t[4])
 // -------------------------------------------------------------------------------------------------------------
 // {6j} machinery (sf_sixj.cu)
 // -------------------------------------------------------------------------------------------------------------
-// Accuracy envelope of the double-double Racah sum (sf_sixj.cuh): relative 1e-12 for every argument 2j <= 150, degrading
-// to ~1e-9 at 2j = 200 (tests/test_gpu_sixj.py); beyond this bound the alternating sum cancels more than 106 bits resolve,
-// so larger arguments are refused (SF_EARG) instead of returning cancelled digits.
-#define SF_SIXJ_MAX_TWO_J 256
+// Accuracy envelope of the double-double Racah sum (sf_sixj.cuh), measured against the exact oracle on the symbols whose sum
+// cancels most (all six labels within 4 of 2j, every valid combination) and on random symbols (tests/test_gpu_sixj.py,
+// test_large_label_envelope): bit-identical to the correctly rounded value up to 2j ~ 176, relative error <= 4e-15 up to 220,
+// <= 2.5e-13 up to 244; from 2j = 248 on symbols close to a zero of the {6j} miss relative 1e-12 (2.7e-11 at 248, 8.7e-12
+// at 256, absolute error <= 2.5e-17).  The bound is the largest label for which relative 1e-12 has been demonstrated; larger
+// arguments are refused (SF_EARG) instead of returning cancelled digits.  Config 4 at lambda = 6 reaches 168.
+#define SF_SIXJ_MAX_TWO_J 240
 
 struct SfSixjTable {
     int two_jmax;            // -1 if absent

@@ -67,12 +67,39 @@ def test_large_spins_direct():
     rng = random.Random(150)
     args = [_random_valid(rng, 150) for _ in range(150)] + [(150,) * 6, (142, 84, 72, 60, 100, 96)]
     _check(args, sf.sf_sixj_batch(args, mode=0))
-    # beyond that the alternating sum cancels faster than double-double resolves: the accuracy degrades gracefully
     args = [(200,) * 6, (200, 180, 100, 160, 150, 150)]
-    _check(args, sf.sf_sixj_batch(args, mode=0), rel=1e-9)
+    _check(args, sf.sf_sixj_batch(args, mode=0))
     with pytest.raises(sf.SfError) as err:           # beyond the validated envelope: refused, not returned with cancelled digits
-        sf.sf_sixj_batch([(258,) * 6], mode=0)
+        sf.sf_sixj_batch([(242,) * 6], mode=0)
     assert err.value.status == sf.SF_EARG
+
+
+def test_large_label_envelope():
+    """The accuracy bound behind SF_SIXJ_MAX_TWO_J = 240 (include/sfoam.h): relative 1e-12 against the exact oracle up to the
+    largest accepted label.  Strata: for 2j = 152, 160, .., 240 every valid symbol whose six labels lie within 4 of 2j (the
+    Racah sum cancels most when all labels are large and comparable; 2025 symbols each), and 2000 random valid symbols per
+    band with labels in [2j/2, 2j] for 2j = 168 (the largest label of config 4 at lambda = 6), 200 and 240."""
+    rng = random.Random(240)
+    args = []
+    for J in range(152, 241, 8):
+        args += [t for t in itertools.product(range(J - 4, J + 1), repeat=6) if _valid(t)]
+    for J in (168, 200, 240):
+        got = 0
+        while got < 2000:
+            t = tuple(rng.randint(J // 2, J) for _ in range(2)) + (0,) + tuple(rng.randint(J // 2, J) for _ in range(2)) + (0,)
+            a, b, _, d, e, _ = t
+            cs = [c for c in range(abs(a - b), min(a + b, J) + 1, 2) if abs(d - e) <= c <= d + e and (d + e + c) % 2 == 0]
+            fs = [f for f in range(abs(a - e), min(a + e, J) + 1, 2) if abs(d - b) <= f <= d + b and (d + b + f) % 2 == 0]
+            if cs and fs:
+                args.append((a, b, rng.choice(cs), d, e, rng.choice(fs)))
+                got += 1
+    assert len(args) > 29000
+    exact = np.array(_exact_many(args, processes=16))
+    gpu = np.asarray(sf.sf_sixj_batch(args, mode=0))
+    zero = exact == 0.0
+    assert (np.abs(gpu[zero]) <= 1e-18).all()
+    rel = np.abs(gpu[~zero] - exact[~zero]) / np.abs(exact[~zero])
+    assert rel.max() <= 1e-12, (rel.max(), [args[i] for i in np.flatnonzero(~zero)][int(rel.argmax())])
 
 
 def test_table_gather_equals_exact_and_uses_symmetry():
