@@ -200,3 +200,40 @@ def test_threejm_against_sympy_and_orthogonality():
             tot = sum(wigner.threejm(j1, j2, j3, m1, -m3 - m1, m3) ** 2
                       for m1 in range(-j1, j1 + 1, 2) if abs(-m3 - m1) <= j2)
             assert (j3 + 1) * tot == pytest.approx(1.0, rel=1e-14)
+
+
+def test_sixj_class_representatives_by_brute_force():
+    """oracle/sixj_classes.c lists one symbol per class of the 24 tetrahedral symmetries.  Pin: for 2j <= 6 group ALL 7^6
+    label tuples with valid triads into orbits of the 24 images written out by hand here (column permutations, upper/lower
+    exchange in two columns) and take the largest image of each orbit: the same set, nothing twice; and every image of a
+    representative has the same exact value (the symmetries are symmetries of the symbol)."""
+    import itertools
+
+    from oracle import sixj_classes
+
+    def images(t):
+        a, b, c, d, e, f = t
+        cols = [(a, d), (b, e), (c, f)]
+        out = set()
+        for p in itertools.permutations(cols):
+            for fl in ((0, 0, 0), (1, 1, 0), (1, 0, 1), (0, 1, 1)):
+                out.add(tuple(p[q][fl[q]] for q in range(3)) + tuple(p[q][1 - fl[q]] for q in range(3)))
+        return out
+
+    J = 6
+    valid = [t for t in itertools.product(range(J + 1), repeat=6)
+             if is_triad(t[0], t[1], t[2]) and is_triad(t[0], t[4], t[5]) and is_triad(t[3], t[1], t[5])
+             and is_triad(t[3], t[4], t[2])]
+    want = {max(images(t)) for t in valid}
+    got = [tuple(int(v) for v in row) for row in sixj_classes.all_classes(J)]
+    assert len(got) == len(set(got)) == len(want) and set(got) == want
+    assert sum(len(images(t)) for t in want) == len(valid)            # the orbits partition the valid tuples
+    for t in got[::7]:
+        assert len({sixj_fixed(*im) for im in images(t)}) == 1
+    # a larger bound, counts only: every representative is valid, maximal among its images, and below the bound
+    J = 12
+    reps = sixj_classes.all_classes(J)
+    assert reps.max() <= J and reps.min() >= 0
+    for row in reps[::97]:
+        t = tuple(int(v) for v in row)
+        assert t == max(images(t)) and wigner.sixj_parts(*t)[1] != 0
