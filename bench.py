@@ -545,6 +545,7 @@ def run_ours(args, cfg, rank, world, local_rank):
                                 if dram else None),
                     "traffic_note": "DRAM bytes per launch of the dominant kernel (mean over its launches of one step)",
                     "traffic_source": dram["source"] if dram else None,
+                    "traffic_kind": "replayed: read from the committed ncu launch list named in traffic_source, NOT measured in this run" if dram else None,
                     "peak_source": peak_source,
                     "definition": "useful FP64 flop (2 x multiply-adds on valid index ranges, sf_factor_work) / CUDA-event time",
                     "kernels": per,
@@ -558,7 +559,10 @@ def run_ours(args, cfg, rank, world, local_rank):
                             "dram_bytes_per_step": dram["total"] if dram else None,
                             "dram_per_kernel": dram["per_kernel"] if dram else None,
                             "hbm_frac": dram["total"] / (ms_step * 1e-3) / 1e9 / hbm if dram else None,
-                            "peak": hbm, "peak_source": hbm_src, "source": dram["source"] if dram else None}}
+                            "peak": hbm, "peak_source": hbm_src, "source": dram["source"] if dram else None,
+                            "kind": ("replayed: dram_bytes_per_step / dram_per_kernel are read from the committed ncu launch list "
+                                     "in `source` (a capture of the same command on the same kernels), not measured in this run; "
+                                     "hbm_frac divides them by this run's time") if dram else None}}
     else:
         roofline = {"bound": "alu", "kernel": {3: "k_vertex_line"}.get(last_path, "k_stage_*"),
                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
