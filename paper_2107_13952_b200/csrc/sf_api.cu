@@ -26,6 +26,7 @@ struct SfContext {
     bool poison = false;
     cudaEvent_t ev[4] = {};
     double stage_ms[3] = {};
+    long epoch = 0;        // contexts created so far (sf_context_epoch): per-device caches of the other files are refilled when it moves
     long gen = 0;          // bumped by everything a recorded launch sequence depends on (scratch blocks, settings, the {6j} table)
     bool capturing = false;
     bool graphs = true;    // sf_set_graphs
@@ -82,6 +83,7 @@ SfHostLock::SfHostLock() { g_call_mutex.lock(); }
 SfHostLock::~SfHostLock() { g_call_mutex.unlock(); }
 
 void sf_bump_generation(void) { ++g_ctx.gen; }
+long sf_context_epoch(void) { return g_ctx.epoch; }
 
 void sf_count_launch(int n) { g_ctx.launches += n; }
 
@@ -149,6 +151,7 @@ extern "C" int sf_init(double gamma)
     g_ctx.have_last = false;
     g_ctx.gamma = gamma;
     g_ctx.init = true;
+    ++g_ctx.epoch;
     g_ctx.launches = 0;
     g_ctx.replays = 0;
     return SF_OK;

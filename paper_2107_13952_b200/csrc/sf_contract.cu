@@ -301,7 +301,9 @@ static int ke_grid(long work)
 }
 
 enum { KE_SLOT_TICKET = 20, KE_SLOT_PART = 21 };
-static unsigned* g_ke_ticket_zeroed = nullptr;         // the ticket block that has been zeroed (tickets return to 0 at the end of every call)
+// the ticket block that has been zeroed (tickets return to 0 at the end of every call); per context: the block of a new context
+// may come back at the old address with other contents
+static SfPerContext<unsigned*> g_ke_ticket_zeroed(nullptr);
 
 extern "C" int sf_contract_vertices(const double* a, const double* b, long n, double* result, sf_stream_t stream)
 {
@@ -313,9 +315,10 @@ extern "C" int sf_contract_vertices(const double* a, const double* b, long n, do
     double* partial = (double*)sf_scratch(KE_SLOT_PART, sizeof(double) * 2 * KE_MAX_CTAS);
     unsigned* ticket = (unsigned*)sf_scratch(KE_SLOT_TICKET, 64);
     if (!partial || !ticket) return SF_ENOMEM;
-    if (g_ke_ticket_zeroed != ticket) {
+    unsigned*& zeroed = g_ke_ticket_zeroed.get();
+    if (zeroed != ticket) {
         SF_CUDA_OK(cudaMemsetAsync(ticket, 0, 64, st));
-        g_ke_ticket_zeroed = ticket;
+        zeroed = ticket;
     }
     k_ke_dot<<<grid, KE_THREADS, 0, st>>>(a, b, n, partial, ticket + 1, result);
     sf_count_launch(1);
@@ -335,14 +338,16 @@ extern "C" int sf_contract_vectors(const double* A, const int n_i[5], const doub
     if (n_i[4] > KE_TILE || rows > 2147483647L) return SF_EARG;
     // warp-private bulk-copy pipeline: tiles of 32 rows are 16-byte sized and aligned (a shorter last tile is copied by hand)
     if (n_i[4] <= 48 && ((size_t)A & 15) == 0) {
-        static int n_sm = 0;
+        static SfPerContext<int> n_sm_c(0);
+        int& n_sm = n_sm_c.get();
         if (!n_sm) {
             int dev = 0;
             SF_CUDA_OK(cudaGetDevice(&dev));
             SF_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
         }
         const size_t smem = sizeof(double) * 2 * KE2_WARPS * KE2_ROWS * (size_t)n_i[4];
-        static size_t attr = 48 * 1024;
+        static SfPerContext<size_t> attr_c(48 * 1024);
+        size_t& attr = attr_c.get();
         if (smem > attr) {
             SF_CUDA_OK(cudaFuncSetAttribute(k_ke_vectors2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr = smem;
@@ -350,9 +355,10 @@ extern "C" int sf_contract_vectors(const double* A, const int n_i[5], const doub
         unsigned* ticket = (unsigned*)sf_scratch(KE_SLOT_TICKET, 64);
         double* part2 = (double*)sf_scratch(KE_SLOT_PART, sizeof(double) * 2 * KE_MAX_CTAS);
         if (!ticket || !part2) return SF_ENOMEM;
-        if (g_ke_ticket_zeroed != ticket) {
+        unsigned*& zeroed = g_ke_ticket_zeroed.get();
+        if (zeroed != ticket) {
             SF_CUDA_OK(cudaMemsetAsync(ticket, 0, 64, st));
-            g_ke_ticket_zeroed = ticket;
+            zeroed = ticket;
         }
         const long nt = (rows + KE2_ROWS - 1) / KE2_ROWS;
         const int per_sm = smem <= 100 * 1024 ? 2 : 1;

@@ -322,7 +322,8 @@ int fz_launch_qp2(const FzParams& p, const SfDims& D, const double* Bw4P, int* s
     a.n_items = (int)n_items;
     a.sched = sched;
     a.Bw4P = Bw4P;
-    static size_t attr = 0;
+    static SfPerContext<size_t> attr_c(0);
+    size_t& attr = attr_c.get();
     if (smem > attr) {
         if (cudaFuncSetAttribute(k_fz_qp2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SF_ECUDA;
         attr = smem;

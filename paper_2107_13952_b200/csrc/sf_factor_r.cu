@@ -281,7 +281,8 @@ int fz_launch_r2(const FzParams& p, const SfDims& D, int* sched, int n_sm, cudaS
     if (n_chunks > 2000000000L) return SF_EARG;
     a.n_chunks = (int)n_chunks;
     a.sched = sched;
-    static size_t attr = 0;
+    static SfPerContext<size_t> attr_c(0);
+    size_t& attr = attr_c.get();
     if (smem > attr) {
         if (cudaFuncSetAttribute(k_fz_r2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SF_ECUDA;
         attr = smem;
@@ -557,12 +558,13 @@ int fz_launch_r3(const FzParams& p, const SfDims& D, double* Bw3W, bool build, c
     if (items > 2147483647L) return SF_EARG;
     const bool deep = n54 <= 122;                             // a row of P fits the pitch of the 3 x 24 ring
     const size_t smem = deep ? sizeof(double) * 3 * 24 * (124 + FZ3_LDB) : sizeof(double) * 2 * 32 * (132 + FZ3_LDB);
-    static bool attr[2] = {false, false};
-    if (!attr[deep]) {
+    static SfPerContext<bool> attr_c[2] = {SfPerContext<bool>(false), SfPerContext<bool>(false)};
+    bool& attr_set = attr_c[deep].get();
+    if (!attr_set) {
         const cudaError_t e = deep ? cudaFuncSetAttribute(k_fz_r3<24, 3, 124>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
                                    : cudaFuncSetAttribute(k_fz_r3<32, 2, 132>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return SF_ECUDA;
-        attr[deep] = true;
+        attr_set = true;
     }
     if (deep)
         k_fz_r3<24, 3, 124><<<(unsigned)items, FZ3_THREADS, smem, st>>>(p, a);

@@ -137,6 +137,25 @@ struct SfHostLock {
     SfHostLock();
     ~SfHostLock();
 };
+// What a function caches about the device (SM count, memory size, "shared-memory attribute already raised" flags) holds for one
+// context only: sf_finalize + sf_init may continue on another device.  A cached value remembers the context it was filled in and
+// starts again from `init` in the next one.   static SfPerContext<int> c(0); int& n_sm = c.get();
+long sf_context_epoch(void);                      // number of contexts created so far (sf_init)
+template <class T>
+struct SfPerContext {
+    T value, init;
+    long epoch;
+    explicit SfPerContext(T i) : value(i), init(i), epoch(-1) {}
+    T& get()
+    {
+        const long e = sf_context_epoch();
+        if (epoch != e) {
+            value = init;
+            epoch = e;
+        }
+        return value;
+    }
+};
 bool sf_stream_is_captured(cudaStream_t st);      // the caller is capturing `st`: entry points that use the scratch return SF_ECAPTURE
 void sf_bump_generation(void);                    // drops the recorded launch sequences (sf_api.cu): call when a setting they depend on changes
 bool sf_timing_on(void);

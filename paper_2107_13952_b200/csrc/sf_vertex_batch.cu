@@ -301,7 +301,8 @@ int sf_vertex_batch_run(int n, const int* two_j, const int* two_dl, const sf_boo
         }
     }
     if (n_small > 0) {
-        static size_t attr = 48 * 1024;
+        static SfPerContext<size_t> attr_c(48 * 1024);
+        size_t& attr = attr_c.get();
         if (smem_max > attr) {
             SF_CUDA_OK(cudaFuncSetAttribute(k_vertex_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
             attr = smem_max;

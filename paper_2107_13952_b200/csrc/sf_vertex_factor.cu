@@ -1052,7 +1052,8 @@ static int fz_launch_gemm(const FzParams& p, int kcap, cudaStream_t st)
     constexpr int BM = WGM * TM * 8, BN = WGN * TN * 8;
     const size_t smem = sizeof(double) * Map::ST * Map::KC * (BM + 4 + BN + 4) + sizeof(int) * (2 * BM + 2 * BN + 240 + (size_t)kcap);
     if (smem > 226 * 1024) return SF_EARG;
-    static size_t attr = 0;
+    static SfPerContext<size_t> attr_c(0);
+    size_t& attr = attr_c.get();
     if (smem > attr) {
         if (cudaFuncSetAttribute(k_fz_gemm<Map, WGM, WGN, TM, TN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
             return SF_ECUDA;
@@ -1148,18 +1149,21 @@ int sf_vertex_factor(const SfDims& D, const SfProblem& P, long shell_lo, long sh
     p.w4A = w4A;
     p.w4B = w4B;
     p.Apart = Apart;
-    static bool qp_attr = false;
+    static SfPerContext<bool> qp_attr_c(false);
+    bool& qp_attr = qp_attr_c.get();
     if (!qp_attr) {
         if (cudaFuncSetAttribute(k_fz_qp, cudaFuncAttributeMaxDynamicSharedMemorySize, 201 * 1024) != cudaSuccess) return SF_ECUDA;
         qp_attr = true;
     }
-    static int n_sm = 0;
+    static SfPerContext<int> n_sm_c(0);
+    int& n_sm = n_sm_c.get();
     if (!n_sm) {
         int dev = 0;
         SF_CUDA_OK(cudaGetDevice(&dev));
         SF_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     }
-    static size_t total_b = 0;                       // device memory size: asked once (cudaMemGetInfo costs milliseconds)
+    static SfPerContext<size_t> total_b_c(0);        // device memory size: asked once per context (cudaMemGetInfo costs milliseconds)
+    size_t& total_b = total_b_c.get();
     if (!total_b) {
         size_t free_b = 0;
         if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return SF_ECUDA;

@@ -646,7 +646,8 @@ bool sf_vertex_line_supported(const SfDims& D) { return line_plan(D).ok; }
 template <int NT, int TPW>
 static int launch_line(const LinePlan& pl, int grid, cudaStream_t st)
 {
-    static bool attr_set = false;
+    static SfPerContext<bool> attr_set_c(false);
+    bool& attr_set = attr_set_c.get();
     if (!attr_set) {
         if (cudaFuncSetAttribute(k_vertex_line<NT, TPW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 226 * 1024) != cudaSuccess)
             return SF_ECUDA;
@@ -660,7 +661,8 @@ int sf_vertex_line(const SfDims& D, const SfProblem& P, long shell_lo, long shel
 {
     LinePlan pl = line_plan(D);
     if (!pl.ok) return SF_EARG;
-    static int n_sm = 0;
+    static SfPerContext<int> n_sm_c(0);
+    int& n_sm = n_sm_c.get();
     if (!n_sm) {
         int dev = 0;
         SF_CUDA_OK(cudaGetDevice(&dev));

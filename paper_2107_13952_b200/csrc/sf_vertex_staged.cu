@@ -193,7 +193,8 @@ int sf_vertex_staged(const SfDims& D, const SfProblem& P, long shell_lo, long sh
             const size_t b = sizeof(double) * (size_t)D.n_i[e + 1] * D.k_max[e];
             if (b > need) need = b;
         }
-        static size_t attr = 48 * 1024;
+        static SfPerContext<size_t> attr_c(48 * 1024);
+        size_t& attr = attr_c.get();
         if (need > 226 * 1024) return SF_EARG;       // a booster sub-matrix beyond one SM's shared memory: not held
         if (need > attr) {
             SF_CUDA_OK(cudaFuncSetAttribute(k_stage_mode, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need));

@@ -56,3 +56,42 @@ def test_refused_pass_size_is_remembered_and_calls_get_recorded():
         torch.cuda.empty_cache()
         sf.sf_init(wl.GAMMA)
         sf.sf_set_path(0)
+
+
+def test_a_new_context_after_finalize_starts_clean():
+    """sf_finalize + sf_init: what the library cached about the device and its scratch in the first context (SM count, memory
+    size, shared-memory attributes already raised, the zeroed ticket block of the contractions) is not carried over: all
+    paths, the batch call and both contractions give the same bits in the second context."""
+    cfg = wl.CONFIGS[0]
+    two_j, two_dl = cfg["two_j"], cfg["two_dl"]
+    Bdev = to_device(boosters_for(cfg))
+    _, n_i = sf.sf_vertex_dims(two_j)
+    st = torch.cuda.current_stream()
+    psi = [torch.full((n,), 0.5 + 0.25j, dtype=torch.complex128, device="cuda") for n in n_i]
+
+    def everything():
+        res = []
+        for path in (1, 3, 4):
+            sf.sf_set_path(path)
+            out = torch.full(tuple(n_i), float("nan"), dtype=torch.float64, device="cuda")
+            sf.sf_vertex_amplitude(two_j, two_dl, Bdev, out, st)
+            res.append(out)
+        sf.sf_set_path(0)
+        outb = torch.full(tuple(n_i), float("nan"), dtype=torch.float64, device="cuda")
+        sf.sf_vertex_amplitude_batch([two_j], [two_dl], [Bdev], [outb], st)
+        r1 = torch.zeros(1, dtype=torch.float64, device="cuda")
+        r2 = torch.zeros(2, dtype=torch.float64, device="cuda")
+        sf.sf_contract_vertices(res[0], outb, r1, st)
+        sf.sf_contract_vectors(res[0], psi, r2, st)
+        torch.cuda.synchronize()
+        return res + [outb, r1, r2]
+
+    sf.sf_init(wl.GAMMA)
+    first = everything()
+    sf.sf_finalize()
+    junk = torch.full((1 << 22,), 7.0, dtype=torch.float64, device="cuda")      # whatever the freed blocks held is overwritten
+    del junk
+    sf.sf_init(wl.GAMMA)
+    second = everything()
+    for a, b in zip(first, second):
+        assert torch.equal(a, b)
