@@ -423,6 +423,39 @@ def test_config3_full_tensor_against_the_cached_oracle_tensor(golden_dir):
         sf.sf_sixj_table(-1)
 
 
+@pytest.mark.parametrize("name", ["config2_dl8", "config4_lam1", "config4_lam2"])
+def test_secondary_workloads_full_tensor_against_the_cached_oracle_tensor(golden_dir, name):
+    """The other tensors bench.py times (its `other_workloads` rows), in full and entry by entry against the oracle: config 2
+    at Delta_l = 8 (all 9^6 = 531 441 shells) and config 4 at lambda = 1, 2 (all 7^6 = 117 649 shells each).  The files
+    tests/golden/<name>_full.npz are written by tests/golden/make_full_tensor.py from `oracle/` alone (exact-{6j} S arrays, long
+    double loops) and keyed by the hash of the inputs.  Automatic path (what bench.py runs), S arrays gathered from the table
+    and evaluated directly, at the tolerance of north_star."""
+    import hashlib
+    import os
+    f = os.path.join(golden_dir, name + "_full.npz")
+    assert os.path.exists(f), f"{f} is missing: run tests/golden/make_full_tensor.py"
+    z = np.load(f)
+    cfg = wl.config2(8) if name == "config2_dl8" else _config4(int(name[-1]))
+    B = boosters_for(cfg)
+    h = hashlib.sha256()
+    h.update(np.asarray(list(cfg["two_j"]) + [cfg["two_dl"]], dtype=np.int64).tobytes())
+    for edge in (2, 3, 4, 5):
+        h.update(np.ascontiguousarray(B[edge], dtype=np.float64).tobytes())
+    assert h.hexdigest() == str(z["input_sha256"]), "the cached oracle tensor was computed from different inputs"
+    Ao, Aabs = z["A"], z["Aabs"]
+    assert int(z["nonempty"]) > 0 and np.abs(Ao).max() > 0
+    Bdev = to_device(B)
+    sf.sf_set_path(0)
+    try:
+        for table in (60, -1):
+            sf.sf_sixj_table(table)
+            Ag = run_gpu(cfg["two_j"], cfg["two_dl"], B, Bdev=Bdev)
+            assert sf.sf_last_path() == 4                      # the factorised path, as in bench.py
+            assert_parity(Ag, Ao, Aabs, what=f"{name}, all shells, table {table}")
+    finally:
+        sf.sf_sixj_table(-1)
+
+
 def test_table_and_direct_slices_agree(path):
     """With a resident table the S arrays are gathered from it; the tensor must not change beyond rounding."""
     cfg = wl.config2(2)
