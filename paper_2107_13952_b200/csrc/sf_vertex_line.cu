@@ -695,6 +695,8 @@ int sf_vertex_line(const SfDims& D, const SfProblem& P, long shell_lo, long shel
     double* Zg = (double*)sf_scratch(19, sizeof(double) * (size_t)pl.z_doubles);
     double* Bw4g = (double*)sf_scratch(20, sizeof(double) * (size_t)pl.b4_doubles);
     if (!partial || !Zg || !Bw4g) return SF_ENOMEM;
+    // a unit without work writes no slice, and k_reduce_units adds every slice: start from zeros (recycled device memory is not)
+    SF_CUDA_OK(cudaMemsetAsync(partial, 0, sizeof(double) * (size_t)(lp.n_units > 0 ? lp.n_units : 1) * slice, st));
     lp.partial = partial;
     lp.Zg = Zg;
     lp.Bw4g = Bw4g;
