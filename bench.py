@@ -45,7 +45,7 @@ METRIC = "eprl_shells_contracted_per_s"
 PATH_NAMES = {1: "staged", 3: "line", 4: "factorised"}
 # DRAM traffic per launch comes from the committed ncu launch list of one config-3 step (every kernel of one
 # sf_vertex_amplitude call with dram__bytes_read.sum, dram__bytes_write.sum, gpu__time_duration.sum); null for other workloads
-NCU_LAUNCHES_CONFIG3 = os.path.join("profiles", "r2_config3_step_launches.csv")
+NCU_LAUNCHES_CONFIG3 = os.path.join("profiles", "r3_config3_step_launches.csv")
 FZ_KERNELS = {"qp": ("k_fz_qp",), "R": ("k_fz_r3", "k_fz_r2", "k_fz_gemm<FzMapR"), "A": ("k_fz_gemm<FzMapA",)}
 UNIT = "shells/s"
 
@@ -287,7 +287,7 @@ def hbm_peak():
 
 def ncu_dram_per_step():
     """{kernel class: (launches, bytes)} and the total, summed over all launches of one config-3 step, from the committed ncu
-    launch list (profiles/r2_config3_step_launches.csv: one row per launch and metric).  None if the file is absent."""
+    launch list (profiles/r3_config3_step_launches.csv: one row per launch and metric).  None if the file is absent."""
     import csv
     path = os.path.join(ROOT, NCU_LAUNCHES_CONFIG3)
     if not os.path.exists(path):
