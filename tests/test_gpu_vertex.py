@@ -423,7 +423,7 @@ def test_config3_full_tensor_against_the_cached_oracle_tensor(golden_dir):
         sf.sf_sixj_table(-1)
 
 
-@pytest.mark.parametrize("name", ["config2_dl8", "config4_lam1"])
+@pytest.mark.parametrize("name", ["config2_dl8", "config4_lam1", "config4_lam2"])
 def test_secondary_workloads_full_tensor_against_the_cached_oracle_tensor(golden_dir, name):
     """The other tensors bench.py times (its `other_workloads` rows), in full and entry by entry against the oracle: config 2
     at Delta_l = 8 (all 9^6 = 531 441 shells) and config 4 at lambda = 1, 2 (all 7^6 = 117 649 shells each).  The files
